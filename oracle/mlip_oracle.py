@@ -1,0 +1,431 @@
+"""float64 CPU ORACLE for the energy-and-force hot path (TEST INFRASTRUCTURE ONLY).
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference`
+legs may import this module. It shares no code with `paper_2509_21694_b200/` and never
+imports it. It is deliberately plain and slow: NumPy float64, no blocking, fusion or
+re-ordering beyond what the definitions below state (edges are only processed in chunks
+to bound memory; a chunk boundary changes nothing but the order of independent rows).
+
+What it computes (citations are PAPER.md lines; O1..O6 / R1..R19 are the readings listed
+in DESIGN.md, taken from SURVEY.md 8(c), because the paper treats the network as a black
+box):
+
+  O1  radius graph under periodic boundaries with local cutoff r_c
+  O2  Gaussian RBF x cosine envelope edge features                       BASELINE.json configs
+  O3  L message-passing layers, first L of L_max kept (MPDP)
+  O4  per-atom energy readout, E = sum_i E_i
+  O5  forces F = -grad E (hand-derived reverse mode)
+  O6  partition into spatial bins + halo; sum ROOT-node energies, sum the
+      gradients of root energies w.r.t. ALL sub-graph atoms
+
+The method (prune + partition + halo) reaches exactly the unpartitioned result
+(PAPER.md:165), so `energy_forces` IS the definition and `energy_forces_partitioned`
+restates the assembly rule. Pins (tests/test_oracle_*.py): brute-force O(N^2) neighbour
+lists, fcc shell counts, scipy cKDTree, finite differences, torch.float64 autograd,
+L=0 closed form, dimer closed form, invariances, partition equality + negative control,
+NVE energy conservation order. Nothing here is "parity unpinned".
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import numpy as np
+import scipy.sparse as sp
+from scipy.spatial import cKDTree
+from scipy.special import expit
+
+EDGE_CHUNK = 1 << 18
+
+
+# --------------------------------------------------------------------------------------
+# weights
+# --------------------------------------------------------------------------------------
+@dataclass
+class Model:
+    n_species: int
+    d: int
+    n_rbf: int
+    L_max: int
+    r_cut: float
+    agg_scale: float
+    T: np.ndarray
+    E0: np.ndarray
+    layers: list  # dicts W1,b1,W2,b2,V1,c1,V2,c2
+    Wo: np.ndarray
+    bo: np.ndarray
+    wo: np.ndarray
+    bE: float
+
+
+def parse_weights(n_species, d, n_rbf, L_max, r_cut, agg_scale, blob) -> Model:
+    """Blob order of include/mlip.h: T[S,d], E0[S], per layer W1[d,2d+k] (columns: receiver h_i,
+    sender h_j, e_hat), b1, W2[d,d], b2, V1[d,2d] (columns: h, m), c1, V2[d,d], c2; then
+    Wo[d,d], bo, wo, b_E. fp32 values are promoted to float64 unrounded (reading R15)."""
+    w = np.asarray(blob, dtype=np.float64)
+    pos = 0
+
+    def take(*shape):
+        nonlocal pos
+        n = int(np.prod(shape))
+        out = w[pos:pos + n].reshape(shape)
+        pos += n
+        return out
+
+    T = take(n_species, d)
+    E0 = take(n_species)
+    layers = []
+    for _ in range(L_max):
+        layers.append(dict(W1=take(d, 2 * d + n_rbf), b1=take(d), W2=take(d, d), b2=take(d),
+                           V1=take(d, 2 * d), c1=take(d), V2=take(d, d), c2=take(d)))
+    Wo = take(d, d); bo = take(d); wo = take(d); bE = float(take(1)[0])
+    assert pos == w.size, "weight blob size does not match the header"
+    return Model(n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), T, E0, layers, Wo, bo, wo, bE)
+
+
+# --------------------------------------------------------------------------------------
+# O1 graph
+# --------------------------------------------------------------------------------------
+def perpendicular_widths(cell):
+    """w_k = V / |a_i x a_j|: distance between the two faces of the cell normal to axis k."""
+    a1, a2, a3 = cell
+    vol = abs(np.dot(a1, np.cross(a2, a3)))
+    return np.array([vol / np.linalg.norm(np.cross(a2, a3)),
+                     vol / np.linalg.norm(np.cross(a3, a1)),
+                     vol / np.linalg.norm(np.cross(a1, a2))])
+
+
+def _canonical_d2(pos, cell, i, j, n):
+    """d^2 of the canonical predicate, in this operation order (reading R10):
+    t = (nx*a1 + ny*a2) + nz*a3 ; r = (x_j - x_i) + t ; d2 = (rx*rx + ry*ry) + rz*rz."""
+    nf = n.astype(np.float64)
+    t = (nf[:, 0:1] * cell[0][None, :] + nf[:, 1:2] * cell[1][None, :]) + nf[:, 2:3] * cell[2][None, :]
+    r = (pos[j] - pos[i]) + t
+    d2 = (r[:, 0] * r[:, 0] + r[:, 1] * r[:, 1]) + r[:, 2] * r[:, 2]
+    return r, d2
+
+
+def _canonical_sort(i, j, n):
+    order = np.lexsort((n[:, 2], n[:, 1], n[:, 0], j, i))
+    return i[order].astype(np.int32), j[order].astype(np.int32), n[order].astype(np.int32)
+
+
+def neighbor_list_bruteforce(pos, cell, r_cut):
+    """All directed edges (i <- j, n): d2 < r_cut^2 (strict), not (i == j and n == 0).
+    O(N^2 * images). Positions are used as given (unwrapped), n is relative to them."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    N = len(pos)
+    wk = perpendicular_widths(cell)
+    frac = pos @ np.linalg.inv(cell)
+    spread = np.ceil(frac.max(0) - frac.min(0)).astype(int) + 1 if N else np.zeros(3, int)
+    R = np.ceil(r_cut / wk).astype(int) + spread
+    ii, jj = np.meshgrid(np.arange(N), np.arange(N), indexing="ij")
+    ii = ii.ravel(); jj = jj.ravel()
+    out_i, out_j, out_n = [], [], []
+    rc2 = r_cut * r_cut
+    for nx in range(-R[0], R[0] + 1):
+        for ny in range(-R[1], R[1] + 1):
+            for nz in range(-R[2], R[2] + 1):
+                n = np.broadcast_to(np.array([nx, ny, nz]), (len(ii), 3))
+                _, d2 = _canonical_d2(pos, cell, ii, jj, n)
+                keep = d2 < rc2
+                if nx == 0 and ny == 0 and nz == 0:
+                    keep &= ii != jj
+                out_i.append(ii[keep]); out_j.append(jj[keep]); out_n.append(n[keep])
+    if not out_i:
+        return (np.zeros(0, np.int32),) * 2 + (np.zeros((0, 3), np.int32),)
+    return _canonical_sort(np.concatenate(out_i), np.concatenate(out_j), np.concatenate(out_n))
+
+
+def neighbor_list(pos, cell, r_cut):
+    """Same edge set as `neighbor_list_bruteforce`, found by a spatial search.
+
+    Candidates: wrap atoms into the cell, add every periodic image that lies within r_cut of
+    the cell, and ask a k-d tree (library routine) for all pairs within r_cut*(1+1e-9).
+    Acceptance: the canonical float64 predicate on the ORIGINAL positions, so the result does
+    not depend on how candidates were produced."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    N = len(pos)
+    if N == 0:
+        return (np.zeros(0, np.int32),) * 2 + (np.zeros((0, 3), np.int32),)
+    inv = np.linalg.inv(cell)
+    frac = pos @ inv
+    wrap = np.floor(frac).astype(np.int64)
+    fw = frac - wrap
+    wk = perpendicular_widths(cell)
+    margin = r_cut * (1.0 + 1e-6) / wk  # fractional thickness of the image shell
+    R = np.ceil(margin).astype(int)
+    img_j, img_n, img_x = [], [], []
+    base = fw @ cell
+    for nx in range(-R[0], R[0] + 1):
+        for ny in range(-R[1], R[1] + 1):
+            for nz in range(-R[2], R[2] + 1):
+                f = fw + np.array([nx, ny, nz], np.float64)
+                inside = np.all((f >= -margin) & (f <= 1.0 + margin), axis=1)
+                idx = np.nonzero(inside)[0]
+                if idx.size:
+                    img_j.append(idx)
+                    img_n.append(np.broadcast_to(np.array([nx, ny, nz]), (idx.size, 3)))
+                    img_x.append(base[idx] + np.array([nx, ny, nz], np.float64) @ cell)
+    img_j = np.concatenate(img_j); img_n = np.concatenate(img_n); img_x = np.concatenate(img_x)
+    tree_img = cKDTree(img_x)
+    tree_own = cKDTree(base)
+    coo = tree_own.sparse_distance_matrix(tree_img, r_cut * (1.0 + 1e-9), output_type="coo_matrix")
+    i = coo.row.astype(np.int64)
+    j = img_j[coo.col]
+    n = img_n[coo.col] - wrap[j] + wrap[i]  # shift relative to the unwrapped input positions
+    _, d2 = _canonical_d2(pos, cell, i, j, n)
+    keep = (d2 < r_cut * r_cut) & ~((i == j) & np.all(n == 0, axis=1))
+    return _canonical_sort(i[keep], j[keep], n[keep])
+
+
+def edge_vectors(pos, cell, recv, send, shift):
+    """r_e = (x_j - x_i) + n.C and its length, canonical operation order (O1)."""
+    r, d2 = _canonical_d2(np.asarray(pos, np.float64), np.asarray(cell, np.float64), recv, send, shift)
+    return r, np.sqrt(d2)
+
+
+# --------------------------------------------------------------------------------------
+# O2 features
+# --------------------------------------------------------------------------------------
+def envelope(r, r_cut):
+    """u(r) = (cos(pi r / r_cut) + 1) / 2 and u'(r)."""
+    x = np.pi * r / r_cut
+    return 0.5 * (np.cos(x) + 1.0), -(0.5 * np.pi / r_cut) * np.sin(x)
+
+
+def rbf(r, r_cut, n_rbf):
+    """g_k(r) = exp(-gamma (r - mu_k)^2), mu_k = k r_cut/(n_rbf-1), gamma = 1/(2 Delta^2),
+    Delta = r_cut/(n_rbf-1) (reading R8); returns g [E,k] and g' [E,k]."""
+    delta = r_cut / (n_rbf - 1)
+    mu = np.arange(n_rbf, dtype=np.float64) * delta
+    gamma = 0.5 / (delta * delta)
+    diff = r[:, None] - mu[None, :]
+    g = np.exp(-gamma * diff * diff)
+    return g, -2.0 * gamma * diff * g
+
+
+def silu(x):
+    return x * expit(x)
+
+
+def dsilu(x):
+    s = expit(x)
+    return s * (1.0 + x * (1.0 - s))
+
+
+# --------------------------------------------------------------------------------------
+# O3-O5 model
+# --------------------------------------------------------------------------------------
+def _scatter_matrix(index, n_rows, weights=None):
+    """Sparse [n_rows, len(index)] matrix S with S[index[e], e] = weights[e]; S @ X sums rows of
+    X into their targets (the scatter-sum of message passing as a library sparse product)."""
+    e = len(index)
+    data = np.ones(e) if weights is None else weights
+    return sp.csr_matrix((data, (index, np.arange(e))), shape=(n_rows, e))
+
+
+def _edge_layer_forward(model, lay, h, recv, send, r, want_cache=False):
+    """m_i = alpha sum_{e in in(i)} u(r_e) phi_e with
+    a_e = W1 [h_i || h_j || e_hat_e] + b1 ; s = SiLU(a) ; p = W2 s + b2 ; phi = SiLU(p)."""
+    N, d = h.shape
+    m = np.zeros((N, d))
+    for lo in range(0, len(recv), EDGE_CHUNK):
+        sl = slice(lo, lo + EDGE_CHUNK)
+        u, _ = envelope(r[sl], model.r_cut)
+        g, _ = rbf(r[sl], model.r_cut, model.n_rbf)
+        x = np.concatenate([h[recv[sl]], h[send[sl]], u[:, None] * g], axis=1)
+        a = x @ lay["W1"].T + lay["b1"]
+        p = silu(a) @ lay["W2"].T + lay["b2"]
+        phi = silu(p)
+        m += _scatter_matrix(recv[sl], N, model.agg_scale * u) @ phi
+    return m
+
+
+def forward(model, L, species, recv, send, r):
+    """h^0 = T[z]; L layers (O3); E_i = wo . SiLU(Wo h^L + bo) + b_E + E0[z] (O4).
+    Returns E_i and the per-layer node states needed by the reverse pass."""
+    assert 0 <= L <= model.L_max
+    h = model.T[species].copy()
+    hs, ms, cs = [], [], []
+    for l in range(L):
+        lay = model.layers[l]
+        m = _edge_layer_forward(model, lay, h, recv, send, r)
+        c = np.concatenate([h, m], axis=1) @ lay["V1"].T + lay["c1"]
+        hs.append(h); ms.append(m); cs.append(c)
+        h = h + silu(c) @ lay["V2"].T + lay["c2"]
+    o = h @ model.Wo.T + model.bo
+    E_i = silu(o) @ model.wo + model.bE + model.E0[species]
+    return E_i, dict(hs=hs, ms=ms, cs=cs, hL=h, o=o)
+
+
+def backward_rbar(model, L, species, recv, send, r, cache, omega):
+    """Reverse mode of sum_i omega_i E_i down to the per-edge scalar rbar_e = d(.)/d r_e (O5)."""
+    N = len(species)
+    d = model.d
+    hbar = omega[:, None] * ((model.wo * dsilu(cache["o"])) @ model.Wo)
+    rbar = np.zeros(len(recv))
+    for l in range(L - 1, -1, -1):
+        lay = model.layers[l]
+        h, c = cache["hs"][l], cache["cs"][l]
+        cbar = (hbar @ lay["V2"]) * dsilu(c)
+        hm = cbar @ lay["V1"]
+        hbar = hbar + hm[:, :d]
+        mbar = hm[:, d:]
+        hadd = np.zeros((N, d))
+        for lo in range(0, len(recv), EDGE_CHUNK):
+            sl = slice(lo, lo + EDGE_CHUNK)
+            ri, si = recv[sl], send[sl]
+            u, du = envelope(r[sl], model.r_cut)
+            g, dg = rbf(r[sl], model.r_cut, model.n_rbf)
+            x = np.concatenate([h[ri], h[si], u[:, None] * g], axis=1)
+            a = x @ lay["W1"].T + lay["b1"]
+            p = silu(a) @ lay["W2"].T + lay["b2"]
+            phi = silu(p)
+            mb = mbar[ri]
+            phibar = model.agg_scale * u[:, None] * mb
+            ubar = model.agg_scale * np.sum(mb * phi, axis=1)
+            pbar = phibar * dsilu(p)
+            sbar = pbar @ lay["W2"]
+            abar = sbar * dsilu(a)
+            xbar = abar @ lay["W1"]
+            hadd += _scatter_matrix(ri, N) @ xbar[:, :d]
+            hadd += _scatter_matrix(si, N) @ xbar[:, d:2 * d]
+            ebar = xbar[:, 2 * d:]
+            ubar = ubar + np.sum(ebar * g, axis=1)
+            rbar[sl] += ubar * du + np.sum(u[:, None] * ebar * dg, axis=1)
+        hbar = hbar + hadd
+    return rbar
+
+
+def forces_from_rbar(n_atoms, recv, send, rvec, r, rbar):
+    """F_k = sum_{e in in(k)} rbar_e rhat_e - sum_{e in out(k)} rbar_e rhat_e, rhat := 0 at r = 0
+    (reading R13), because d r_e / d x_send = rhat_e and d r_e / d x_recv = -rhat_e."""
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rhat = np.where(r[:, None] > 0.0, rvec / r[:, None], 0.0)
+    f_edge = rbar[:, None] * rhat
+    return _scatter_matrix(recv, n_atoms) @ f_edge - _scatter_matrix(send, n_atoms) @ f_edge
+
+
+def energy_forces(model, L, pos, cell, species, graph=None, omega=None, return_extra=False):
+    """E, E_i and F = -dE/dx of the unpartitioned model (the plain definition).
+    `omega` (default all ones) weights the per-atom energies in the differentiated sum."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    species = np.asarray(species)
+    if graph is None:
+        graph = neighbor_list(pos, cell, model.r_cut)
+    recv, send, shift = graph
+    rvec, r = edge_vectors(pos, cell, recv, send, shift)
+    E_i, cache = forward(model, L, species, recv, send, r)
+    if omega is None:
+        omega = np.ones(len(species))
+    rbar = backward_rbar(model, L, species, recv, send, r, cache, np.asarray(omega, np.float64))
+    F = forces_from_rbar(len(species), recv, send, rvec, r, rbar)
+    E = float(np.sum(omega * E_i))
+    if return_extra:
+        return E, E_i, F, dict(rbar=rbar, r=r, rvec=rvec, cache=cache, graph=graph)
+    return E, E_i, F
+
+
+# --------------------------------------------------------------------------------------
+# O6 partitioned evaluation
+# --------------------------------------------------------------------------------------
+def slab_axis(cell):
+    """Axis with the largest perpendicular width, ties -> lowest index (reading R3)."""
+    return int(np.argmax(perpendicular_widths(cell)))
+
+
+def partition_grid(pos, cell, grid, halo):
+    """Stage 1: uniform grid of P = gx*gy*gz bins on the unit cube; atom -> bin
+    by its wrapped scaled position, bin index min(floor(f*g), g-1) per axis.
+    Stage 2 (reading R2): extended set = atoms whose periodic distance to the bin interval is
+    <= halo along every axis (a superset of the K-hop BFS set of PAPER.md:165 when
+    halo >= K*r_cut). Returns a list of (owned_idx, ext_idx) with owned a subset of ext."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    frac = pos @ np.linalg.inv(cell)
+    f = frac - np.floor(frac)
+    wk = perpendicular_widths(cell)
+    g = np.asarray(grid, int)
+    bins = np.minimum(np.floor(f * g).astype(int), g - 1)
+    parts = []
+    for bx in range(g[0]):
+        for by in range(g[1]):
+            for bz in range(g[2]):
+                b = np.array([bx, by, bz])
+                owned = np.all(bins == b, axis=1)
+                ext = np.ones(len(pos), bool)
+                for k in range(3):
+                    lo, hi = b[k] / g[k], (b[k] + 1) / g[k]
+                    inside = (f[:, k] >= lo) & (f[:, k] < hi)
+                    below = np.mod(lo - f[:, k], 1.0)
+                    above = np.mod(f[:, k] - hi, 1.0)
+                    dist = np.where(inside, 0.0, np.minimum(below, above)) * wk[k]
+                    ext &= dist <= halo
+                ext |= owned
+                parts.append((np.nonzero(owned)[0], np.nonzero(ext)[0]))
+    return parts
+
+
+def partition_slabs(pos, cell, n_sub, halo):
+    g = [1, 1, 1]
+    g[slab_axis(cell)] = n_sub
+    return partition_grid(pos, cell, g, halo)
+
+
+def induced_subgraph(graph, ext_idx, n_atoms):
+    """Sub-graph of the GLOBAL graph induced on ext (edges keep their shifts)."""
+    recv, send, shift = graph
+    local = -np.ones(n_atoms, np.int64)
+    local[ext_idx] = np.arange(len(ext_idx))
+    keep = (local[recv] >= 0) & (local[send] >= 0)
+    return local[recv[keep]], local[send[keep]], shift[keep]
+
+
+def energy_forces_partitioned(model, L, pos, cell, species, parts, graph=None):
+    """E = sum_s sum_{i in own(s)} E_i^(s);  F = sum_s scatter_{k in ext(s)} of
+    -d( sum_{i in own(s)} E_i^(s) ) / d x_k   (reading R1)."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    species = np.asarray(species)
+    N = len(pos)
+    if graph is None:
+        graph = neighbor_list(pos, cell, model.r_cut)
+    E = 0.0
+    E_i = np.zeros(N)
+    F = np.zeros((N, 3))
+    stats = []
+    for owned, ext in parts:
+        lrecv, lsend, lshift = induced_subgraph(graph, ext, N)
+        omega = np.isin(ext, owned).astype(np.float64)
+        Es, Eis, Fs = energy_forces(model, L, pos[ext], cell, species[ext], (lrecv, lsend, lshift), omega)
+        E += Es
+        E_i[owned] += Eis[omega > 0]
+        F[ext] += Fs
+        stats.append(dict(n_owned=len(owned), n_ext=len(ext), n_edges=len(lrecv)))
+    return E, E_i, F, stats
+
+
+def halo_growth_factor(parts):
+    """H = (# atoms added by the halo) / (# root atoms), PAPER.md:289 (S1)."""
+    return [(len(ext) - len(owned)) / max(len(owned), 1) for owned, ext in parts]
+
+
+# --------------------------------------------------------------------------------------
+# short NVE run (pin only)
+# --------------------------------------------------------------------------------------
+ACC_UNIT = 9.648533e-3  # (eV/A)/amu -> A/fs^2
+
+
+def nve_velocity_verlet(model, L, pos, cell, species, masses, vel, dt, n_steps):
+    """Velocity-Verlet; returns total energy (potential + kinetic, eV) per step."""
+    pos = np.array(pos, np.float64); vel = np.array(vel, np.float64)
+    E, _, F = energy_forces(model, L, pos, cell, species)
+    out = []
+    for _ in range(n_steps):
+        kin = 0.5 * np.sum(masses[:, None] * vel * vel) / ACC_UNIT
+        out.append(E + kin)
+        vel += 0.5 * dt * ACC_UNIT * F / masses[:, None]
+        pos += dt * vel
+        E, _, F = energy_forces(model, L, pos, cell, species)
+        vel += 0.5 * dt * ACC_UNIT * F / masses[:, None]
+    kin = 0.5 * np.sum(masses[:, None] * vel * vel) / ACC_UNIT
+    out.append(E + kin)
+    return np.array(out)
