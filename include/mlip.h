@@ -1,0 +1,149 @@
+/*
+ * mlip.h -- C ABI of the B200-native energy-and-force hot path of
+ * "Scalable Foundation Interatomic Potentials via Message-Passing Pruning and Graph
+ * Partitioning" (arxiv 2509.21694; citations below are PAPER.md line numbers).
+ *
+ * The calls follow the paper's statement of the problem:
+ *   atoms + cell -> radius graph (r_c)                      mlip_build_graph
+ *   graph -> P spatial bins + halo of width K*r_c           mlip_partition / _grid
+ *   first K of M message-passing layers (MPDP) on every
+ *   extended sub-graph, sum root energies, sum gradients    mlip_energy_forces
+ *
+ * Conventions
+ *   - Every entry point returns 0 (MLIP_OK) or a negative mlip_status; it never throws,
+ *     aborts or exits. mlip_last_error(ctx) gives a human readable message for the last
+ *     failure on that context.
+ *   - "dev" pointers are CUDA device pointers on the context's device; "host" pointers are
+ *     ordinary host memory. The library never takes ownership of caller arrays; inputs are
+ *     only read during the call, outputs are fully overwritten.
+ *   - Work is enqueued on the stream given to mlip_ctx_create. Calls that return a host
+ *     scalar (build_graph: edge count; partition: sizes) synchronise that stream once.
+ *     mlip_energy_forces is asynchronous: its outputs are valid after the caller
+ *     synchronises the stream.
+ *   - Handles are owned by the library and released only by the matching *_destroy.
+ *   - Atom ids are int32; the number of directed edges must stay below 2^31.
+ *   - Everything runs in hand-written sm_100a kernels; there is no CPU fallback. If no
+ *     CUDA device is usable the calls fail with MLIP_ERR_CUDA.
+ */
+#ifndef MLIP_H_
+#define MLIP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  MLIP_OK = 0,
+  MLIP_ERR_INVALID_ARG = -1,
+  MLIP_ERR_UNSUPPORTED = -2,     /* singular / non-orthorhombic cell, d not in {64,128,256}, L > L_max ... */
+  MLIP_ERR_HALO_TOO_SMALL = -3,  /* halo < L*r_cut: refused rather than silently wrong forces */
+  MLIP_ERR_OUT_OF_MEMORY = -4,
+  MLIP_ERR_OVERFLOW = -5,        /* number of edges >= 2^31 or image shift outside [-127,127] */
+  MLIP_ERR_CUDA = -6
+} mlip_status;
+
+enum { MLIP_FP32 = 0, MLIP_BF16 = 1 };
+
+typedef struct mlip_ctx mlip_ctx;
+typedef struct mlip_model mlip_model;
+typedef struct mlip_graph mlip_graph;
+typedef struct mlip_part mlip_part;
+
+#define MLIP_MAGIC 0x50494c4du /* "MLIP" */
+
+/* Shape of the message-passing network (BASELINE.json configs; the paper treats the network
+ * as a black box, PAPER.md:23,151 -- the concrete equations are readings O2-O4 of DESIGN.md). */
+typedef struct {
+  uint32_t magic;     /* MLIP_MAGIC */
+  uint32_t version;   /* 1 */
+  int32_t n_species;  /* S */
+  int32_t d;          /* hidden width, one of 64, 128, 256 */
+  int32_t n_rbf;      /* number of Gaussian radial basis functions, 2..16 */
+  int32_t L_max;      /* M: number of message-passing layers stored in the blob */
+  float r_cut;        /* local cutoff r_c in Angstrom */
+  float agg_scale;    /* alpha multiplying the neighbour sum (reading R7) */
+  int32_t flags;      /* must be 0 (bit 0 reserved for the three-body variant) */
+  int32_t reserved[3];
+} mlip_model_header;
+
+/* Number of floats the weight blob must hold for a header. */
+size_t mlip_model_num_weights(const mlip_model_header* h);
+
+/* Create a context bound to CUDA device `device` and to `stream` (a cudaStream_t, may be
+ * NULL for the default stream). */
+int mlip_ctx_create(int device, void* stream, mlip_ctx** out);
+void mlip_ctx_destroy(mlip_ctx* ctx);
+const char* mlip_last_error(const mlip_ctx* ctx);
+
+/* Load a weight blob (HOST pointer, fp32, `n` floats, copied). Order, every matrix row-major
+ * [out,in]:  T[S,d], E0[S], then for each of the L_max layers
+ *   W1[d, 2d+n_rbf] (columns: receiver h_i | sender h_j | e_hat), b1[d], W2[d,d], b2[d],
+ *   V1[d, 2d] (columns: h | m), c1[d], V2[d,d], c2[d];   finally Wo[d,d], bo[d], wo[d], b_E. */
+int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const float* w_host, size_t n,
+                    mlip_model** out);
+void mlip_model_destroy(mlip_model* m);
+
+/* Radius graph under periodic boundaries, by a cell list built with a counting
+ * sort + prefix sum. Directed edge (i <- j, n) exists iff |x_j - x_i + n.C|^2 < r_cut^2
+ * (strict, float64, fixed operation order, reading R10) and not (i == j and n == 0).
+ *   pos_dev     [n_atoms,3] float64, device, unwrapped Cartesian positions (Angstrom)
+ *   cell_host   [3,3] float64, HOST, rows are the lattice vectors a1,a2,a3; must be
+ *               orthorhombic (diagonal) in this version, else MLIP_ERR_UNSUPPORTED (R12)
+ *   species_dev [n_atoms] int32, device, values in [0, n_species)
+ * The graph keeps its own (cell-sorted) copy of what it needs. */
+int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const double* cell_host,
+                     const int32_t* species_dev, int64_t n_atoms, double r_cut, mlip_graph** out);
+int mlip_graph_num_edges(const mlip_graph* g, int64_t* n_edges);
+/* Edge list in canonical order: lexicographic by (i, j, n_x, n_y, n_z) in the caller's atom
+ * numbering. recv_dev/send_dev [E] int32, shift_dev [E,3] int32, all device. */
+int mlip_graph_export_edges(mlip_ctx* ctx, const mlip_graph* g, int32_t* recv_dev,
+                            int32_t* send_dev, int32_t* shift_dev);
+void mlip_graph_destroy(mlip_graph* g);
+
+/* Spatial partition (PAPER.md:157 Stage 1: uniform grid of P bins on the scaled positions;
+ * Stage 2: every bin is extended so that each root atom keeps its K-hop
+ * neighbourhood -- here by the geometric halo: atoms whose periodic distance to the bin is
+ * <= halo along every axis, a superset of the K-hop BFS set when halo >= K*r_c, reading R2).
+ * mlip_partition cuts n_sub slabs along the axis of largest perpendicular width (R3). */
+int mlip_partition(mlip_ctx* ctx, const mlip_graph* g, int n_sub, double halo, mlip_part** out);
+int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* g, const int grid[3], double halo,
+                        mlip_part** out);
+int mlip_part_count(const mlip_part* p, int* n_sub);
+/* Sizes of sub-domain s: root (owned) atoms, extended atoms, induced directed edges. The halo
+ * growth factor of PAPER.md:289 is (n_ext - n_owned) / n_owned. */
+int mlip_part_info(const mlip_part* p, int s, int64_t* n_owned, int64_t* n_ext, int64_t* n_edges);
+void mlip_part_destroy(mlip_part* p);
+
+/* Energy and forces with the first L of L_max layers (MPDP).
+ * E = sum over sub-domains of the ROOT-atom energies; F = - sum over
+ * sub-domains of the gradient of that sub-domain's root energy w.r.t. ALL of its atoms
+ * (reading R1). part == NULL evaluates the whole box as one domain.
+ * Sub-domains are evaluated one after another on the context stream.
+ *   precision       MLIP_FP32 (fp32 CUDA-core contractions) or MLIP_BF16 (bf16 tensor-core
+ *                   contractions with fp32 accumulation; requires d = 256 or 128)
+ *   energy_dev      [1] float64, device
+ *   forces_dev      [n_atoms,3] float32, device, caller's atom numbering (eV/Angstrom)
+ *   atom_energy_dev [n_atoms] float32, device, or NULL
+ * Fails with MLIP_ERR_HALO_TOO_SMALL if part was built with halo < L*r_cut. */
+int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* m, int L, const mlip_graph* g,
+                       const mlip_part* part, int precision, double* energy_dev,
+                       float* forces_dev, float* atom_energy_dev);
+
+/* Whole step from HOST buffers: copies positions/species to the device, builds the graph,
+ * partitions (grid = {1,1,1} means one domain), evaluates, copies E and F back and
+ * synchronises. This is the call bench.py times for its end-to-end figure. */
+int mlip_step_host(mlip_ctx* ctx, const mlip_model* m, int L, const double* pos_host,
+                   const double* cell_host, const int32_t* species_host, int64_t n_atoms,
+                   const int grid[3], double halo, int precision, double* energy_host,
+                   float* forces_host);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MLIP_H_ */

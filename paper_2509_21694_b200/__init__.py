@@ -1,0 +1,8 @@
+"""B200-native (sm_100a) energy-and-force hot path of arxiv 2509.21694 behind a C ABI.
+
+`binding` is a thin ctypes layer over `libmlip_b200.so` (include/mlip.h): argument marshalling
+only, every step runs in the library's CUDA kernels. Importing this package does not load the
+library; the first call does, and fails loudly if it is missing or no B200 is present.
+"""
+from .binding import (MLIP_BF16, MLIP_FP32, Context, Graph, MlipError, Model, Partition, energy_forces,  # noqa: F401
+                      lib_path, load_library, step_host)

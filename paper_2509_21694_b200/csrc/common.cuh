@@ -1,0 +1,160 @@
+// Shared host-side definitions of the mlip B200 library: context, handles, error plumbing and
+// the declarations of the kernel launchers implemented in the other translation units.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "../../include/mlip.h"
+
+#define MLIP_CUDA_CHECK(ctx, expr)                                                        \
+  do {                                                                                    \
+    cudaError_t _e = (expr);                                                              \
+    if (_e != cudaSuccess) {                                                              \
+      (ctx)->set_error(std::string(#expr) + ": " + cudaGetErrorString(_e));               \
+      return _e == cudaErrorMemoryAllocation ? MLIP_ERR_OUT_OF_MEMORY : MLIP_ERR_CUDA;    \
+    }                                                                                     \
+  } while (0)
+
+#define MLIP_TRY(expr)              \
+  do {                              \
+    int _s = (expr);                \
+    if (_s != MLIP_OK) return _s;   \
+  } while (0)
+
+struct mlip_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  int num_sms = 148;
+  std::string err;
+  int64_t launches = 0;
+  void set_error(const std::string& s) { err = s; }
+  // stream-ordered allocation (pool keeps memory between steps)
+  template <class T>
+  int alloc(T** p, size_t n) {
+    *p = nullptr;
+    if (n == 0) n = 1;
+    cudaError_t e = cudaMallocAsync((void**)p, n * sizeof(T), stream);
+    if (e != cudaSuccess) {
+      set_error(std::string("cudaMallocAsync: ") + cudaGetErrorString(e));
+      cudaGetLastError();
+      return MLIP_ERR_OUT_OF_MEMORY;
+    }
+    return MLIP_OK;
+  }
+  void free(void* p) {
+    if (p) cudaFreeAsync(p, stream);
+  }
+};
+
+// ---- model --------------------------------------------------------------------------------
+struct LayerWeights {
+  // fp32 device pointers into the blob copy (row-major [out,in])
+  const float *W1, *b1, *W2, *b2, *V1, *c1, *V2, *c2;
+  // derived fp32 matrices (device, owned by the model)
+  float* W1ab;    // [2d, d]  rows 0..d-1 = W1a (receiver block), d..2d-1 = W1b (sender block)
+  float* W1c;     // [d, n_rbf]
+  float* W1abT;   // [d, 2d]  = [W1a^T | W1b^T]   (backward: hbar += Pbar W1a + Qbar W1b)
+  float* W2T;     // [d, d]   W2 transposed ([in,out])
+  float* V2T;     // [d, d]
+  float* V1aT;    // [d, d]   (V1[:, :d])^T
+  float* V1bT;    // [d, d]   (V1[:, d:])^T
+  float* b1pad;   // [2d] = [b1 | 0]
+  // bf16 operand images for the tensor-core path (device, owned); see tc_common.cuh
+  __nv_bfloat16 *W2img, *W1cimg, *W1cTimg;
+  __nv_bfloat16 *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;
+};
+
+struct mlip_model {
+  mlip_model_header h;
+  mlip_ctx* ctx;
+  float* blob = nullptr;  // device copy of the caller's blob
+  const float *T, *E0, *Wo, *bo, *wo, *bE;
+  float* WoT = nullptr;   // [d,d]
+  __nv_bfloat16 *Wo_bf = nullptr, *WoT_bf = nullptr;
+  std::vector<LayerWeights> layers;
+  std::vector<void*> owned;  // everything to cudaFree
+};
+
+// ---- graph --------------------------------------------------------------------------------
+// A (sub)graph in the form the model kernels consume: atoms are numbered locally, edges are
+// sorted by receiver, rows sorted by (sender, shift).
+struct SubGraph {
+  int64_t n = 0;        // atoms (extended set)
+  int64_t n_owned = 0;  // root atoms
+  int64_t E = 0;        // directed edges
+  const int32_t* gid = nullptr;    // [n] index into the graph's internal numbering (nullptr = identity)
+  const float* omega = nullptr;    // [n] 1 for root atoms, 0 for halo atoms (nullptr = all ones)
+  const int32_t* species = nullptr;  // [n]
+  const int32_t* rowptr = nullptr;   // [n+1]
+  const int32_t* recv = nullptr;     // [E]
+  const int32_t* send = nullptr;     // [E]
+  const int32_t* rev = nullptr;      // [E] index of the reverse edge
+  const float4* rvec = nullptr;      // [E] (r_x, r_y, r_z, |r|), float32 rounded from float64
+};
+
+struct mlip_graph {
+  mlip_ctx* ctx;
+  int64_t N = 0, E = 0;
+  double cell[9], inv[9], width[3];
+  double r_cut = 0;
+  int nc[3];
+  int32_t* perm = nullptr;      // [N] internal -> caller index
+  double* frac = nullptr;       // [N,3] wrapped fractional coordinates, internal order
+  int32_t* species = nullptr;   // [N] internal order
+  int32_t* rowptr = nullptr;    // [N+1]
+  int32_t* recv = nullptr;      // [E]
+  int32_t* send = nullptr;      // [E]
+  int32_t* shift = nullptr;     // [E] packed (nx+128)<<16 | (ny+128)<<8 | (nz+128)
+  int32_t* rev = nullptr;       // [E]
+  float4* rvec = nullptr;       // [E]
+  SubGraph view() const {
+    SubGraph s;
+    s.n = N; s.n_owned = N; s.E = E; s.species = species; s.rowptr = rowptr; s.recv = recv;
+    s.send = send; s.rev = rev; s.rvec = rvec;
+    return s;
+  }
+};
+
+struct PartSub {
+  SubGraph g;
+  int32_t *gid = nullptr, *species = nullptr, *rowptr = nullptr, *recv = nullptr, *send = nullptr,
+          *rev = nullptr;
+  float* omega = nullptr;
+  float4* rvec = nullptr;
+};
+
+struct mlip_part {
+  mlip_ctx* ctx;
+  int grid[3];
+  double halo = 0;
+  int64_t N = 0;
+  std::vector<PartSub> subs;
+};
+
+// ---- launchers (each bumps ctx->launches by the number of kernels it enqueues) ---------------
+// scan.cu
+int mlip_exclusive_scan_i32(mlip_ctx* ctx, const int32_t* in, int32_t* out, int64_t n,
+                            int64_t* total_host /*nullable; synchronises when given*/);
+
+// node_f32.cu -- Y[n,N] = epi( act(X)[n,K] . B^T + bias ), X = [X1 | X2] column blocks
+struct GemmArgs {
+  const float* X1 = nullptr; int ld1 = 0; int K1 = 0;
+  const float* X2 = nullptr; int ld2 = 0; int K2 = 0;
+  int act_in = 0;                 // 1: SiLU applied to X on load
+  const void* B = nullptr;        // [N, K1+K2] row-major (fp32 path) / bf16 row-major (tensor path)
+  const float* bias = nullptr;    // [N]
+  const float* mul_dsilu = nullptr; int ldz = 0;  // epilogue: y *= SiLU'(Z[row, col])
+  const float* residual = nullptr; int ldr = 0;   // epilogue: y += R[row, col] (may alias Y)
+  float* Y = nullptr; int ldy = 0;                // fp32 output (or)
+  __nv_bfloat16* Ybf = nullptr;                   // bf16 output (same ldy)
+  int64_t n = 0; int N = 0;
+};
+int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a);
+int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a);
+
+// energy_forces.cu
+int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* m, int L, const SubGraph& g, int precision,
+                       double* energy_accum_dev, float* forces_internal /*[N,3]*/,
+                       float* atom_energy_internal /*[N] or null*/);

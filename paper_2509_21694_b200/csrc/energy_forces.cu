@@ -1,0 +1,323 @@
+// Host orchestration of one energy-and-force evaluation (steps A6-A12 of SURVEY.md 8(a)):
+// embedding, L x (pre-projection, fused edge layer, node update), readout, the hand-written
+// reverse pass, force assembly per sub-domain, and the loop over sub-domains
+// with root-energy / all-atom-gradient assembly.
+#include "common.cuh"
+#include "edge.cuh"
+#include "mathfn.cuh"
+
+namespace {
+inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+__global__ void k_embed(int64_t n, int d, const int32_t* __restrict__ species, const float* __restrict__ T,
+                        float* __restrict__ h) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n * (d / 4)) return;
+  const int64_t i = idx / (d / 4);
+  const int c = (int)(idx % (d / 4)) * 4;
+  *reinterpret_cast<float4*>(h + i * d + c) = *reinterpret_cast<const float4*>(T + (size_t)species[i] * d + c);
+}
+
+// E_i = wo . SiLU(o_i) + b_E + E0[z_i];  obar_i = omega_i wo * SiLU'(o_i)   (O4, first line of O5)
+__global__ void __launch_bounds__(256) k_readout(int64_t n, int d, const float* __restrict__ o,
+                                                 const float* __restrict__ wo, const float* __restrict__ bE,
+                                                 const float* __restrict__ E0, const int32_t* __restrict__ species,
+                                                 const float* __restrict__ omega, float* __restrict__ E_i,
+                                                 float* __restrict__ obar) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= n) return;
+  const float w = omega ? omega[i] : 1.0f;
+  float acc = 0.f;
+  for (int c = lane * 4; c < d; c += 128) {
+    const float4 x = *reinterpret_cast<const float4*>(o + i * d + c);
+    const float4 q = *reinterpret_cast<const float4*>(wo + c);
+    float s, ds;
+    float4 ob;
+    silu_both_f(x.x, s, ds); acc = fmaf(q.x, s, acc); ob.x = w * q.x * ds;
+    silu_both_f(x.y, s, ds); acc = fmaf(q.y, s, acc); ob.y = w * q.y * ds;
+    silu_both_f(x.z, s, ds); acc = fmaf(q.z, s, acc); ob.z = w * q.z * ds;
+    silu_both_f(x.w, s, ds); acc = fmaf(q.w, s, acc); ob.w = w * q.w * ds;
+    *reinterpret_cast<float4*>(obar + i * d + c) = ob;
+  }
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+  if (lane == 0) E_i[i] = acc + bE[0] + E0[species[i]];
+}
+
+// deterministic float64 sum of the root-atom energies: per-block partials, then one block
+__global__ void __launch_bounds__(256) k_energy_partial(int64_t n, const float* __restrict__ E_i,
+                                                        const float* __restrict__ omega, const int32_t* __restrict__ gid,
+                                                        double* __restrict__ partial, float* __restrict__ atom_energy) {
+  __shared__ double sh[256];
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double v = 0.0;
+  if (i < n) {
+    const float w = omega ? omega[i] : 1.0f;
+    v = (double)w * (double)E_i[i];
+    if (atom_energy && w != 0.f) atom_energy[gid ? gid[i] : i] = E_i[i];
+  }
+  sh[threadIdx.x] = v;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(256) k_energy_final(int64_t n_partial, const double* __restrict__ partial,
+                                                      double* __restrict__ energy) {
+  __shared__ double sh[256];
+  double v = 0.0;
+  for (int64_t i = threadIdx.x; i < n_partial; i += 256) v += partial[i];
+  sh[threadIdx.x] = v;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) energy[0] += sh[0];
+}
+
+// A11: f_k = sum_{e in in(k)} (rbar_e + rbar_rev(e)) rhat_e ; F[gid_k] += f_k
+__global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __restrict__ rowptr,
+                                                const int32_t* __restrict__ rev, const float4* __restrict__ rvec,
+                                                const float* __restrict__ rbar, const int32_t* __restrict__ gid,
+                                                float* __restrict__ F) {
+  const int lane = threadIdx.x & 31;
+  const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (k >= n) return;
+  float fx = 0.f, fy = 0.f, fz = 0.f;
+  for (int e = rowptr[k] + lane; e < rowptr[k + 1]; e += 32) {
+    const float4 rv = rvec[e];
+    const float w = (rbar[e] + rbar[rev[e]]) * (rv.w > 0.f ? 1.0f / rv.w : 0.f);
+    fx = fmaf(w, rv.x, fx); fy = fmaf(w, rv.y, fy); fz = fmaf(w, rv.z, fz);
+  }
+#pragma unroll
+  for (int s = 16; s > 0; s >>= 1) {
+    fx += __shfl_xor_sync(0xffffffffu, fx, s);
+    fy += __shfl_xor_sync(0xffffffffu, fy, s);
+    fz += __shfl_xor_sync(0xffffffffu, fz, s);
+  }
+  if (lane == 0) {
+    const int64_t g = gid ? gid[k] : k;
+    F[3 * g] += fx; F[3 * g + 1] += fy; F[3 * g + 2] += fz;
+  }
+}
+
+__global__ void k_unpermute(int64_t N, const int32_t* __restrict__ perm, const float* __restrict__ F_int,
+                            const float* __restrict__ E_int, float* __restrict__ F_out, float* __restrict__ E_out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= N) return;
+  const int64_t a = perm[k];
+  F_out[3 * a] = F_int[3 * k]; F_out[3 * a + 1] = F_int[3 * k + 1]; F_out[3 * a + 2] = F_int[3 * k + 2];
+  if (E_out) E_out[a] = E_int[k];
+}
+}  // namespace
+
+int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph& g, int precision,
+                       double* energy_accum, float* F_int, float* Ei_int) {
+  const int64_t n = g.n, E = g.E;
+  if (n == 0) return MLIP_OK;
+  const int d = M->h.d;
+  const bool bf = precision == MLIP_BF16;
+  cudaStream_t st = ctx->stream;
+  auto gemm = bf ? mlip_gemm_bf16 : mlip_gemm_f32;
+  const int64_t tiles = bf ? mlip_edge_bf16_tiles(E) : mlip_edge_f32_tiles(E);
+
+  std::vector<void*> ws;
+  auto release = [&]() { for (void* p : ws) ctx->free(p); };
+#define W_ALLOC(ptr, T, count)                                         \
+  do {                                                                 \
+    int _s = ctx->alloc(&ptr, (size_t)(count));                        \
+    if (_s != MLIP_OK) { release(); return _s; }                       \
+    ws.push_back(ptr);                                                 \
+  } while (0)
+#define W_TRY(x) do { int _s = (x); if (_s != MLIP_OK) { release(); return _s; } } while (0)
+
+  std::vector<float*> h(L + 1), P(L), c(L);
+  std::vector<float*> Qf(L, nullptr);
+  std::vector<__nv_bfloat16*> Qb(L, nullptr);
+  for (int l = 0; l <= L; ++l) W_ALLOC(h[l], float, n * d);
+  for (int l = 0; l < L; ++l) {
+    if (bf) { W_ALLOC(P[l], float, n * d); W_ALLOC(Qb[l], __nv_bfloat16, n * d); }
+    else { W_ALLOC(P[l], float, n * 2 * d); Qf[l] = P[l] + d; }
+    W_ALLOC(c[l], float, n * d);
+  }
+  float *m = nullptr, *o = nullptr, *hbar = nullptr, *cbar = nullptr, *PQbar = nullptr, *head = nullptr, *tail = nullptr,
+        *rbar = nullptr, *E_i = nullptr, *abar = nullptr;
+  __nv_bfloat16* abar_bf = nullptr;
+  double* partial = nullptr;
+  W_ALLOC(m, float, n * d); W_ALLOC(o, float, n * d); W_ALLOC(hbar, float, n * d); W_ALLOC(cbar, float, n * d);
+  W_ALLOC(PQbar, float, n * 2 * d); W_ALLOC(head, float, (tiles + 1) * d); W_ALLOC(tail, float, (tiles + 1) * d);
+  W_ALLOC(rbar, float, E + 1); W_ALLOC(E_i, float, n);
+  if (L > 0) { if (bf) W_ALLOC(abar_bf, __nv_bfloat16, E * d); else W_ALLOC(abar, float, E * d); }
+  const int64_t n_part = (n + 255) / 256;
+  W_ALLOC(partial, double, n_part);
+  float* mbar = m;           // m is dead after the forward pass
+  float* Pbar = PQbar;
+  float* Qbar = PQbar + n * d;  // stored as two dense [n,d] blocks
+
+  k_embed<<<nblk(n * (d / 4), 256), 256, 0, st>>>(n, d, g.species, M->T, h[0]);
+  ctx->launches++;
+
+  EdgeArgs ea;
+  ea.E = E; ea.n = n; ea.rowptr = g.rowptr; ea.recv = g.recv; ea.send = g.send; ea.rev = g.rev; ea.rvec = g.rvec;
+  ea.r_cut = M->h.r_cut; ea.alpha = M->h.agg_scale; ea.n_rbf = M->h.n_rbf; ea.head = head; ea.tail = tail;
+
+  auto set_layer = [&](int l) {
+    const LayerWeights& W = M->layers[l];
+    ea.P = P[l]; ea.ldp = bf ? d : 2 * d; ea.Q = Qf[l]; ea.ldq = 2 * d; ea.Qbf = Qb[l];
+    ea.W1c = W.W1c; ea.W2T = W.W2T; ea.W2 = W.W2; ea.b2 = W.b2;
+    ea.W2img = W.W2img; ea.W1cimg = W.W1cimg; ea.W1cTimg = W.W1cTimg;
+  };
+
+  for (int l = 0; l < L; ++l) {
+    const LayerWeights& W = M->layers[l];
+    GemmArgs a;
+    if (bf) {
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1; a.Y = P[l]; a.ldy = d; a.n = n; a.N = d;
+      W_TRY(gemm(ctx, a));
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Ybf = Qb[l]; a.ldy = d; a.n = n; a.N = d;
+      W_TRY(gemm(ctx, a));
+    } else {
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1ab; a.bias = W.b1pad; a.Y = P[l]; a.ldy = 2 * d; a.n = n; a.N = 2 * d;
+      W_TRY(gemm(ctx, a));
+    }
+    cudaMemsetAsync(m, 0, sizeof(float) * n * d, st);
+    set_layer(l);
+    ea.m = m;
+    W_TRY(bf ? mlip_edge_forward_bf16(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
+    a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.X2 = m; a.ld2 = d; a.K2 = d;
+    a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+    a = GemmArgs(); a.X1 = c[l]; a.ld1 = d; a.K1 = d; a.act_in = 1;
+    a.B = bf ? (const void*)W.V2_bf : (const void*)W.V2; a.bias = W.c2; a.residual = h[l]; a.ldr = d;
+    a.Y = h[l + 1]; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+  }
+  {
+    GemmArgs a;
+    a.X1 = h[L]; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->Wo_bf : (const void*)M->Wo; a.bias = M->bo;
+    a.Y = o; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+  }
+  float* obar = cbar;
+  k_readout<<<nblk(n * 32, 256), 256, 0, st>>>(n, d, o, M->wo, M->bE, M->E0, g.species, g.omega, E_i, obar);
+  k_energy_partial<<<(unsigned)n_part, 256, 0, st>>>(n, E_i, g.omega, g.gid, partial, Ei_int);
+  k_energy_final<<<1, 256, 0, st>>>(n_part, partial, energy_accum);
+  ctx->launches += 3;
+  {
+    GemmArgs a;
+    a.X1 = obar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->WoT_bf : (const void*)M->WoT;
+    a.Y = hbar; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+  }
+  cudaMemsetAsync(rbar, 0, sizeof(float) * (E + 1), st);
+  for (int l = L - 1; l >= 0; --l) {
+    const LayerWeights& W = M->layers[l];
+    GemmArgs a;
+    a = GemmArgs(); a.X1 = hbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V2T_bf : (const void*)W.V2T;
+    a.mul_dsilu = c[l]; a.ldz = d; a.Y = cbar; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+    a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1bT_bf : (const void*)W.V1bT;
+    a.Y = mbar; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+    a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
+    a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+    cudaMemsetAsync(Pbar, 0, sizeof(float) * n * d, st);
+    set_layer(l);
+    ea.mbar = mbar; ea.abar = abar; ea.abar_bf = abar_bf; ea.Pbar = Pbar; ea.rbar = rbar;
+    W_TRY(bf ? mlip_edge_backward_bf16(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
+    W_TRY(bf ? mlip_gather_rev_bf16(ctx, n, d, g.rowptr, g.rev, abar_bf, Qbar)
+             : mlip_gather_rev_f32(ctx, n, d, g.rowptr, g.rev, abar, Qbar));
+    a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.X2 = Qbar; a.ld2 = d; a.K2 = d;
+    a.B = bf ? (const void*)W.W1abT_bf : (const void*)W.W1abT; a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d;
+    a.n = n; a.N = d;
+    W_TRY(gemm(ctx, a));
+  }
+  k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, F_int);
+  ctx->launches++;
+  release();
+#undef W_ALLOC
+#undef W_TRY
+  MLIP_CUDA_CHECK(ctx, cudaGetLastError());
+  return MLIP_OK;
+}
+
+extern "C" int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G, const mlip_part* part,
+                                  int precision, double* energy_dev, float* forces_dev, float* atom_energy_dev) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!M || !G || !energy_dev || (G->N > 0 && !forces_dev)) { ctx->set_error("mlip_energy_forces: null argument"); return MLIP_ERR_INVALID_ARG; }
+  if (L < 0 || L > M->h.L_max) { ctx->set_error("L outside [0, L_max]"); return MLIP_ERR_UNSUPPORTED; }
+  if (precision != MLIP_FP32 && precision != MLIP_BF16) { ctx->set_error("unknown precision"); return MLIP_ERR_INVALID_ARG; }
+  if (precision == MLIP_BF16 && !(M->h.d == 256 || M->h.d == 128)) { ctx->set_error("MLIP_BF16 needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
+  if (part && part->N != G->N) { ctx->set_error("partition does not belong to this graph"); return MLIP_ERR_INVALID_ARG; }
+  if (part && part->subs.size() > 1 && part->halo < (double)L * (double)M->h.r_cut * (1.0 - 1e-12)) {
+    ctx->set_error("halo < L * r_cut: sub-graphs would not keep the K-hop neighbourhood of their root atoms");
+    return MLIP_ERR_HALO_TOO_SMALL;
+  }
+  if (fabs(G->r_cut - (double)M->h.r_cut) > 1e-6 * G->r_cut) { ctx->set_error("graph r_cut differs from model r_cut"); return MLIP_ERR_INVALID_ARG; }
+  MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+  const int64_t N = G->N;
+  float *F_int = nullptr, *E_int = nullptr;
+  MLIP_TRY(ctx->alloc(&F_int, 3 * N));
+  MLIP_TRY(ctx->alloc(&E_int, N));
+  cudaMemsetAsync(F_int, 0, sizeof(float) * 3 * N, st);
+  cudaMemsetAsync(E_int, 0, sizeof(float) * N, st);
+  cudaMemsetAsync(energy_dev, 0, sizeof(double), st);
+  int status = MLIP_OK;
+  if (!part) {
+    status = mlip_eval_subgraph(ctx, M, L, G->view(), precision, energy_dev, F_int, E_int);
+  } else {
+    for (const PartSub& s : part->subs) {
+      status = mlip_eval_subgraph(ctx, M, L, s.g, precision, energy_dev, F_int, E_int);
+      if (status != MLIP_OK) break;
+    }
+  }
+  if (status == MLIP_OK && N > 0) {
+    k_unpermute<<<nblk(N, 256), 256, 0, st>>>(N, G->perm, F_int, E_int, forces_dev, atom_energy_dev);
+    ctx->launches++;
+  }
+  ctx->free(F_int); ctx->free(E_int);
+  if (status != MLIP_OK) return status;
+  MLIP_CUDA_CHECK(ctx, cudaGetLastError());
+  return MLIP_OK;
+}
+
+extern "C" int mlip_step_host(mlip_ctx* ctx, const mlip_model* M, int L, const double* pos_host, const double* cell_host,
+                              const int32_t* species_host, int64_t N, const int grid[3], double halo, int precision,
+                              double* energy_host, float* forces_host) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!M || !pos_host || !cell_host || !species_host || !grid || !energy_host || !forces_host || N < 0) {
+    ctx->set_error("mlip_step_host: null argument");
+    return MLIP_ERR_INVALID_ARG;
+  }
+  MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+  double *pos_d = nullptr, *e_d = nullptr;
+  int32_t* sp_d = nullptr;
+  float* f_d = nullptr;
+  MLIP_TRY(ctx->alloc(&pos_d, 3 * N)); MLIP_TRY(ctx->alloc(&sp_d, N)); MLIP_TRY(ctx->alloc(&f_d, 3 * N));
+  MLIP_TRY(ctx->alloc(&e_d, 1));
+  MLIP_CUDA_CHECK(ctx, cudaMemcpyAsync(pos_d, pos_host, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, st));
+  MLIP_CUDA_CHECK(ctx, cudaMemcpyAsync(sp_d, species_host, sizeof(int32_t) * N, cudaMemcpyHostToDevice, st));
+  mlip_graph* G = nullptr;
+  mlip_part* P = nullptr;
+  int status = mlip_build_graph(ctx, pos_d, cell_host, sp_d, N, (double)M->h.r_cut, &G);
+  if (status == MLIP_OK && (grid[0] > 1 || grid[1] > 1 || grid[2] > 1)) status = mlip_partition_grid(ctx, G, grid, halo, &P);
+  if (status == MLIP_OK) status = mlip_energy_forces(ctx, M, L, G, P, precision, e_d, f_d, nullptr);
+  if (status == MLIP_OK) {
+    cudaMemcpyAsync(energy_host, e_d, sizeof(double), cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(forces_host, f_d, sizeof(float) * 3 * N, cudaMemcpyDeviceToHost, st);
+  }
+  mlip_part_destroy(P);
+  mlip_graph_destroy(G);
+  ctx->free(pos_d); ctx->free(sp_d); ctx->free(f_d); ctx->free(e_d);
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (status != MLIP_OK) return status;
+  if (e != cudaSuccess) { ctx->set_error(std::string("step: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
+  return MLIP_OK;
+}

@@ -1,0 +1,165 @@
+// Context + model handles: weight blob upload and the derived operand layouts (transposed /
+// sliced fp32 matrices for the CUDA-core path, bf16 operand images for the tcgen05 path).
+#include <string.h>
+#include "common.cuh"
+#include "tc_images.cuh"
+
+namespace {
+// dst[r, c] = src[(r0 + (T ? c : r)) * ld + c0 + (T ? r : c)], dst is [rows, cols] dense (ld_dst)
+__global__ void k_copy_sub(const float* __restrict__ src, int ld, int r0, int c0, int transpose,
+                           float* __restrict__ dst, int ld_dst, int rows, int cols) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= rows * cols) return;
+  const int r = idx / cols, c = idx % cols;
+  const int sr = r0 + (transpose ? c : r), sc = c0 + (transpose ? r : c);
+  dst[(size_t)r * ld_dst + c] = src[(size_t)sr * ld + sc];
+}
+__global__ void k_to_bf16(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, int n) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = __float2bfloat16_rn(src[i]);
+}
+}  // namespace
+
+extern "C" size_t mlip_model_num_weights(const mlip_model_header* h) {
+  if (!h) return 0;
+  const size_t S = h->n_species, d = h->d, k = h->n_rbf, L = h->L_max;
+  const size_t per_layer = d * (2 * d + k) + d + d * d + d + d * 2 * d + d + d * d + d;
+  return S * d + S + L * per_layer + d * d + d + d + 1;
+}
+
+extern "C" int mlip_ctx_create(int device, void* stream, mlip_ctx** out) {
+  if (!out) return MLIP_ERR_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) {
+    cudaGetLastError();
+    return MLIP_ERR_CUDA;  // no CPU fallback: without a usable device nothing runs
+  }
+  if (cudaSetDevice(device) != cudaSuccess) return MLIP_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return MLIP_ERR_CUDA;
+  if (prop.major != 10) return MLIP_ERR_UNSUPPORTED;  // sm_100a only
+  mlip_ctx* c = new mlip_ctx();
+  c->device = device;
+  c->stream = (cudaStream_t)stream;
+  c->num_sms = prop.multiProcessorCount;
+  cudaMemPool_t pool;
+  if (cudaDeviceGetDefaultMemPool(&pool, device) == cudaSuccess) {
+    uint64_t thr = ~0ull;  // keep freed blocks in the pool between steps
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+  }
+  *out = c;
+  return MLIP_OK;
+}
+
+extern "C" void mlip_ctx_destroy(mlip_ctx* ctx) { delete ctx; }
+extern "C" const char* mlip_last_error(const mlip_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+extern "C" int64_t mlip_ctx_launch_count(const mlip_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" void mlip_model_destroy(mlip_model* m) {
+  if (!m) return;
+  for (void* p : m->owned) cudaFree(p);
+  delete m;
+}
+
+extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const float* w_host, size_t n,
+                               mlip_model** out) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!h || !w_host || !out) { ctx->set_error("mlip_model_load: null argument"); return MLIP_ERR_INVALID_ARG; }
+  *out = nullptr;
+  if (h->magic != MLIP_MAGIC || h->version != 1) { ctx->set_error("bad model header magic/version"); return MLIP_ERR_INVALID_ARG; }
+  if (h->flags != 0) { ctx->set_error("three-body variant not implemented"); return MLIP_ERR_UNSUPPORTED; }
+  if (!(h->d == 64 || h->d == 128 || h->d == 256) || h->n_rbf < 2 || h->n_rbf > 16 || h->n_species < 1 ||
+      h->L_max < 0 || !(h->r_cut > 0.f)) {
+    ctx->set_error("unsupported model shape (d in {64,128,256}, 2 <= n_rbf <= 16)");
+    return MLIP_ERR_UNSUPPORTED;
+  }
+  if (n != mlip_model_num_weights(h)) { ctx->set_error("weight blob size does not match header"); return MLIP_ERR_INVALID_ARG; }
+  MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+  mlip_model* M = new mlip_model();
+  M->h = *h; M->ctx = ctx;
+  const int S = h->n_species, d = h->d, k = h->n_rbf, L = h->L_max;
+  auto fail = [&](int code) { mlip_model_destroy(M); return code; };
+  auto dalloc = [&](size_t bytes) -> void* {
+    void* p = nullptr;
+    if (cudaMalloc(&p, bytes ? bytes : 1) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    M->owned.push_back(p);
+    return p;
+  };
+#define M_ALLOC(ptr, T, count)                                                         \
+  do {                                                                                 \
+    ptr = (T*)dalloc(sizeof(T) * (size_t)(count));                                     \
+    if (!ptr) { ctx->set_error("out of device memory (model)"); return fail(MLIP_ERR_OUT_OF_MEMORY); } \
+  } while (0)
+  M_ALLOC(M->blob, float, n);
+  if (cudaMemcpyAsync(M->blob, w_host, n * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) {
+    ctx->set_error("weight upload failed");
+    return fail(MLIP_ERR_CUDA);
+  }
+  const float* p = M->blob;
+  M->T = p; p += (size_t)S * d;
+  M->E0 = p; p += S;
+  M->layers.resize(L);
+  auto sub = [&](const float* src, int ld, int r0, int c0, int tr, float* dst, int ld_dst, int rows, int cols) {
+    k_copy_sub<<<(rows * cols + 255) / 256, 256, 0, st>>>(src, ld, r0, c0, tr, dst, ld_dst, rows, cols);
+  };
+  auto tobf = [&](const float* src, __nv_bfloat16* dst, int cnt) {
+    k_to_bf16<<<(cnt + 255) / 256, 256, 0, st>>>(src, dst, cnt);
+  };
+  for (int l = 0; l < L; ++l) {
+    LayerWeights& W = M->layers[l];
+    memset(&W, 0, sizeof(W));
+    W.W1 = p; p += (size_t)d * (2 * d + k);
+    W.b1 = p; p += d;
+    W.W2 = p; p += (size_t)d * d;
+    W.b2 = p; p += d;
+    W.V1 = p; p += (size_t)d * 2 * d;
+    W.c1 = p; p += d;
+    W.V2 = p; p += (size_t)d * d;
+    W.c2 = p; p += d;
+    M_ALLOC(W.W1ab, float, 2 * d * d); M_ALLOC(W.W1c, float, d * 16); M_ALLOC(W.W1abT, float, 2 * d * d);
+    M_ALLOC(W.W2T, float, d * d); M_ALLOC(W.V2T, float, d * d); M_ALLOC(W.V1aT, float, d * d);
+    M_ALLOC(W.V1bT, float, d * d); M_ALLOC(W.b1pad, float, 2 * d);
+    const int ld1 = 2 * d + k;
+    sub(W.W1, ld1, 0, 0, 0, W.W1ab, d, d, d);                    // W1a
+    sub(W.W1, ld1, 0, d, 0, W.W1ab + (size_t)d * d, d, d, d);    // W1b
+    cudaMemsetAsync(W.W1c, 0, sizeof(float) * d * 16, st);
+    sub(W.W1, ld1, 0, 2 * d, 0, W.W1c, 16, d, k);                // W1c padded to 16 columns
+    sub(W.W1, ld1, 0, 0, 1, W.W1abT, 2 * d, d, d);               // W1a^T
+    sub(W.W1, ld1, 0, d, 1, W.W1abT + d, 2 * d, d, d);           // W1b^T
+    sub(W.W2, d, 0, 0, 1, W.W2T, d, d, d);
+    sub(W.V2, d, 0, 0, 1, W.V2T, d, d, d);
+    sub(W.V1, 2 * d, 0, 0, 1, W.V1aT, d, d, d);
+    sub(W.V1, 2 * d, 0, d, 1, W.V1bT, d, d, d);
+    cudaMemsetAsync(W.b1pad, 0, sizeof(float) * 2 * d, st);
+    cudaMemcpyAsync(W.b1pad, W.b1, sizeof(float) * d, cudaMemcpyDeviceToDevice, st);
+    // bf16 row-major copies for the tensor-core node GEMMs (B operands are [N, K] row-major)
+    M_ALLOC(W.W1a_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1b_bf, __nv_bfloat16, d * d);
+    M_ALLOC(W.V1_bf, __nv_bfloat16, 2 * d * d); M_ALLOC(W.V2_bf, __nv_bfloat16, d * d);
+    M_ALLOC(W.V2T_bf, __nv_bfloat16, d * d); M_ALLOC(W.V1aT_bf, __nv_bfloat16, d * d);
+    M_ALLOC(W.V1bT_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1abT_bf, __nv_bfloat16, 2 * d * d);
+    tobf(W.W1ab, W.W1a_bf, d * d); tobf(W.W1ab + (size_t)d * d, W.W1b_bf, d * d);
+    tobf(W.V1, W.V1_bf, 2 * d * d); tobf(W.V2, W.V2_bf, d * d); tobf(W.V2T, W.V2T_bf, d * d);
+    tobf(W.V1aT, W.V1aT_bf, d * d); tobf(W.V1bT, W.V1bT_bf, d * d); tobf(W.W1abT, W.W1abT_bf, 2 * d * d);
+    // operand images of the fused edge kernels (tc_images.cuh documents the layouts)
+    M_ALLOC(W.W2img, __nv_bfloat16, d * d); M_ALLOC(W.W1cimg, __nv_bfloat16, d * 16);
+    M_ALLOC(W.W1cTimg, __nv_bfloat16, 16 * d);
+    mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg, W.W1cTimg);
+  }
+  M->Wo = p; p += (size_t)d * d;
+  M->bo = p; p += d;
+  M->wo = p; p += d;
+  M->bE = p; p += 1;
+  M_ALLOC(M->WoT, float, d * d);
+  sub(M->Wo, d, 0, 0, 1, M->WoT, d, d, d);
+  M_ALLOC(M->Wo_bf, __nv_bfloat16, d * d); M_ALLOC(M->WoT_bf, __nv_bfloat16, d * d);
+  tobf(M->Wo, M->Wo_bf, d * d); tobf(M->WoT, M->WoT_bf, d * d);
+#undef M_ALLOC
+  if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+    ctx->set_error("model preparation kernels failed");
+    return fail(MLIP_ERR_CUDA);
+  }
+  *out = M;
+  return MLIP_OK;
+}

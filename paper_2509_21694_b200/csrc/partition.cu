@@ -1,0 +1,227 @@
+// Spatial partition + halo (PAPER.md:157 Stage 1, PAPER.md:165 Stage 2 with the geometric halo of
+// reading R2) and construction of each extended sub-graph as the sub-graph of the global graph
+// induced on the extended atom set (O6). Step A5 of SURVEY.md 8(a). Integer work + float64
+// comparisons on fractional coordinates.
+#include <math.h>
+#include "common.cuh"
+
+namespace {
+struct BinGeom {
+  int grid[3];
+  int bin[3];
+  double halo_frac[3];  // halo / perpendicular width
+};
+
+// flag: 0 outside, 1 halo, 2 root (owned)
+__global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom b, int32_t* __restrict__ ext,
+                             int32_t* __restrict__ owned) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  bool own = true, in_ext = true;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double f = frac[3 * i + k];
+    int bin = (int)floor(f * b.grid[k]);
+    if (bin > b.grid[k] - 1) bin = b.grid[k] - 1;
+    own = own && (bin == b.bin[k]);
+    const double lo = (double)b.bin[k] / b.grid[k], hi = (double)(b.bin[k] + 1) / b.grid[k];
+    double dist = 0.0;
+    if (!(f >= lo && f < hi)) {
+      double below = lo - f; below -= floor(below);
+      double above = f - hi; above -= floor(above);
+      dist = below < above ? below : above;
+    }
+    in_ext = in_ext && (dist <= b.halo_frac[k]);
+  }
+  in_ext = in_ext || own;
+  ext[i] = in_ext ? 1 : 0;
+  owned[i] = own ? 1 : 0;
+}
+
+__global__ void k_part_compact(int64_t N, const int32_t* __restrict__ ext, const int32_t* __restrict__ owned,
+                               const int32_t* __restrict__ scan, const int32_t* __restrict__ species,
+                               int32_t* __restrict__ lid, int32_t* __restrict__ gid, float* __restrict__ omega,
+                               int32_t* __restrict__ species_l, unsigned long long* __restrict__ n_owned) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  if (ext[i]) {
+    const int l = scan[i];
+    lid[i] = l;
+    gid[l] = (int32_t)i;
+    omega[l] = owned[i] ? 1.0f : 0.0f;
+    species_l[l] = species[i];
+    if (owned[i]) atomicAdd(n_owned, 1ull);
+  } else {
+    lid[i] = -1;
+  }
+}
+
+template <bool FILL>
+__global__ void __launch_bounds__(256) k_part_edges(int64_t n_ext, const int32_t* __restrict__ gid,
+                                                    const int32_t* __restrict__ lid,
+                                                    const int32_t* __restrict__ g_rowptr,
+                                                    const int32_t* __restrict__ g_send,
+                                                    const float4* __restrict__ g_rvec, int32_t* __restrict__ deg,
+                                                    const int32_t* __restrict__ rowptr, int32_t* __restrict__ recv,
+                                                    int32_t* __restrict__ send, float4* __restrict__ rvec,
+                                                    int32_t* __restrict__ geid) {
+  const int lane = threadIdx.x & 31;
+  const int64_t l = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (l >= n_ext) return;
+  const int i = gid[l];
+  const int lo = g_rowptr[i], hi = g_rowptr[i + 1];
+  int count = 0;
+  const int base = FILL ? rowptr[l] : 0;
+  for (int b = lo; b < hi; b += 32) {
+    const int e = b + lane;
+    int sl = -1;
+    if (e < hi) sl = lid[g_send[e]];
+    const unsigned m = __ballot_sync(0xffffffffu, sl >= 0);
+    if (FILL && sl >= 0) {
+      const int o = base + count + __popc(m & ((1u << lane) - 1u));
+      recv[o] = (int32_t)l;
+      send[o] = sl;
+      rvec[o] = g_rvec[e];
+      geid[o] = e;
+    }
+    count += __popc(m);
+  }
+  if (!FILL && lane == 0) deg[l] = count;
+}
+
+__global__ void k_part_rev(int64_t E, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ send,
+                           const int32_t* __restrict__ geid, const int32_t* __restrict__ g_rev,
+                           int32_t* __restrict__ rev, int* __restrict__ err_flag) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= E) return;
+  const int want = g_rev[geid[e]];
+  const int j = send[e];
+  int lo = rowptr[j], hi = rowptr[j + 1] - 1, found = -1;
+  while (lo <= hi) {
+    const int mid = (lo + hi) >> 1;
+    const int v = geid[mid];
+    if (v == want) { found = mid; break; }
+    if (v < want) lo = mid + 1; else hi = mid - 1;
+  }
+  if (found < 0) *err_flag = 3;
+  rev[e] = found;
+}
+
+inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+void free_sub(mlip_ctx* c, PartSub& s) {
+  c->free(s.gid); c->free(s.species); c->free(s.rowptr); c->free(s.recv); c->free(s.send); c->free(s.rev);
+  c->free(s.omega); c->free(s.rvec);
+}
+}  // namespace
+
+extern "C" void mlip_part_destroy(mlip_part* p) {
+  if (!p) return;
+  for (auto& s : p->subs) free_sub(p->ctx, s);
+  delete p;
+}
+
+extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo,
+                                   mlip_part** out) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!G || !grid || !out || grid[0] < 1 || grid[1] < 1 || grid[2] < 1 || !(halo >= 0.0)) {
+    ctx->set_error("mlip_partition_grid: invalid argument");
+    return MLIP_ERR_INVALID_ARG;
+  }
+  *out = nullptr;
+  MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+  const int64_t N = G->N;
+  mlip_part* P = new mlip_part();
+  P->ctx = ctx; P->halo = halo; P->N = N;
+  for (int k = 0; k < 3; ++k) P->grid[k] = grid[k];
+  auto fail = [&](int code) { mlip_part_destroy(P); return code; };
+#define P_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
+  int32_t *ext = nullptr, *owned = nullptr, *scan = nullptr, *lid = nullptr, *deg = nullptr, *geid = nullptr;
+  unsigned long long* n_owned_d = nullptr;
+  int* err_flag = nullptr;
+  P_TRY(ctx->alloc(&ext, N + 1)); P_TRY(ctx->alloc(&owned, N + 1)); P_TRY(ctx->alloc(&scan, N + 1));
+  P_TRY(ctx->alloc(&lid, N + 1)); P_TRY(ctx->alloc(&n_owned_d, 1)); P_TRY(ctx->alloc(&err_flag, 1));
+  cudaMemsetAsync(err_flag, 0, sizeof(int), st);
+  for (int bx = 0; bx < grid[0]; ++bx)
+    for (int by = 0; by < grid[1]; ++by)
+      for (int bz = 0; bz < grid[2]; ++bz) {
+        BinGeom b;
+        b.bin[0] = bx; b.bin[1] = by; b.bin[2] = bz;
+        for (int k = 0; k < 3; ++k) { b.grid[k] = grid[k]; b.halo_frac[k] = halo / G->width[k]; }
+        P->subs.emplace_back();
+        PartSub& S = P->subs.back();
+        int64_t n_ext = 0, E = 0;
+        cudaMemsetAsync(n_owned_d, 0, sizeof(unsigned long long), st);
+        if (N > 0) {
+          k_part_flags<<<nblk(N, 256), 256, 0, st>>>(N, G->frac, b, ext, owned);
+          ctx->launches++;
+        }
+        P_TRY(mlip_exclusive_scan_i32(ctx, ext, scan, N, &n_ext));
+        P_TRY(ctx->alloc(&S.gid, n_ext)); P_TRY(ctx->alloc(&S.omega, n_ext)); P_TRY(ctx->alloc(&S.species, n_ext));
+        P_TRY(ctx->alloc(&S.rowptr, n_ext + 1)); P_TRY(ctx->alloc(&deg, n_ext + 1));
+        if (N > 0) {
+          k_part_compact<<<nblk(N, 256), 256, 0, st>>>(N, ext, owned, scan, G->species, lid, S.gid, S.omega,
+                                                       S.species, n_owned_d);
+          ctx->launches++;
+        }
+        if (n_ext > 0) {
+          k_part_edges<false><<<nblk(n_ext * 32, 256), 256, 0, st>>>(n_ext, S.gid, lid, G->rowptr, G->send, G->rvec,
+                                                                     deg, nullptr, nullptr, nullptr, nullptr, nullptr);
+          ctx->launches++;
+        }
+        P_TRY(mlip_exclusive_scan_i32(ctx, deg, S.rowptr, n_ext, &E));
+        unsigned long long n_owned_h = 0;
+        cudaMemcpyAsync(&n_owned_h, n_owned_d, sizeof(n_owned_h), cudaMemcpyDeviceToHost, st);
+        cudaStreamSynchronize(st);
+        P_TRY(ctx->alloc(&S.recv, E)); P_TRY(ctx->alloc(&S.send, E)); P_TRY(ctx->alloc(&S.rev, E));
+        P_TRY(ctx->alloc(&S.rvec, E)); P_TRY(ctx->alloc(&geid, E));
+        if (E > 0) {
+          k_part_edges<true><<<nblk(n_ext * 32, 256), 256, 0, st>>>(n_ext, S.gid, lid, G->rowptr, G->send, G->rvec,
+                                                                    nullptr, S.rowptr, S.recv, S.send, S.rvec, geid);
+          k_part_rev<<<nblk(E, 256), 256, 0, st>>>(E, S.rowptr, S.send, geid, G->rev, S.rev, err_flag);
+          ctx->launches += 2;
+        }
+        ctx->free(deg); deg = nullptr;
+        ctx->free(geid); geid = nullptr;
+        S.g.n = n_ext; S.g.n_owned = (int64_t)n_owned_h; S.g.E = E;
+        S.g.gid = S.gid; S.g.omega = S.omega; S.g.species = S.species; S.g.rowptr = S.rowptr;
+        S.g.recv = S.recv; S.g.send = S.send; S.g.rev = S.rev; S.g.rvec = S.rvec;
+      }
+  int err_h = 0;
+  cudaMemcpyAsync(&err_h, err_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+  cudaError_t e = cudaStreamSynchronize(st);
+  ctx->free(ext); ctx->free(owned); ctx->free(scan); ctx->free(lid); ctx->free(n_owned_d); ctx->free(err_flag);
+  if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+    ctx->set_error(std::string("partition: ") + cudaGetErrorString(e));
+    return fail(MLIP_ERR_CUDA);
+  }
+  if (err_h != 0) { ctx->set_error("partition: reverse edge not found (internal error)"); return fail(MLIP_ERR_CUDA); }
+#undef P_TRY
+  *out = P;
+  return MLIP_OK;
+}
+
+extern "C" int mlip_partition(mlip_ctx* ctx, const mlip_graph* G, int n_sub, double halo, mlip_part** out) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!G || n_sub < 1) { ctx->set_error("mlip_partition: invalid argument"); return MLIP_ERR_INVALID_ARG; }
+  int axis = 0;
+  for (int k = 1; k < 3; ++k) if (G->width[k] > G->width[axis]) axis = k;  // ties -> lowest index (R3)
+  int grid[3] = {1, 1, 1};
+  grid[axis] = n_sub;
+  return mlip_partition_grid(ctx, G, grid, halo, out);
+}
+
+extern "C" int mlip_part_count(const mlip_part* p, int* n_sub) {
+  if (!p || !n_sub) return MLIP_ERR_INVALID_ARG;
+  *n_sub = (int)p->subs.size();
+  return MLIP_OK;
+}
+
+extern "C" int mlip_part_info(const mlip_part* p, int s, int64_t* n_owned, int64_t* n_ext, int64_t* n_edges) {
+  if (!p || s < 0 || s >= (int)p->subs.size()) return MLIP_ERR_INVALID_ARG;
+  if (n_owned) *n_owned = p->subs[s].g.n_owned;
+  if (n_ext) *n_ext = p->subs[s].g.n;
+  if (n_edges) *n_edges = p->subs[s].g.E;
+  return MLIP_OK;
+}

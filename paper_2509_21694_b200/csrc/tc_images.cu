@@ -1,0 +1,24 @@
+#include "tc_images.cuh"
+
+namespace {
+__global__ void k_edge_images(const float* __restrict__ W2, const float* __restrict__ W1c, int d,
+                              __nv_bfloat16* __restrict__ W2img, __nv_bfloat16* __restrict__ W1cimg,
+                              __nv_bfloat16* __restrict__ W1cTimg) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < d * d) {
+    const int o = idx / d, i = idx % d;
+    W2img[tc_sw128_index(d, o, i)] = __float2bfloat16_rn(W2[idx]);
+  }
+  if (idx < d * 16) {
+    const int c = idx / 16, k = idx % 16;
+    const __nv_bfloat16 v = __float2bfloat16_rn(W1c[idx]);
+    W1cimg[tc_nosw_index(16, c, k)] = v;
+    W1cTimg[tc_sw128_index(16, k, c)] = v;
+  }
+}
+}  // namespace
+
+void mlip_make_edge_images(cudaStream_t st, const float* W2, const float* W1c, int d,
+                           __nv_bfloat16* W2img, __nv_bfloat16* W1cimg, __nv_bfloat16* W1cTimg) {
+  k_edge_images<<<(d * d + 255) / 256, 256, 0, st>>>(W2, W1c, d, W2img, W1cimg, W1cTimg);
+}

@@ -1,0 +1,106 @@
+"""-m gpu: energies and forces of the CUDA path (through the C ABI) against the float64 oracle on
+the same seeded inputs. Tolerances are those of north_star / reading R14:
+fp32 path  eps_E <= 1e-5, max|dF| <= 1e-4 RMS(F);  bf16 path  RMS(dF)/RMS(F) <= 2e-2;
+partitioned vs unpartitioned GPU forces within 1e-5 RMS(F) in fp32."""
+import numpy as np
+import pytest
+
+from oracle import mlip_oracle as O
+from synth_inputs import ModelSpec, make_config, make_weights, small_system
+from tests.gpu_util import errors, gpu_energy_forces, gpu_graph, gpu_setup, oracle_model, rms
+
+pytestmark = pytest.mark.gpu
+
+FP32_EPS_E, FP32_MAX_F = 1e-5, 1e-4
+BF16_RMS_F = 2e-2
+
+
+def _run(spec, blob, system, L, precision=0, grid=None, halo=0.0):
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, system, spec.r_cut)
+    part = mlip.Partition(ctx, g, halo, grid=grid) if grid is not None else None
+    return gpu_energy_forces(mlip, ctx, model, L, g, part, precision)
+
+
+def test_config1_fp32_parity():
+    cfg = make_config(1)
+    s = cfg.system
+    ref = O.energy_forces(oracle_model(cfg.model, cfg.weights), cfg.L, s.pos, s.cell, s.species)
+    E, F, Ei = _run(cfg.model, cfg.weights, s, cfg.L)
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    print(err)
+    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+
+
+@pytest.mark.parametrize("d,L,n_cells,r_cut,nbar", [(64, 3, 4, 5.0, 43.0), (128, 4, 4, 5.0, 43.0), (256, 2, 4, 6.0, 76.0),
+                                                   (128, 0, 3, 5.0, 43.0), (64, 1, 2, 5.0, 43.0)])
+def test_fp32_parity_shapes(d, L, n_cells, r_cut, nbar):
+    spec = ModelSpec(4, d, 16 if d > 64 else 8, max(L, 1), r_cut, 1.0 / np.sqrt(nbar))
+    blob = make_weights(spec, 77 + d)
+    s = small_system(n_cells, 0.1, seed=d + L, vacancy_fraction=0.03)
+    ref = O.energy_forces(oracle_model(spec, blob), L, s.pos, s.cell, s.species)
+    E, F, Ei = _run(spec, blob, s, L)
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    print(d, L, err)
+    assert err["eps_E"] <= FP32_EPS_E
+    if L > 0:
+        assert err["max_F"] <= FP32_MAX_F
+    else:
+        assert np.all(F == 0)
+
+
+def test_fp32_partitioned_equals_unpartitioned_and_oracle():
+    spec = ModelSpec(4, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 5)
+    s = small_system(8, 0.08, seed=31)  # 28.8 A box, 2048 atoms; L r_cut = 6
+    ref = O.energy_forces(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    E0, F0, Ei0 = _run(spec, blob, s, 2)
+    for grid in [(2, 1, 1), (3, 1, 1), (2, 2, 1), (1, 1, 4)]:
+        E, F, Ei = _run(spec, blob, s, 2, grid=grid, halo=6.0)
+        assert np.abs(F - F0).max() <= 1e-5 * rms(F0)
+        assert abs(E - E0) <= 1e-5 * np.abs(Ei0).sum()
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+    # negative control: a halo of (L-1) r_cut is refused, not silently wrong
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, s, spec.r_cut)
+    part = mlip.Partition(ctx, g, 3.0, grid=(3, 1, 1))
+    with pytest.raises(mlip.MlipError) as ei:
+        mlip.energy_forces(ctx, model, 2, g, part, 0)
+    assert ei.value.code == -3
+
+
+def test_run_to_run_bitwise_and_order_independent():
+    """No floating-point atomics: repeated evaluations are bitwise identical."""
+    cfg = make_config(1)
+    a = _run(cfg.model, cfg.weights, cfg.system, cfg.L)
+    b = _run(cfg.model, cfg.weights, cfg.system, cfg.L)
+    assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+def test_mpdp_L_argument():
+    """the first L of L_max layers; L is a run-time argument."""
+    spec = ModelSpec(4, 64, 8, 3, 5.0, 1.0 / np.sqrt(43.0))
+    blob = make_weights(spec, 9)
+    s = small_system(3, 0.05, seed=2)
+    om = oracle_model(spec, blob)
+    for L in (1, 2, 3):
+        ref = O.energy_forces(om, L, s.pos, s.cell, s.species)
+        E, F, Ei = _run(spec, blob, s, L)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, s, spec.r_cut)
+    with pytest.raises(mlip.MlipError):
+        mlip.energy_forces(ctx, model, 4, g, None, 0)
+
+
+def test_step_host_matches_device_path():
+    cfg = make_config(1)
+    mlip, ctx, model = gpu_setup(cfg.model, cfg.weights)
+    s = cfg.system
+    E1, F1, _ = _run(cfg.model, cfg.weights, s, cfg.L)
+    E2, F2 = mlip.step_host(ctx, model, cfg.L, s.pos, s.cell, s.species)
+    assert E1 == E2 and np.array_equal(F1.astype(np.float32), F2)
+    E3, F3 = mlip.step_host(ctx, model, cfg.L, s.pos, s.cell, s.species, grid=(1, 1, 1), halo=0.0)
+    assert E3 == E2
