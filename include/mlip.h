@@ -132,6 +132,16 @@ int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* m, int L, const mlip_gra
                        const mlip_part* part, int precision, double* energy_dev,
                        float* forces_dev, float* atom_energy_dev);
 
+/* The same evaluation restricted to the sub-domains k with k mod n_shards == shard (sub-graph
+ * predictions are completely independent, and are distributed over devices in
+ * PAPER.md:177). Energies and forces are this shard's PARTIAL sums over the whole box (zeros
+ * where it contributes nothing); summing the outputs of all shards -- one all-reduce of E and F
+ * when the shards live on different GPUs -- gives exactly the unsharded result up to fp32
+ * summation order. atom_energy_dev holds E_i for the atoms this shard owns, 0 elsewhere. */
+int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* m, int L, const mlip_graph* g,
+                             const mlip_part* part, int shard, int n_shards, int precision,
+                             double* energy_dev, float* forces_dev, float* atom_energy_dev);
+
 /* Whole step from HOST buffers: copies positions/species to the device, builds the graph,
  * partitions (grid = {1,1,1} means one domain), evaluates, copies E and F back and
  * synchronises. This is the call bench.py times for its end-to-end figure. */
@@ -142,6 +152,23 @@ int mlip_step_host(mlip_ctx* ctx, const mlip_model* m, int L, const double* pos_
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);
+
+/* Per-kernel-group device timing (SURVEY.md 5 "tracing": CUDA events on the context stream,
+ * one pair around each launch group). mlip_ctx_profile(ctx, 1) clears the counters and starts
+ * recording, (ctx, 0) stops. mlip_ctx_profile_read synchronises the stream and returns the
+ * accumulated milliseconds and kernel-launch count of one group since the last enable. */
+typedef enum {
+  MLIP_GROUP_EDGE_FWD = 0,       /* fused gather -> edge MLP -> segmented sum (steps A6+A7) */
+  MLIP_GROUP_EDGE_BWD = 1,       /* its reverse pass (edge part of A10) */
+  MLIP_GROUP_GATHER_REV = 2,     /* sender-side adjoint gather through the reverse-edge index */
+  MLIP_GROUP_NODE_GEMM = 3,      /* node pre-projection / update / readout contractions (A8-A10) */
+  MLIP_GROUP_READOUT_FORCES = 4, /* embedding, readout, energy sum, force assembly (A9, A11) */
+  MLIP_GROUP_GRAPH = 5,          /* mlip_build_graph (A1-A4) */
+  MLIP_GROUP_PARTITION = 6,      /* mlip_partition / mlip_partition_grid (A5) */
+  MLIP_GROUP_COUNT = 7
+} mlip_group;
+int mlip_ctx_profile(mlip_ctx* ctx, int enable);
+int mlip_ctx_profile_read(mlip_ctx* ctx, int group, double* ms_total, int64_t* n_launches);
 
 #ifdef __cplusplus
 }

@@ -14,6 +14,7 @@ import numpy as np
 MLIP_FP32 = 0
 MLIP_BF16 = 1
 MLIP_MAGIC = 0x50494C4D
+GROUPS = ("edge_fwd", "edge_bwd", "gather_rev", "node_gemm", "readout_forces", "graph", "partition")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
@@ -63,8 +64,11 @@ def load_library():
     lib.mlip_part_info.argtypes = [vp, i32, P(i64), P(i64), P(i64)]
     lib.mlip_part_destroy.argtypes = [vp]; lib.mlip_part_destroy.restype = None
     lib.mlip_energy_forces.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
+    lib.mlip_energy_forces_shard.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.mlip_step_host.argtypes = [vp, vp, i32, vp, vp, vp, i64, P(i32), dbl, i32, vp, vp]
     lib.mlip_ctx_launch_count.argtypes = [vp]; lib.mlip_ctx_launch_count.restype = i64
+    lib.mlip_ctx_profile.argtypes = [vp, i32]
+    lib.mlip_ctx_profile_read.argtypes = [vp, i32, P(dbl), P(i64)]
     _LIB = lib
     return lib
 
@@ -107,6 +111,19 @@ class Context:
     @property
     def launches(self) -> int:
         return int(self.lib.mlip_ctx_launch_count(self.h))
+
+    def profile(self, enable: bool):
+        """mlip_ctx_profile: start (clearing the counters) or stop per-kernel-group event timing."""
+        self.check(self.lib.mlip_ctx_profile(self.h, 1 if enable else 0))
+
+    def profile_read(self) -> dict:
+        """mlip_ctx_profile_read for every group -> {name: (ms_total, n_launches)}."""
+        out = {}
+        for gid, name in enumerate(GROUPS):
+            ms, n = C.c_double(), C.c_int64()
+            self.check(self.lib.mlip_ctx_profile_read(self.h, gid, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, int(n.value))
+        return out
 
     def __del__(self):
         if getattr(self, "_refs", 0) > 0:
@@ -216,6 +233,23 @@ def energy_forces(ctx: Context, model: Model, L: int, graph: Graph, part: Partit
     ctx.check(ctx.lib.mlip_energy_forces(ctx.h, model.h, int(L), graph.h, part.h if part is not None else None,
                                          int(precision), C.c_void_p(E.data_ptr()), C.c_void_p(F.data_ptr()),
                                          C.c_void_p(Ei.data_ptr()) if Ei is not None else None))
+    return E, F, Ei
+
+
+def energy_forces_shard(ctx: Context, model: Model, L: int, graph: Graph, part: Partition, shard: int, n_shards: int,
+                        precision: int = MLIP_FP32, want_atom_energy: bool = False, out=None):
+    """mlip_energy_forces_shard -> this shard's partial (E, F, E_i); sum over shards = full result."""
+    torch = _torch()
+    dev = f"cuda:{ctx.device}"
+    if out is None:
+        E = torch.empty(1, dtype=torch.float64, device=dev)
+        F = torch.empty((graph.n_atoms, 3), dtype=torch.float32, device=dev)
+        Ei = torch.empty(graph.n_atoms, dtype=torch.float32, device=dev) if want_atom_energy else None
+    else:
+        E, F, Ei = out
+    ctx.check(ctx.lib.mlip_energy_forces_shard(ctx.h, model.h, int(L), graph.h, part.h, int(shard), int(n_shards),
+                                               int(precision), C.c_void_p(E.data_ptr()), C.c_void_p(F.data_ptr()),
+                                               C.c_void_p(Ei.data_ptr()) if Ei is not None else None))
     return E, F, Ei
 
 

@@ -23,6 +23,18 @@
     if (_s != MLIP_OK) return _s;   \
   } while (0)
 
+// kernel groups timed by mlip_ctx_profile (CUDA events on the context stream)
+enum {
+  MLIP_PROF_EDGE_FWD = 0,   // fused gather -> edge MLP -> segmented sum (A6+A7)
+  MLIP_PROF_EDGE_BWD = 1,   // its reverse pass (edge part of A10)
+  MLIP_PROF_GATHER_REV = 2, // sender-side adjoint gather through rev[]
+  MLIP_PROF_NODE_GEMM = 3,  // node pre-projection / node update / readout GEMMs and adjoints
+  MLIP_PROF_READOUT_FORCES = 4,  // embedding, readout, energy sum, force assembly
+  MLIP_PROF_GRAPH = 5,      // mlip_build_graph
+  MLIP_PROF_PARTITION = 6,  // mlip_partition*
+  MLIP_PROF_COUNT = 7
+};
+
 struct mlip_ctx {
   int device = 0;
   cudaStream_t stream = nullptr;
@@ -30,6 +42,33 @@ struct mlip_ctx {
   std::string err;
   int64_t launches = 0;
   void set_error(const std::string& s) { err = s; }
+  // ---- optional per-group timing ----
+  struct ProfRec { int cat; int64_t launches; cudaEvent_t a, b; };
+  bool profiling = false;
+  std::vector<ProfRec> prof;
+  std::vector<cudaEvent_t> event_pool;
+  double prof_ms[MLIP_PROF_COUNT] = {0};
+  int64_t prof_launches[MLIP_PROF_COUNT] = {0};
+  cudaEvent_t get_event() {
+    cudaEvent_t e;
+    if (!event_pool.empty()) { e = event_pool.back(); event_pool.pop_back(); return e; }
+    cudaEventCreate(&e);
+    return e;
+  }
+  // returns a token (index + 1) or 0 when profiling is off
+  size_t prof_begin(int cat) {
+    if (!profiling) return 0;
+    ProfRec r; r.cat = cat; r.launches = launches; r.a = get_event(); r.b = get_event();
+    cudaEventRecord(r.a, stream);
+    prof.push_back(r);
+    return prof.size();
+  }
+  void prof_end(size_t token) {
+    if (!token) return;
+    ProfRec& r = prof[token - 1];
+    r.launches = launches - r.launches;
+    cudaEventRecord(r.b, stream);
+  }
   // stream-ordered allocation (pool keeps memory between steps)
   template <class T>
   int alloc(T** p, size_t n) {
@@ -46,6 +85,12 @@ struct mlip_ctx {
   void free(void* p) {
     if (p) cudaFreeAsync(p, stream);
   }
+};
+
+struct ProfScope {
+  mlip_ctx* c; size_t t;
+  ProfScope(mlip_ctx* ctx, int cat) : c(ctx), t(ctx->prof_begin(cat)) {}
+  ~ProfScope() { c->prof_end(t); }
 };
 
 // ---- model --------------------------------------------------------------------------------

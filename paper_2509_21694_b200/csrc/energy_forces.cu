@@ -122,7 +122,8 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   const int d = M->h.d;
   const bool bf = precision == MLIP_BF16;
   cudaStream_t st = ctx->stream;
-  auto gemm = bf ? mlip_gemm_bf16 : mlip_gemm_f32;
+  auto gemm_raw = bf ? mlip_gemm_bf16 : mlip_gemm_f32;
+  auto gemm = [&](mlip_ctx* c, const GemmArgs& ga) { ProfScope p(c, MLIP_PROF_NODE_GEMM); return gemm_raw(c, ga); };
   const int64_t tiles = bf ? mlip_edge_bf16_tiles(E) : mlip_edge_f32_tiles(E);
 
   std::vector<void*> ws;
@@ -158,8 +159,11 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   float* Pbar = PQbar;
   float* Qbar = PQbar + n * d;  // stored as two dense [n,d] blocks
 
-  k_embed<<<nblk(n * (d / 4), 256), 256, 0, st>>>(n, d, g.species, M->T, h[0]);
-  ctx->launches++;
+  {
+    ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
+    k_embed<<<nblk(n * (d / 4), 256), 256, 0, st>>>(n, d, g.species, M->T, h[0]);
+    ctx->launches++;
+  }
 
   EdgeArgs ea;
   ea.E = E; ea.n = n; ea.rowptr = g.rowptr; ea.recv = g.recv; ea.send = g.send; ea.rev = g.rev; ea.rvec = g.rvec;
@@ -187,7 +191,10 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     cudaMemsetAsync(m, 0, sizeof(float) * n * d, st);
     set_layer(l);
     ea.m = m;
-    W_TRY(bf ? mlip_edge_forward_bf16(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
+    {
+      ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
+      W_TRY(bf ? mlip_edge_forward_bf16(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
+    }
     a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.X2 = m; a.ld2 = d; a.K2 = d;
     a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = n; a.N = d;
     W_TRY(gemm(ctx, a));
@@ -203,10 +210,13 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     W_TRY(gemm(ctx, a));
   }
   float* obar = cbar;
-  k_readout<<<nblk(n * 32, 256), 256, 0, st>>>(n, d, o, M->wo, M->bE, M->E0, g.species, g.omega, E_i, obar);
-  k_energy_partial<<<(unsigned)n_part, 256, 0, st>>>(n, E_i, g.omega, g.gid, partial, Ei_int);
-  k_energy_final<<<1, 256, 0, st>>>(n_part, partial, energy_accum);
-  ctx->launches += 3;
+  {
+    ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
+    k_readout<<<nblk(n * 32, 256), 256, 0, st>>>(n, d, o, M->wo, M->bE, M->E0, g.species, g.omega, E_i, obar);
+    k_energy_partial<<<(unsigned)n_part, 256, 0, st>>>(n, E_i, g.omega, g.gid, partial, Ei_int);
+    k_energy_final<<<1, 256, 0, st>>>(n_part, partial, energy_accum);
+    ctx->launches += 3;
+  }
   {
     GemmArgs a;
     a.X1 = obar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->WoT_bf : (const void*)M->WoT;
@@ -229,16 +239,25 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     cudaMemsetAsync(Pbar, 0, sizeof(float) * n * d, st);
     set_layer(l);
     ea.mbar = mbar; ea.abar = abar; ea.abar_bf = abar_bf; ea.Pbar = Pbar; ea.rbar = rbar;
-    W_TRY(bf ? mlip_edge_backward_bf16(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
-    W_TRY(bf ? mlip_gather_rev_bf16(ctx, n, d, g.rowptr, g.rev, abar_bf, Qbar)
-             : mlip_gather_rev_f32(ctx, n, d, g.rowptr, g.rev, abar, Qbar));
+    {
+      ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
+      W_TRY(bf ? mlip_edge_backward_bf16(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
+    }
+    {
+      ProfScope p(ctx, MLIP_PROF_GATHER_REV);
+      W_TRY(bf ? mlip_gather_rev_bf16(ctx, n, d, g.rowptr, g.rev, abar_bf, Qbar)
+               : mlip_gather_rev_f32(ctx, n, d, g.rowptr, g.rev, abar, Qbar));
+    }
     a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.X2 = Qbar; a.ld2 = d; a.K2 = d;
     a.B = bf ? (const void*)W.W1abT_bf : (const void*)W.W1abT; a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d;
     a.n = n; a.N = d;
     W_TRY(gemm(ctx, a));
   }
-  k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, F_int);
-  ctx->launches++;
+  {
+    ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
+    k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, F_int);
+    ctx->launches++;
+  }
   release();
 #undef W_ALLOC
 #undef W_TRY
@@ -248,7 +267,15 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
 
 extern "C" int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G, const mlip_part* part,
                                   int precision, double* energy_dev, float* forces_dev, float* atom_energy_dev) {
+  return mlip_energy_forces_shard(ctx, M, L, G, part, 0, 1, precision, energy_dev, forces_dev, atom_energy_dev);
+}
+
+extern "C" int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G,
+                                        const mlip_part* part, int shard, int n_shards, int precision,
+                                        double* energy_dev, float* forces_dev, float* atom_energy_dev) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (n_shards < 1 || shard < 0 || shard >= n_shards) { ctx->set_error("shard outside [0, n_shards)"); return MLIP_ERR_INVALID_ARG; }
+  if (n_shards > 1 && !part) { ctx->set_error("sharded evaluation needs a partition"); return MLIP_ERR_INVALID_ARG; }
   if (!M || !G || !energy_dev || (G->N > 0 && !forces_dev)) { ctx->set_error("mlip_energy_forces: null argument"); return MLIP_ERR_INVALID_ARG; }
   if (L < 0 || L > M->h.L_max) { ctx->set_error("L outside [0, L_max]"); return MLIP_ERR_UNSUPPORTED; }
   if (precision != MLIP_FP32 && precision != MLIP_BF16) { ctx->set_error("unknown precision"); return MLIP_ERR_INVALID_ARG; }
@@ -272,8 +299,9 @@ extern "C" int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* M, int L, con
   if (!part) {
     status = mlip_eval_subgraph(ctx, M, L, G->view(), precision, energy_dev, F_int, E_int);
   } else {
-    for (const PartSub& s : part->subs) {
-      status = mlip_eval_subgraph(ctx, M, L, s.g, precision, energy_dev, F_int, E_int);
+    for (size_t k = 0; k < part->subs.size(); ++k) {
+      if ((int)(k % (size_t)n_shards) != shard) continue;  // sub-domain k belongs to shard k mod n_shards
+      status = mlip_eval_subgraph(ctx, M, L, part->subs[k].g, precision, energy_dev, F_int, E_int);
       if (status != MLIP_OK) break;
     }
   }

@@ -370,6 +370,7 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
   memcpy(G->cell, g.cell, sizeof(g.cell)); memcpy(G->inv, g.inv, sizeof(g.inv));
   memcpy(G->width, width, sizeof(width)); memcpy(G->nc, g.nc, sizeof(g.nc));
   auto fail = [&](int code) { mlip_graph_destroy(G); return code; };
+  ProfScope prof(ctx, MLIP_PROF_GRAPH);
 
   double *frac = nullptr, *pos_s = nullptr;
   int32_t *wrap = nullptr, *cellid = nullptr, *cell_count = nullptr, *cell_start = nullptr, *order = nullptr,

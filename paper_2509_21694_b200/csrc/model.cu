@@ -52,7 +52,47 @@ extern "C" int mlip_ctx_create(int device, void* stream, mlip_ctx** out) {
   return MLIP_OK;
 }
 
-extern "C" void mlip_ctx_destroy(mlip_ctx* ctx) { delete ctx; }
+extern "C" void mlip_ctx_destroy(mlip_ctx* ctx) {
+  if (!ctx) return;
+  for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
+  delete ctx;
+}
+
+static void prof_collect(mlip_ctx* ctx) {
+  cudaStreamSynchronize(ctx->stream);
+  for (auto& r : ctx->prof) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) {
+      ctx->prof_ms[r.cat] += ms;
+      ctx->prof_launches[r.cat] += r.launches;
+    } else {
+      cudaGetLastError();
+    }
+    ctx->event_pool.push_back(r.a);
+    ctx->event_pool.push_back(r.b);
+  }
+  ctx->prof.clear();
+}
+
+extern "C" int mlip_ctx_profile(mlip_ctx* ctx, int enable) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  prof_collect(ctx);
+  if (enable) {
+    for (int i = 0; i < MLIP_PROF_COUNT; ++i) { ctx->prof_ms[i] = 0.0; ctx->prof_launches[i] = 0; }
+  }
+  ctx->profiling = enable != 0;
+  return MLIP_OK;
+}
+
+extern "C" int mlip_ctx_profile_read(mlip_ctx* ctx, int group, double* ms_total, int64_t* n_launches) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (group < 0 || group >= MLIP_PROF_COUNT) { ctx->set_error("unknown kernel group"); return MLIP_ERR_INVALID_ARG; }
+  prof_collect(ctx);
+  if (ms_total) *ms_total = ctx->prof_ms[group];
+  if (n_launches) *n_launches = ctx->prof_launches[group];
+  return MLIP_OK;
+}
 extern "C" const char* mlip_last_error(const mlip_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 extern "C" int64_t mlip_ctx_launch_count(const mlip_ctx* ctx) { return ctx ? ctx->launches : 0; }
 

@@ -136,6 +136,7 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
   P->ctx = ctx; P->halo = halo; P->N = N;
   for (int k = 0; k < 3; ++k) P->grid[k] = grid[k];
   auto fail = [&](int code) { mlip_part_destroy(P); return code; };
+  ProfScope prof(ctx, MLIP_PROF_PARTITION);
 #define P_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
   int32_t *ext = nullptr, *owned = nullptr, *scan = nullptr, *lid = nullptr, *deg = nullptr, *geid = nullptr;
   unsigned long long* n_owned_d = nullptr;
