@@ -152,7 +152,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   W_ALLOC(m, float, n * d); W_ALLOC(o, float, n * d); W_ALLOC(hbar, float, n * d); W_ALLOC(cbar, float, n * d);
   W_ALLOC(PQbar, float, n * 2 * d); W_ALLOC(head, float, (tiles + 1) * d); W_ALLOC(tail, float, (tiles + 1) * d);
   W_ALLOC(rbar, float, E + 1); W_ALLOC(E_i, float, n);
-  if (L > 0) { if (bf) W_ALLOC(abar_bf, __nv_bfloat16, E * d); else W_ALLOC(abar, float, E * d); }
+  if (L > 0) { if (bf) W_ALLOC(abar_bf, __nv_bfloat16, tiles * 128 * d); else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
   const int64_t n_part = (n + 255) / 256;
   W_ALLOC(partial, double, n_part);
   float* mbar = m;           // m is dead after the forward pass

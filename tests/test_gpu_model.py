@@ -104,3 +104,71 @@ def test_step_host_matches_device_path():
     assert E1 == E2 and np.array_equal(F1.astype(np.float32), F2)
     E3, F3 = mlip.step_host(ctx, model, cfg.L, s.pos, s.cell, s.species, grid=(1, 1, 1), halo=0.0)
     assert E3 == E2
+
+
+# ---- MLIP_BF16: bf16 tensor-core contractions (tcgen05), fp32 accumulation ------------------------
+@pytest.mark.parametrize("d,L,n_cells,r_cut,nbar", [(256, 0, 3, 5.0, 43.0), (256, 1, 3, 5.0, 43.0), (256, 2, 4, 6.0, 76.0),
+                                                   (128, 2, 4, 5.0, 43.0), (256, 5, 5, 6.0, 76.0)])
+def test_bf16_parity_shapes(d, L, n_cells, r_cut, nbar):
+    """Reference = oracle with the UNROUNDED fp32 weights (reading R15). Sizes span several 128-edge
+    tiles with a ragged last tile and segments that straddle tiles."""
+    spec = ModelSpec(4, d, 16, max(L, 1), r_cut, 1.0 / np.sqrt(nbar))
+    blob = make_weights(spec, 77 + d)
+    s = small_system(n_cells, 0.1, seed=d + L, vacancy_fraction=0.03)
+    ref = O.energy_forces(oracle_model(spec, blob), L, s.pos, s.cell, s.species)
+    E, F, Ei = _run(spec, blob, s, L, precision=1)
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    print(d, L, err)
+    assert np.isfinite(F).all() and np.isfinite(E)
+    assert err["eps_E"] <= 5e-3  # not a north_star bound; catches gross errors of the forward pass
+    if L > 0:
+        assert err["rms_F"] <= BF16_RMS_F
+    else:
+        assert np.all(F == 0)
+
+
+def test_bf16_config2_shape_pruned_vs_unpruned():
+    """BASELINE.json configs 2/3 on a shrunk box (fcc 6^3 with vacancies): L=5 of L_max=15 (MPDP,
+    PAPER.md:151) and the unpruned L=15, bf16 GEMM inputs, force RMS error <= 2e-2."""
+    cfg = make_config(3, n_cells_override=6)
+    s = cfg.system
+    om = oracle_model(cfg.model, cfg.weights)
+    for L in (5, 15):
+        ref = O.energy_forces(om, L, s.pos, s.cell, s.species)
+        E, F, Ei = _run(cfg.model, cfg.weights, s, L, precision=1)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        print(L, err)
+        assert err["rms_F"] <= BF16_RMS_F
+
+
+def test_bf16_partitioned_matches_unpartitioned():
+    spec = ModelSpec(4, 256, 16, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 6)
+    s = small_system(8, 0.08, seed=32)
+    ref = O.energy_forces(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    E0, F0, Ei0 = _run(spec, blob, s, 2, precision=1)
+    for grid in [(2, 1, 1), (1, 3, 1)]:
+        E, F, Ei = _run(spec, blob, s, 2, precision=1, grid=grid, halo=6.0)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        assert err["rms_F"] <= BF16_RMS_F
+        # each owned atom sees the same neighbourhood in its sub-domain, but tile boundaries differ,
+        # so the bf16 roundings of partial sums differ: equal only to bf16-path accuracy
+        assert rms(F - F0) <= BF16_RMS_F * rms(F0)
+
+
+def test_bf16_run_to_run_bitwise():
+    spec = ModelSpec(4, 256, 16, 2, 5.0, 1.0 / np.sqrt(43.0))
+    blob = make_weights(spec, 8)
+    s = small_system(4, 0.1, seed=3)
+    a = _run(spec, blob, s, 2, precision=1)
+    b = _run(spec, blob, s, 2, precision=1)
+    assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+def test_bf16_rejects_d64():
+    cfg = make_config(1)
+    mlip, ctx, model = gpu_setup(cfg.model, cfg.weights)
+    g = gpu_graph(mlip, ctx, cfg.system, cfg.model.r_cut)
+    with pytest.raises(mlip.MlipError) as ei:
+        mlip.energy_forces(ctx, model, cfg.L, g, None, 1)
+    assert ei.value.code == -2
