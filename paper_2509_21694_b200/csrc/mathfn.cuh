@@ -31,3 +31,20 @@ __device__ __forceinline__ void rbf_f(float r, float r_cut, int n_rbf, int k, fl
   g = expf(-gamma * diff * diff);
   dg = -2.0f * gamma * diff * g;
 }
+
+// SiLU through the hardware tanh (MUFU.TANH, abs. error ~2^-11): used by the MLIP_BF16 kernels only,
+// where every result is rounded to bf16 (ulp 2^-8) anyway. sigma(x) = 1/2 + 1/2 tanh(x/2).
+__device__ __forceinline__ float tanh_approx_f(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float silu_tanh_f(float x) {
+  const float h = 0.5f * x;
+  return fmaf(h, tanh_approx_f(h), h);
+}
+__device__ __forceinline__ void silu_both_tanh_f(float x, float& y, float& dy) {
+  const float s = fmaf(0.5f, tanh_approx_f(0.5f * x), 0.5f);
+  y = x * s;
+  dy = fmaf(y, 1.0f - s, s);  // s (1 + x (1 - s))
+}
