@@ -106,6 +106,7 @@ struct LayerWeights {
   float* V1aT;    // [d, d]   (V1[:, :d])^T
   float* V1bT;    // [d, d]   (V1[:, d:])^T
   float* b1pad;   // [2d] = [b1 | 0]
+  float* b1h;     // [d] = b1 / 2 (bias of the halved receiver pre-projection of the bf16 path)
   // bf16 operand images for the tensor-core path (device, owned); see tc_common.cuh
   __nv_bfloat16 *W2img, *W1cimg, *W1cTimg;
   __nv_bfloat16 *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;

@@ -1,51 +1,97 @@
 // MLIP_BF16 path of the fused edge kernels (steps A6, A7 and the edge part of A10) on the sm_100a
 // tensor cores: bf16 operands, fp32 accumulation in TMEM.
 //
-// A persistent CTA (one per SM) keeps the bf16 image of W2 (and the small W1c images) resident in
-// shared memory and walks over tiles of 128 consecutive receiver-sorted edges. Per tile:
-//   G1  D1[edge, c]  = e_hat[edge, 0:16] . W1c^T                       tcgen05.mma  M128 N=d K16
-//   E1  a = D1 + P_i + Q_j ; s = SiLU(a) -> bf16 S tile (the gathered Q rows are overwritten in
-//       place); backward keeps SiLU'(a) in D1 (tcgen05.st)
-//   G2  D2[edge, c]  = S . W2^T                                          K-major W2 image
-//   E2  forward : phi = SiLU(D2 + b2), alpha u_e phi -> S tile, segmented column sums -> m_i
-//       backward: pbar = alpha u_e mbar_i SiLU'(D2 + b2) -> S tile; ubar_e = alpha <mbar_i, phi_e>
-//   G3  D3[edge, c']  = pbar . W2    (the SAME W2 image read as an MN-major operand)
-//   E3  abar = D3 * SiLU'(a) -> S tile -> (i) one linear bulk copy to the spill buffer (read back
-//       through rev[] by k_gather_rev_bf16), (ii) segmented column sums -> Pbar_i, (iii) G4
-//   G4  D4[edge, k]  = abar . W1c   (ebar)                               N = 16
-//   E4  rbar_e += ubar_e u' + sum_k ebar_k (u' g_k + u g'_k)
-// Each thread owns one edge row (TMEM lane) and half of the channels. Segments that straddle
-// tiles go through per-tile head/tail rows and k_segment_fixup_bf16: no floating-point atomics.
+// One persistent, warp-specialised CTA per SM walks over tiles of 128 consecutive receiver-sorted
+// edges. The bf16 image of W2 (and the small W1c images) stays resident in shared memory.
+//   warps 0..15  epilogue: thread = (edge row, 16 of every 64 channels); TMEM -> registers -> SiLU ->
+//                bf16 operand slab in shared memory, chunk by chunk (64 channels = one SW128 slab)
+//   warp 16      one thread issues every tcgen05.mma as soon as the slab it needs is published
+//   warp 17      producer, one tile ahead: edge metadata, envelope, radial basis (A6), the bf16 e_hat
+//                operand, the receiver-selector operand of the segmented sum
+// Per tile (all factors 1/2 of the SiLU arguments are folded into the weight images, so that
+// SiLU(2x) = x + x tanh(x) costs one MUFU and one FMA):
+//   G1  X[edge, c]  = e_hat . (W1c/2)^T                                  M128 N=d K16
+//   E1  a' = X + P'_i + Q'_j ; s = SiLU(2a') -> slab c/64 ; backward keeps 2 SiLU'(2a') in registers
+//   G2  Y[edge, o] += s . (W2/2)^T      issued per 64-channel K slab while E1 works on the next one
+//   E2  forward : alpha u_e SiLU(2(Y + b2/2)) -> slabs
+//       backward: pbar = alpha u_e mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
+//   G3  X[edge, i] += pbar . (W2/2)     (backward; the SAME W2 image read MN-major), per slab
+//   E3  abar = X * 2 SiLU'(2a') -> slabs -> (i) bulk copy to the spill buffer (read back through
+//       rev[] by k_gather_rev_bf16), (ii) segmented sum, (iii) G4
+//   GS  segmented sum over runs of equal receiver as an MMA: Yseg[channel, r] = slab^T . Sel with the
+//       0/1 selector Sel[edge, r] (M = 128 channels, N = 16 receivers, K = 128 edges); its result is
+//       m_i (forward) / Pbar_i (backward). Tiles with more than 16 receivers take a shared-memory loop.
+//   G4  ebar[edge, k] = abar . W1c  (N = 16) ; E4  rbar_e += ubar_e u' + sum_k ebar_k (u' g_k + u g'_k)
+// Segments that straddle tiles go through per-tile head/tail rows and k_segment_fixup_bf16: no
+// floating-point atomics anywhere, results are bitwise reproducible.
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
 #include "tc_ptx.cuh"
 
 namespace {
-constexpr int TE = 128;  // edges per tile = MMA M
+constexpr int TE = 128;          // edges per tile = MMA M
+constexpr int N_EPI_WARPS = 16;  // 4 lane quarters x 4 column groups
+constexpr int WARP_MMA = 16, WARP_PROD = 17;
+constexpr int N_THREADS = 18 * 32;
+constexpr int SLOT_BYTES = TE * 128;  // one [128 x 64] bf16 SW128 slab
+constexpr int MAX_SEG = 16;           // receivers per tile handled by the selector MMA
 
-template <int D>
-struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
-  static constexpr uint32_t w2 = 0;                          // [D x D] bf16, K-major SW128 image
-  static constexpr uint32_t s = w2 + D * D * 2;              // [128 x D] bf16, K-major SW128
-  static constexpr uint32_t w1cT = s + TE * D * 2;           // [16 x D] bf16, K-major SW128
-  static constexpr uint32_t w1c = w1cT + 16 * D * 2;         // [D x 16] bf16, K-major no swizzle
-  static constexpr uint32_t ehat = w1c + D * 16 * 2;         // [128 x 16] bf16, K-major no swizzle
-  static constexpr uint32_t b2 = ehat + TE * 16 * 2;         // [D] fp32
-  static constexpr uint32_t recv = b2 + D * 4;               // [128] int
-  static constexpr uint32_t u = recv + TE * 4;               // [128] fp32
-  static constexpr uint32_t du = u + TE * 4;
-  static constexpr uint32_t r = du + TE * 4;
-  static constexpr uint32_t ubar = r + TE * 4;               // [2][128] fp32
-  static constexpr uint32_t bar = ubar + 2 * TE * 4;         // mbarrier
-  static constexpr uint32_t slot = bar + 8;                  // TMEM base address
-  static constexpr uint32_t bytes = slot + 8 + 1024;         // + alignment slack
-  static constexpr int tmem_cols = 2 * D;                    // D1 | D2 (D3, D4 alias D2)
+struct TileMeta {       // written by the producer warp, double buffered
+  int recv[TE];         // local receiver (-1 beyond E)
+  int send[TE];
+  float w[TE];          // alpha * u(r_e)   (0 beyond E)
+  float r[TE], u[TE], du[TE];
+  int rid[MAX_SEG];     // receivers of the tile in order of appearance
+  int cls[MAX_SEG];     // 0: segment complete inside the tile, 1: continues from an earlier tile, 2: into a later one
+  int R;                // number of distinct receivers in the tile
+  int pad[3];
 };
 
-// Column sums of the bf16 S tile over runs of equal receiver (thread = channel). Complete segments
-// go to out[recv], segments continuing from an earlier tile to head[tile], segments continuing
-// into a later tile to tail[tile].
+template <int D, bool BWD>
+struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
+  static constexpr int NCH = D / 64;
+  static constexpr uint32_t w2 = 0;                                   // [D x D] bf16, K-major SW128 image of W2/2
+  static constexpr uint32_t ring = w2 + D * D * 2;                    // NCH slabs [128 x 64] bf16, K-major SW128
+  static constexpr uint32_t w1c = ring + NCH * SLOT_BYTES;            // [D x 16] bf16, K-major no swizzle (W1c/2)
+  static constexpr uint32_t w1cT = w1c + D * 16 * 2;                  // [16 x D] bf16, K-major SW128 (backward)
+  static constexpr uint32_t ehat = w1cT + (BWD ? 16 * D * 2 : 0);     // [128 x 16] bf16, K-major no swizzle
+  static constexpr uint32_t sel = ehat + TE * 16 * 2;                 // [16 x 128] bf16, K-major no swizzle
+  static constexpr uint32_t b2 = sel + MAX_SEG * TE * 2;              // [D] fp32 (b2/2)
+  static constexpr uint32_t meta = b2 + D * 4;                        // TileMeta[2]
+  static constexpr uint32_t ubar = meta + 2 * sizeof(TileMeta);       // [4][128] fp32 (backward)
+  static constexpr uint32_t bars = ubar + (BWD ? 4 * TE * 4 : 0);     // mbarriers
+  static constexpr uint32_t slot = bars + 32 * 8;                     // TMEM base address
+  static constexpr uint32_t bytes = slot + 16 + 1024;                 // + alignment slack
+  static constexpr int tmem_cols = 2 * D;                             // X | Y
+};
+
+// barrier indices
+enum { B_META_FULL = 0, B_META_EMPTY = 2, B_EHAT_FULL = 4, B_SEL_FULL = 5, B_D1_FULL = 6, B_D2_FULL = 7,
+       B_D3_FULL = 8, B_SEG_FULL = 9, B_X_FREE = 10, B_S_READY = 11 /* .. +NCH */ };
+
+__device__ __forceinline__ float tanh_mufu(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&r)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr)
+      : "memory");
+}
+
+// Shared-memory fallback of the segmented sum (tiles with more than MAX_SEG receivers): column sums
+// of the bf16 slabs over runs of equal receiver (thread = channel). Complete segments go to
+// out[recv], segments continuing from an earlier tile to head[tile], segments continuing into a
+// later tile to tail[tile].
 template <int D>
 __device__ __forceinline__ void segmented_store_bf16(const unsigned char* __restrict__ S, const int* __restrict__ recv_s,
                                                      const int32_t* __restrict__ rowptr, int64_t e0, int64_t tile,
@@ -53,7 +99,7 @@ __device__ __forceinline__ void segmented_store_bf16(const unsigned char* __rest
                                                      float* __restrict__ tail, int c) {
   int cur = recv_s[0];
   float sum = 0.f;
-  const uint32_t coff = (uint32_t)((c >> 6) * TE * 128 + (c & 7) * 2);
+  const uint32_t coff = (uint32_t)((c >> 6) * SLOT_BYTES + (c & 7) * 2);
   const int cc = (c & 63) >> 3;
   for (int e = 0; e <= TE; ++e) {
     const int rcv = e < TE ? recv_s[e] : -2;
@@ -75,40 +121,42 @@ __device__ __forceinline__ void segmented_store_bf16(const unsigned char* __rest
 }
 
 template <int D, bool BWD>
-__global__ void __launch_bounds__(256, 1) k_edge_bf16(EdgeArgs a, int64_t n_tiles) {
+__global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t n_tiles) {
   extern __shared__ unsigned char smem_raw[];
-  using SM = ES<D>;
+  using SM = ES<D, BWD>;
+  constexpr int NCH = SM::NCH;
   const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
   unsigned char* gen = smem_raw + (base - tc::smem_u32(smem_raw));
-  unsigned char* S = gen + SM::s;
+  TileMeta* meta = reinterpret_cast<TileMeta*>(gen + SM::meta);
   float* b2_s = reinterpret_cast<float*>(gen + SM::b2);
-  int* recv_s = reinterpret_cast<int*>(gen + SM::recv);
-  float* u_s = reinterpret_cast<float*>(gen + SM::u);
-  float* du_s = reinterpret_cast<float*>(gen + SM::du);
-  float* r_s = reinterpret_cast<float*>(gen + SM::r);
   float* ubar_s = reinterpret_cast<float*>(gen + SM::ubar);
   uint32_t* slot = reinterpret_cast<uint32_t*>(gen + SM::slot);
-  const uint32_t bar = base + SM::bar;
+  auto bar = [&](int i) -> uint32_t { return base + SM::bars + 8u * (uint32_t)i; };
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int q = warp & 3, hf = warp >> 2;
-  const int row = q * 32 + lane;
 
-  // ---- one-time setup: resident weight images, barrier, TMEM ----
+  // ---- one-time setup: resident weight images, barriers, TMEM ----
   {
     const uint4* src = reinterpret_cast<const uint4*>(a.W2img);
     uint4* dst = reinterpret_cast<uint4*>(gen + SM::w2);
-    for (int i = tid; i < D * D * 2 / 16; i += 256) dst[i] = src[i];
+    for (int i = tid; i < D * D * 2 / 16; i += N_THREADS) dst[i] = src[i];
     src = reinterpret_cast<const uint4*>(a.W1cimg);
     dst = reinterpret_cast<uint4*>(gen + SM::w1c);
-    for (int i = tid; i < D * 16 * 2 / 16; i += 256) dst[i] = src[i];
-    src = reinterpret_cast<const uint4*>(a.W1cTimg);
-    dst = reinterpret_cast<uint4*>(gen + SM::w1cT);
-    for (int i = tid; i < 16 * D * 2 / 16; i += 256) dst[i] = src[i];
-    for (int i = tid; i < D; i += 256) b2_s[i] = a.b2[i];
+    for (int i = tid; i < D * 16 * 2 / 16; i += N_THREADS) dst[i] = src[i];
+    if (BWD) {
+      src = reinterpret_cast<const uint4*>(a.W1cTimg);
+      dst = reinterpret_cast<uint4*>(gen + SM::w1cT);
+      for (int i = tid; i < 16 * D * 2 / 16; i += N_THREADS) dst[i] = src[i];
+    }
+    for (int i = tid; i < D; i += N_THREADS) b2_s[i] = 0.5f * a.b2[i];
   }
   if (tid == 0) {
-    tc::mbar_init(bar, 1);
+    tc::mbar_init(bar(B_META_FULL), 1); tc::mbar_init(bar(B_META_FULL + 1), 1);
+    tc::mbar_init(bar(B_META_EMPTY), N_EPI_WARPS + 1); tc::mbar_init(bar(B_META_EMPTY + 1), N_EPI_WARPS + 1);
+    tc::mbar_init(bar(B_EHAT_FULL), 1); tc::mbar_init(bar(B_SEL_FULL), 1);
+    tc::mbar_init(bar(B_D1_FULL), 1); tc::mbar_init(bar(B_D2_FULL), 1); tc::mbar_init(bar(B_D3_FULL), 1);
+    tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
+    for (int s = 0; s < NCH; ++s) tc::mbar_init(bar(B_S_READY + s), N_EPI_WARPS);
     tc::fence_mbar_init();
   }
   if (warp == 0) tc::tmem_alloc<SM::tmem_cols>(slot);
@@ -117,254 +165,375 @@ __global__ void __launch_bounds__(256, 1) k_edge_bf16(EdgeArgs a, int64_t n_tile
   __syncthreads();
   tc::fence_after_sync();
   const uint32_t tmem = *slot;
-  const uint32_t tlane = tmem + ((uint32_t)(q * 32) << 16);
-  uint32_t phase = 0;
+  const uint32_t TX = tmem, TY = tmem + D;  // accumulator regions: X = D1 / D3, Y = D2 / (segment sums, D4)
 
-  constexpr uint32_t IDESC_ND = tc::idesc_bf16(128, D, 0, 0);     // K-major A and B, N = D
-  constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);  // B read MN-major
-  constexpr uint32_t IDESC_N16 = tc::idesc_bf16(128, 16, 0, 0);
-
-  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const int64_t e0 = tile * TE;
-
-    // ---- tile metadata, edge features (A6) and the sender-row gather into the S tile ----
-    if (tid < TE) {
-      const int64_t e = e0 + tid;
-      int rc = -1;
-      float r = 0.f, u = 0.f, du = 0.f;
-      if (e < a.E) {
-        rc = a.recv[e]; r = a.rvec[e].w;
-        envelope_f(r, a.r_cut, u, du);
-      }
-      recv_s[tid] = rc; u_s[tid] = u; du_s[tid] = du; r_s[tid] = r;
-      uint32_t pk[8];
+  if (warp == WARP_PROD) {
+    // =========================== producer: tile metadata, e_hat, selector ===========================
+    const float delta = a.r_cut / (float)(a.n_rbf - 1);
+    const float ngl2 = -(0.5f / (delta * delta)) * 1.4426950408889634f;  // -gamma log2(e)
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int b = it & 1;
+      TileMeta& M = meta[b];
+      tc::mbar_wait(bar(B_META_EMPTY + b), (uint32_t)(((it >> 1) & 1) ^ 1));
+      const int64_t e0 = tile * TE;
+      int rc[4];
+      float rr[4], uu[4];
+      uint32_t fm[4];
 #pragma unroll
-      for (int k = 0; k < 16; k += 2) {
-        float g0 = 0.f, g1 = 0.f, dg;
-        if (e < a.E && k < a.n_rbf) rbf_f(r, a.r_cut, a.n_rbf, k, g0, dg);
-        if (e < a.E && k + 1 < a.n_rbf) rbf_f(r, a.r_cut, a.n_rbf, k + 1, g1, dg);
-        pk[k >> 1] = tc::pack_bf16(u * g0, u * g1);
-      }
-      // K-major, no swizzle: 8x8 core matrices of 128 B; (row, k) -> (row/8)*256 + (k/8)*128 + (row%8)*16
-      unsigned char* dst = gen + SM::ehat + (tid >> 3) * 256 + (tid & 7) * 16;
-      *reinterpret_cast<uint4*>(dst) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-      *reinterpret_cast<uint4*>(dst + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
-    }
-#pragma unroll 4
-    for (int i = 0; i < TE / 8; ++i) {
-      const int rw = warp + 8 * i;
-      const int64_t e = e0 + rw;
-      if (lane < D / 8) {
-        const uint32_t off = tc::sw128_chunk_off(TE, rw, lane);
-        if (e < a.E) {
-          const int sd = a.send[e];
-          tc::cp_async16(base + SM::s + off, a.Qbf + (size_t)sd * D + lane * 8);
-        } else {
-          *reinterpret_cast<uint4*>(S + off) = make_uint4(0u, 0u, 0u, 0u);
+      for (int k = 0; k < 4; ++k) {
+        const int e = lane + 32 * k;
+        const int64_t ge = e0 + e;
+        int sd = 0;
+        float du = 0.f;
+        bool flag = false;
+        rc[k] = -1; rr[k] = 0.f; uu[k] = 0.f;
+        if (ge < a.E) {
+          rc[k] = a.recv[ge]; sd = a.send[ge]; rr[k] = a.rvec[ge].w;
+          envelope_f(rr[k], a.r_cut, uu[k], du);
+          flag = e == 0 || a.recv[ge - 1] != rc[k];
         }
+        M.recv[e] = rc[k]; M.send[e] = sd; M.w[e] = a.alpha * uu[k];
+        M.r[e] = rr[k]; M.u[e] = uu[k]; M.du[e] = du;
+        fm[k] = __ballot_sync(0xffffffffu, flag);
       }
-    }
-    tc::cp_async_commit();
-    tc::cp_async_wait<0>();
-    tc::fence_proxy_async();
-    __syncthreads();
-
-    // ---- G1: D1 = e_hat . W1c^T ----
-    if (tid == 0) {
-      tc::fence_after_sync();
-      const uint64_t ad = tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE);
-      const uint64_t bd = tc::smem_desc(base + SM::w1c, 128, 256, tc::LAYOUT_NONE);
-      tc::mma_bf16(tmem, ad, bd, IDESC_ND, false);
-      tc::mma_commit(bar);
-    }
-    tc::mbar_wait(bar, phase); phase ^= 1;
-    tc::fence_after_sync();
-
-    // ---- E1: a = D1 + P_i + Q_j ; s = SiLU(a) ----
-    const int rc = recv_s[row];
-    const bool valid = rc >= 0;
-    {
-      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp;
-#pragma unroll 1
-      for (int c0 = hf * (D / 2); c0 < (hf + 1) * (D / 2); c0 += 32) {
-        float acc[32];
-        tc::tmem_ld32(tlane + (uint32_t)c0, acc);
+      int rloc[4];
+      int before = 0;
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          unsigned char* sp = S + tc::sw128_chunk_off(TE, row, (c0 >> 3) + g);
-          const uint4 qv = *reinterpret_cast<const uint4*>(sp);
-          uint4 outv = make_uint4(0u, 0u, 0u, 0u);
-          if (valid) {
-            const float4 p0 = *reinterpret_cast<const float4*>(Prow + c0 + 8 * g);
-            const float4 p1 = *reinterpret_cast<const float4*>(Prow + c0 + 8 * g + 4);
-            const float pv[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
-            const float qf[8] = {tc::bf16_lo(qv.x), tc::bf16_hi(qv.x), tc::bf16_lo(qv.y), tc::bf16_hi(qv.y),
-                                 tc::bf16_lo(qv.z), tc::bf16_hi(qv.z), tc::bf16_lo(qv.w), tc::bf16_hi(qv.w)};
-            float sv[8];
+      for (int k = 0; k < 4; ++k) {
+        rloc[k] = before + __popc(fm[k] & (0xffffffffu >> (31 - lane))) - 1;
+        if (((fm[k] >> lane) & 1u) && rloc[k] < MAX_SEG) {
+          const int64_t s0 = a.rowptr[rc[k]], s1 = a.rowptr[rc[k] + 1];
+          M.rid[rloc[k]] = rc[k];
+          M.cls[rloc[k]] = (s0 >= e0 && s1 <= e0 + TE) ? 0 : (s0 < e0 ? 1 : 2);
+        }
+        before += __popc(fm[k]);
+      }
+      if (lane == 0) M.R = before;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_META_FULL + b));
+
+      // e_hat operand of G1: K-major, no swizzle: (row, k) -> (row/8)*256 + (k/8)*128 + (row%8)*16 + (k%8)*2
+      if (it > 0) tc::mbar_wait(bar(B_D1_FULL), (uint32_t)((it - 1) & 1));
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              float ds;
-              silu_both_f(acc[8 * g + j] + pv[j] + qf[j], sv[j], ds);
-              acc[8 * g + j] = ds;
-            }
-            outv = make_uint4(tc::pack_bf16(sv[0], sv[1]), tc::pack_bf16(sv[2], sv[3]), tc::pack_bf16(sv[4], sv[5]),
-                              tc::pack_bf16(sv[6], sv[7]));
+      for (int k = 0; k < 4; ++k) {
+        const int e = lane + 32 * k;
+        uint32_t pk[8];
+#pragma unroll
+        for (int j = 0; j < 16; j += 2) {
+          const float d0 = rr[k] - (float)j * delta, d1 = rr[k] - (float)(j + 1) * delta;
+          const float g0 = (rc[k] >= 0 && j < a.n_rbf) ? uu[k] * exp2f(ngl2 * d0 * d0) : 0.f;
+          const float g1 = (rc[k] >= 0 && j + 1 < a.n_rbf) ? uu[k] * exp2f(ngl2 * d1 * d1) : 0.f;
+          pk[j >> 1] = tc::pack_bf16(g0, g1);
+        }
+        unsigned char* dst = gen + SM::ehat + (e >> 3) * 256 + (e & 7) * 16;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        *reinterpret_cast<uint4*>(dst + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
+      }
+      tc::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_EHAT_FULL));
+
+      // selector operand of GS: Sel[r][e] = 1 if edge e belongs to the r-th receiver of the tile;
+      // K-major (K = edge), no swizzle: (r, e) -> (r/8)*2048 + (e/8)*128 + (r%8)*16 + (e%8)*2
+      if (it > 0) tc::mbar_wait(bar(B_SEG_FULL), (uint32_t)((it - 1) & 1));
+      {
+        uint4* z = reinterpret_cast<uint4*>(gen + SM::sel);
+#pragma unroll
+        for (int i = 0; i < MAX_SEG * TE * 2 / 16 / 32; ++i) z[lane + 32 * i] = make_uint4(0u, 0u, 0u, 0u);
+      }
+      __syncwarp();
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int e = lane + 32 * k;
+        if (rc[k] >= 0 && rloc[k] < MAX_SEG)
+          *reinterpret_cast<unsigned short*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 +
+                                             (e & 7) * 2) = (unsigned short)0x3F80;  // bf16 1.0
+      }
+      tc::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_SEL_FULL));
+    }
+  } else if (warp == WARP_MMA) {
+    // =========================== MMA issuer (one thread) ===========================
+    if (lane == 0) {
+      constexpr uint32_t IDESC_ND = tc::idesc_bf16(128, D, 0, 0);     // K-major A and B, N = D
+      constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);  // B read MN-major
+      constexpr uint32_t IDESC_N16 = tc::idesc_bf16(128, 16, 0, 0);
+      constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);   // A read MN-major (M = channel, K = edge)
+      uint32_t srp = 0;  // bit s: parity of the next completion of S_READY[s]
+      auto wait_slab = [&](int s) {
+        tc::mbar_wait(bar(B_S_READY + s), (srp >> s) & 1u);
+        srp ^= 1u << s;
+        tc::fence_after_sync();
+      };
+      int it = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int b = it & 1;
+        tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)(it & 1));
+        tc::mbar_wait(bar(B_X_FREE), (uint32_t)((it & 1) ^ 1));
+        tc::fence_after_sync();
+        // G1
+        tc::mma_bf16(TX, tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE),
+                     tc::smem_desc(base + SM::w1c, 128, 256, tc::LAYOUT_NONE), IDESC_ND, false);
+        tc::mma_commit(bar(B_D1_FULL));
+        // G2, one K slab at a time
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          wait_slab(s);
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)
+            tc::mma_bf16(TY, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
+                         tc::smem_desc(base + SM::w2 + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC_ND,
+                         (s | kk) != 0);
+        }
+        tc::mma_commit(bar(B_D2_FULL));
+        if (BWD) {
+          // G3: X = pbar . W2 (W2 image as MN-major B: LBO = slab stride, 16 k-rows = 2 KB)
+#pragma unroll
+          for (int s = 0; s < NCH; ++s) {
+            wait_slab(s);
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)
+              tc::mma_bf16(TX, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
+                           tc::smem_desc(base + SM::w2 + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128), IDESC_ND_BT,
+                           (s | kk) != 0);
           }
-          *reinterpret_cast<uint4*>(sp) = outv;
+          tc::mma_commit(bar(B_D3_FULL));
         }
-        if (BWD) tc::tmem_st32(tlane + (uint32_t)c0, acc);  // keep SiLU'(a) for E3
-      }
-      if (BWD) tc::tmem_wait_st();
-    }
-    tc::fence_proxy_async();
-    tc::fence_before_sync();
-    __syncthreads();
-
-    // ---- G2: D2 = S . W2^T ----
-    if (tid == 0) {
-      tc::fence_after_sync();
+        tc::mbar_wait(bar(B_SEL_FULL), (uint32_t)(it & 1));
+        const bool seg_mma = *reinterpret_cast<volatile int*>(&meta[b].R) <= MAX_SEG;
 #pragma unroll
-      for (int kk = 0; kk < D / 16; ++kk) {
-        const uint64_t ad = tc::smem_desc(base + SM::s + (kk >> 2) * (TE * 128) + (kk & 3) * 32, 16, 1024, tc::LAYOUT_SW128);
-        const uint64_t bd = tc::smem_desc(base + SM::w2 + (kk >> 2) * (D * 128) + (kk & 3) * 32, 16, 1024, tc::LAYOUT_SW128);
-        tc::mma_bf16(tmem + D, ad, bd, IDESC_ND, kk != 0);
-      }
-      tc::mma_commit(bar);
-    }
-    tc::mbar_wait(bar, phase); phase ^= 1;
-    tc::fence_after_sync();
-
-    if (!BWD) {
-      // ---- E2 forward: alpha u_e SiLU(p) -> S tile, then segmented column sums ----
-      const float w = valid ? a.alpha * u_s[row] : 0.f;
-#pragma unroll 1
-      for (int c0 = hf * (D / 2); c0 < (hf + 1) * (D / 2); c0 += 32) {
-        float acc[32];
-        tc::tmem_ld32(tlane + (uint32_t)(D + c0), acc);
+        for (int s = 0; s < NCH; ++s) {
+          wait_slab(s);
+          if (BWD) {
+            tc::bulk_s2g(a.abar_bf + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          float v[8];
+            for (int kk = 0; kk < 4; ++kk)  // G4: ebar = abar . W1c
+              tc::mma_bf16(TY + 32, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
+                           tc::smem_desc(base + SM::w1cT + s * 2048 + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC_N16,
+                           (s | kk) != 0);
+          }
+          if ((s & 1) && seg_mma) {  // GS over the 128 channels of slabs s-1, s
 #pragma unroll
-          for (int j = 0; j < 8; ++j) v[j] = w * silu_f(acc[8 * g + j] + b2_s[c0 + 8 * g + j]);
-          *reinterpret_cast<uint4*>(S + tc::sw128_chunk_off(TE, row, (c0 >> 3) + g)) =
-              make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]),
-                         tc::pack_bf16(v[6], v[7]));
+            for (int j = 0; j < TE / 16; ++j)
+              tc::mma_bf16(TY + 16 * (s >> 1),
+                           tc::smem_desc(base + SM::ring + (s - 1) * SLOT_BYTES + j * 2048, SLOT_BYTES, 1024, tc::LAYOUT_SW128),
+                           tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
+          }
         }
+        if (BWD) {
+          tc::bulk_commit();
+          tc::bulk_wait_read0();  // the spill has finished reading the slabs
+        }
+        tc::mma_commit(bar(B_SEG_FULL));
+        mbar_arrive(bar(B_META_EMPTY + b));
       }
+      if (BWD) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
+  } else {
+    // =========================== epilogue warps ===========================
+    const int q = warp & 3, g = warp >> 2;
+    const int row = q * 32 + lane;
+    const uint32_t tlane = (uint32_t)(q * 32) << 16;
+    // byte offsets of this thread's two 16-byte chunks (channels 16g..16g+15 of a slab) inside a slab
+    const uint32_t so0 = (uint32_t)(row * 128 + (((2 * g) ^ (row & 7)) << 4));
+    const uint32_t so1 = (uint32_t)(row * 128 + (((2 * g + 1) ^ (row & 7)) << 4));
+    unsigned char* ring = gen + SM::ring;
+    float* out = BWD ? a.Pbar : a.m;
+    uint32_t ds2[BWD ? NCH * 8 : 1];  // 2 SiLU'(a) of this thread's channels, packed bf16x2
+
+    auto publish = [&](int s) {  // slab s written by this warp: visible to the async proxy, then signal
+      tc::fence_proxy_async();
       tc::fence_before_sync();
-      __syncthreads();
-      if (tid < D) segmented_store_bf16<D>(S, recv_s, a.rowptr, e0, tile, a.m, a.head, a.tail, tid);
-      __syncthreads();
-      continue;
-    }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_S_READY + s));
+    };
+    auto store_slab = [&](int s, const float (&v)[16]) {
+      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so0) =
+          make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
+      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so1) =
+          make_uint4(tc::pack_bf16(v[8], v[9]), tc::pack_bf16(v[10], v[11]), tc::pack_bf16(v[12], v[13]), tc::pack_bf16(v[14], v[15]));
+    };
 
-    // ---- E2 backward: pbar = alpha u mbar_i SiLU'(p) ; ubar_e = alpha <mbar_i, phi_e> ----
-    {
-      const float au = valid ? a.alpha * u_s[row] : 0.f;
-      const float* mrow = a.mbar + (size_t)(valid ? rc : 0) * D;
-      float ub = 0.f;
-#pragma unroll 1
-      for (int c0 = hf * (D / 2); c0 < (hf + 1) * (D / 2); c0 += 32) {
-        float acc[32];
-        tc::tmem_ld32(tlane + (uint32_t)(D + c0), acc);
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int b = it & 1;
+      const uint32_t par = (uint32_t)(it & 1);
+      const TileMeta& M = meta[b];
+      const int64_t e0 = tile * TE;
+      tc::mbar_wait(bar(B_META_FULL + b), (uint32_t)((it >> 1) & 1));
+      const int rc = M.recv[row];
+      const bool valid = rc >= 0;
+      const float w = M.w[row];
+      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
+      const __nv_bfloat16* Qrow = a.Qbf + (size_t)(valid ? M.send[row] : 0) * D + 16 * g;
+      uint4 qn0 = __ldg(reinterpret_cast<const uint4*>(Qrow));
+      uint4 qn1 = __ldg(reinterpret_cast<const uint4*>(Qrow + 8));
+
+      // ---- E1: a' = X + P'_i + Q'_j ; s = a' + a' tanh(a') ----
+      tc::mbar_wait(bar(B_D1_FULL), par);
+      tc::fence_after_sync();
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-          float v[8];
-          float mb[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-          if (valid) {
-            const float4 m0 = *reinterpret_cast<const float4*>(mrow + c0 + 8 * g);
-            const float4 m1 = *reinterpret_cast<const float4*>(mrow + c0 + 8 * g + 4);
-            mb[0] = m0.x; mb[1] = m0.y; mb[2] = m0.z; mb[3] = m0.w; mb[4] = m1.x; mb[5] = m1.y; mb[6] = m1.z; mb[7] = m1.w;
+      for (int s = 0; s < NCH; ++s) {
+        uint32_t acc[16];
+        tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
+        const uint4 q0 = qn0, q1 = qn1;
+        if (s + 1 < NCH) {
+          qn0 = __ldg(reinterpret_cast<const uint4*>(Qrow + 64 * (s + 1)));
+          qn1 = __ldg(reinterpret_cast<const uint4*>(Qrow + 64 * (s + 1) + 8));
+        }
+        float pv[16];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float4 p = __ldg(reinterpret_cast<const float4*>(Prow + 64 * s + 4 * j));
+          pv[4 * j] = p.x; pv[4 * j + 1] = p.y; pv[4 * j + 2] = p.z; pv[4 * j + 3] = p.w;
+        }
+        const uint32_t qw[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+        tc::tmem_wait_ld();
+        float v[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const float qf = (j & 1) ? tc::bf16_hi(qw[j >> 1]) : tc::bf16_lo(qw[j >> 1]);
+          const float x = __uint_as_float(acc[j]) + pv[j] + qf;
+          const float t = tanh_mufu(x);
+          v[j] = fmaf(x, t, x);
+          if (BWD) pv[j] = fmaf(v[j], 1.0f - t, 1.0f + t);  // 2 SiLU'(2x) = (1 + t) + s (1 - t)
+        }
+        store_slab(s, v);
+        if (BWD) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) ds2[s * 8 + j] = tc::pack_bf16(pv[2 * j], pv[2 * j + 1]);
+        }
+        publish(s);
+      }
+      if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
+
+      // ---- E2 ----
+      tc::mbar_wait(bar(B_D2_FULL), par);
+      tc::fence_after_sync();
+      if (!BWD) {
+        // forward: alpha u_e SiLU(p) -> slabs
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          uint32_t acc[16];
+          tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
+          float bv[16];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 p = *reinterpret_cast<const float4*>(b2_s + 64 * s + 16 * g + 4 * j);
+            bv[4 * j] = p.x; bv[4 * j + 1] = p.y; bv[4 * j + 2] = p.z; bv[4 * j + 3] = p.w;
           }
+          tc::tmem_wait_ld();
+          float v[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const float x = __uint_as_float(acc[j]) + bv[j];
+            const float t = tanh_mufu(x);
+            v[j] = w * fmaf(x, t, x);
+          }
+          store_slab(s, v);
+          publish(s);
+        }
+      } else {
+        // backward: pbar = alpha u mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
+        const float* mrow = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        float ub = 0.f;
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          uint32_t acc[16];
+          tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
+          float bv[16], mb[16];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 p = *reinterpret_cast<const float4*>(b2_s + 64 * s + 16 * g + 4 * j);
+            bv[4 * j] = p.x; bv[4 * j + 1] = p.y; bv[4 * j + 2] = p.z; bv[4 * j + 3] = p.w;
+            const float4 m4 = __ldg(reinterpret_cast<const float4*>(mrow + 64 * s + 4 * j));
+            mb[4 * j] = m4.x; mb[4 * j + 1] = m4.y; mb[4 * j + 2] = m4.z; mb[4 * j + 3] = m4.w;
+          }
+          tc::tmem_wait_ld();
+          float v[16];
+#pragma unroll
+          for (int j = 0; j < 16; ++j) {
+            const float x = __uint_as_float(acc[j]) + bv[j];
+            const float t = tanh_mufu(x);
+            const float phi = fmaf(x, t, x);
+            const float dphi = fmaf(phi, fmaf(-0.5f, t, 0.5f), fmaf(0.5f, t, 0.5f));  // sigma + phi (1 - sigma)
+            ub = fmaf(mb[j], phi, ub);
+            v[j] = (w * mb[j]) * dphi;
+          }
+          store_slab(s, v);
+          publish(s);
+        }
+        ubar_s[g * TE + row] = ub;
+
+        // ---- E3: abar = X * 2 SiLU'(a) -> slabs ----
+        tc::mbar_wait(bar(B_D3_FULL), par);
+        tc::fence_after_sync();
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          uint32_t acc[16];
+          tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
+          tc::tmem_wait_ld();
+          float v[16];
 #pragma unroll
           for (int j = 0; j < 8; ++j) {
-            float phi, dphi;
-            silu_both_f(acc[8 * g + j] + b2_s[c0 + 8 * g + j], phi, dphi);
-            ub = fmaf(mb[j], phi, ub);
-            v[j] = au * mb[j] * dphi;
+            v[2 * j] = __uint_as_float(acc[2 * j]) * tc::bf16_lo(ds2[s * 8 + j]);
+            v[2 * j + 1] = __uint_as_float(acc[2 * j + 1]) * tc::bf16_hi(ds2[s * 8 + j]);
           }
-          *reinterpret_cast<uint4*>(S + tc::sw128_chunk_off(TE, row, (c0 >> 3) + g)) =
-              make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]),
-                         tc::pack_bf16(v[6], v[7]));
+          store_slab(s, v);
+          publish(s);
         }
+        if (lane == 0) mbar_arrive(bar(B_X_FREE));
       }
-      ubar_s[hf * TE + row] = ub;
-    }
-    tc::fence_proxy_async();
-    tc::fence_before_sync();
-    __syncthreads();
 
-    // ---- G3: D3 = pbar . W2 (W2 image as MN-major B: LBO = slab stride, 16 k-rows = 2 KB) ----
-    if (tid == 0) {
+      // ---- segment sums (and E4) out of Y ----
+      tc::mbar_wait(bar(B_SEG_FULL), par);
       tc::fence_after_sync();
+      const int R = M.R;
+      if (R <= MAX_SEG) {
+        if (g >= 1 && g <= NCH / 2) {
+          const int h = g - 1;
+          uint32_t acc[16];
+          tmem_ld16_nowait(TY + tlane + (uint32_t)(16 * h), acc);
+          tc::tmem_wait_ld();
+          const int pos = 128 * h + row;
 #pragma unroll
-      for (int kk = 0; kk < D / 16; ++kk) {
-        const uint64_t ad = tc::smem_desc(base + SM::s + (kk >> 2) * (TE * 128) + (kk & 3) * 32, 16, 1024, tc::LAYOUT_SW128);
-        const uint64_t bd = tc::smem_desc(base + SM::w2 + kk * 2048, D * 128, 1024, tc::LAYOUT_SW128);
-        tc::mma_bf16(tmem + D, ad, bd, IDESC_ND_BT, kk != 0);
-      }
-      tc::mma_commit(bar);
-    }
-    tc::mbar_wait(bar, phase); phase ^= 1;
-    tc::fence_after_sync();
-
-    // ---- E3: abar = sbar * SiLU'(a) -> S tile ----
-#pragma unroll 1
-    for (int c0 = hf * (D / 2); c0 < (hf + 1) * (D / 2); c0 += 32) {
-      float sb[32], ds[32];
-      tc::tmem_ld32(tlane + (uint32_t)(D + c0), sb);
-      tc::tmem_ld32(tlane + (uint32_t)c0, ds);
-#pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        float v[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) v[j] = valid ? sb[8 * g + j] * ds[8 * g + j] : 0.f;
-        *reinterpret_cast<uint4*>(S + tc::sw128_chunk_off(TE, row, (c0 >> 3) + g)) =
-            make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]),
-                       tc::pack_bf16(v[6], v[7]));
-      }
-    }
-    tc::fence_proxy_async();
-    tc::fence_before_sync();
-    __syncthreads();
-
-    // ---- spill (bulk copy), G4: D4 = abar . W1c, segmented column sums -> Pbar ----
-    if (tid == 0) {
-      tc::fence_after_sync();
-      tc::bulk_s2g(a.abar_bf + (size_t)tile * TE * D, base + SM::s, TE * D * 2);
-      tc::bulk_commit();
-#pragma unroll
-      for (int kk = 0; kk < D / 16; ++kk) {
-        const uint64_t ad = tc::smem_desc(base + SM::s + (kk >> 2) * (TE * 128) + (kk & 3) * 32, 16, 1024, tc::LAYOUT_SW128);
-        const uint64_t bd = tc::smem_desc(base + SM::w1cT + (kk >> 2) * (16 * 128) + (kk & 3) * 32, 16, 1024, tc::LAYOUT_SW128);
-        tc::mma_bf16(tmem + D, ad, bd, IDESC_N16, kk != 0);
-      }
-      tc::mma_commit(bar);
-    }
-    if (tid < D) segmented_store_bf16<D>(S, recv_s, a.rowptr, e0, tile, a.Pbar, a.head, a.tail, tid);
-    tc::mbar_wait(bar, phase); phase ^= 1;
-    tc::fence_after_sync();
-
-    // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k) ----
-    if (warp < 4) {
-      float eb[16];
-      tc::tmem_ld16(tlane + (uint32_t)D, eb);
-      const float r = r_s[row], u = u_s[row], du = du_s[row];
-      float part = 0.f;
-#pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        if (k < a.n_rbf) {
-          float g, dg;
-          rbf_f(r, a.r_cut, a.n_rbf, k, g, dg);
-          part = fmaf(eb[k], fmaf(du, g, u * dg), part);
+          for (int r = 0; r < MAX_SEG; ++r) {
+            if (r < R) {
+              const int cls = M.cls[r];
+              float* dst = cls == 0 ? out + (size_t)M.rid[r] * D : (cls == 1 ? a.head : a.tail) + (size_t)tile * D;
+              dst[pos] = __uint_as_float(acc[r]);
+            }
+          }
         }
+      } else {
+        named_bar_sync(1, N_EPI_WARPS * 32);
+        if (tid < D) segmented_store_bf16<D>(ring, M.recv, a.rowptr, e0, tile, out, a.head, a.tail, tid);
+        named_bar_sync(1, N_EPI_WARPS * 32);
       }
-      const float ubar = a.alpha * (ubar_s[row] + ubar_s[TE + row]);
-      if (valid) a.rbar[e0 + row] += fmaf(ubar, du, part);
+      if (BWD && g == 0) {
+        // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k) ----
+        uint32_t eb[16];
+        tmem_ld16_nowait(TY + tlane + 32u, eb);
+        tc::tmem_wait_ld();
+        const float r = M.r[row], u = M.u[row], du = M.du[row];
+        float part = 0.f;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+          if (k < a.n_rbf) {
+            float gk, dgk;
+            rbf_f(r, a.r_cut, a.n_rbf, k, gk, dgk);
+            part = fmaf(__uint_as_float(eb[k]), fmaf(du, gk, u * dgk), part);
+          }
+        }
+        const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
+        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, part);
+      }
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_META_EMPTY + b));
     }
-    if (tid == 0) tc::bulk_wait_read0();  // the spill has finished reading the S tile
-    tc::fence_before_sync();
-    __syncthreads();
   }
 
   tc::fence_before_sync();
@@ -421,21 +590,16 @@ __global__ void __launch_bounds__(256) k_gather_rev_bf16(int64_t n, const int32_
   }
 }
 
-template <int D>
-int launch_edge(mlip_ctx* ctx, const EdgeArgs& a, bool bwd) {
+template <int D, bool BWD>
+int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   const int64_t tiles = (a.E + TE - 1) / TE;
   if (tiles == 0) return MLIP_OK;
-  const size_t smem = ES<D>::bytes;
+  const size_t smem = ES<D, BWD>::bytes;
   const unsigned grid = (unsigned)(tiles < ctx->num_sms ? tiles : ctx->num_sms);
-  if (bwd) {
-    MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_bf16<D, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_edge_bf16<D, true><<<grid, 256, smem, ctx->stream>>>(a, tiles);
-  } else {
-    MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_bf16<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k_edge_bf16<D, false><<<grid, 256, smem, ctx->stream>>>(a, tiles);
-  }
+  MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_bf16<D, BWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_edge_bf16<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
   k_segment_fixup_bf16<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
-                                                                               bwd ? a.Pbar : a.m);
+                                                                               BWD ? a.Pbar : a.m);
   ctx->launches += 2;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
@@ -445,14 +609,14 @@ int launch_edge(mlip_ctx* ctx, const EdgeArgs& a, bool bwd) {
 int64_t mlip_edge_bf16_tiles(int64_t E) { return (E + TE - 1) / TE; }
 
 int mlip_edge_forward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a) {
-  if (d == 256) return launch_edge<256>(ctx, a, false);
-  if (d == 128) return launch_edge<128>(ctx, a, false);
+  if (d == 256) return launch_edge_dir<256, false>(ctx, a);
+  if (d == 128) return launch_edge_dir<128, false>(ctx, a);
   ctx->set_error("bf16 edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }
 int mlip_edge_backward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a) {
-  if (d == 256) return launch_edge<256>(ctx, a, true);
-  if (d == 128) return launch_edge<128>(ctx, a, true);
+  if (d == 256) return launch_edge_dir<256, true>(ctx, a);
+  if (d == 128) return launch_edge_dir<128, true>(ctx, a);
   ctx->set_error("bf16 edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }

@@ -180,7 +180,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     const LayerWeights& W = M->layers[l];
     GemmArgs a;
     if (bf) {
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1; a.Y = P[l]; a.ldy = d; a.n = n; a.N = d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Y = P[l]; a.ldy = d; a.n = n; a.N = d;
       W_TRY(gemm(ctx, a));
       a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Ybf = Qb[l]; a.ldy = d; a.n = n; a.N = d;
       W_TRY(gemm(ctx, a));

@@ -14,9 +14,13 @@ __global__ void k_copy_sub(const float* __restrict__ src, int ld, int r0, int c0
   const int sr = r0 + (transpose ? c : r), sc = c0 + (transpose ? r : c);
   dst[(size_t)r * ld_dst + c] = src[(size_t)sr * ld + sc];
 }
-__global__ void k_to_bf16(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, int n) {
+__global__ void k_to_bf16(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, int n, float scale) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) dst[i] = __float2bfloat16_rn(src[i]);
+  if (i < n) dst[i] = __float2bfloat16_rn(scale * src[i]);
+}
+__global__ void k_scale(const float* __restrict__ src, float* __restrict__ dst, int n, float scale) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = scale * src[i];
 }
 }  // namespace
 
@@ -144,8 +148,8 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   auto sub = [&](const float* src, int ld, int r0, int c0, int tr, float* dst, int ld_dst, int rows, int cols) {
     k_copy_sub<<<(rows * cols + 255) / 256, 256, 0, st>>>(src, ld, r0, c0, tr, dst, ld_dst, rows, cols);
   };
-  auto tobf = [&](const float* src, __nv_bfloat16* dst, int cnt) {
-    k_to_bf16<<<(cnt + 255) / 256, 256, 0, st>>>(src, dst, cnt);
+  auto tobf = [&](const float* src, __nv_bfloat16* dst, int cnt, float scale = 1.0f) {
+    k_to_bf16<<<(cnt + 255) / 256, 256, 0, st>>>(src, dst, cnt, scale);
   };
   for (int l = 0; l < L; ++l) {
     LayerWeights& W = M->layers[l];
@@ -179,7 +183,10 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     M_ALLOC(W.V1_bf, __nv_bfloat16, 2 * d * d); M_ALLOC(W.V2_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V2T_bf, __nv_bfloat16, d * d); M_ALLOC(W.V1aT_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V1bT_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1abT_bf, __nv_bfloat16, 2 * d * d);
-    tobf(W.W1ab, W.W1a_bf, d * d); tobf(W.W1ab + (size_t)d * d, W.W1b_bf, d * d);
+    // the bf16 edge kernels consume HALVED pre-projections P' = (W1a h + b1)/2, Q' = (W1b h)/2 (exact scaling)
+    tobf(W.W1ab, W.W1a_bf, d * d, 0.5f); tobf(W.W1ab + (size_t)d * d, W.W1b_bf, d * d, 0.5f);
+    M_ALLOC(W.b1h, float, d);
+    k_scale<<<(d + 255) / 256, 256, 0, st>>>(W.b1, W.b1h, d, 0.5f);
     tobf(W.V1, W.V1_bf, 2 * d * d); tobf(W.V2, W.V2_bf, d * d); tobf(W.V2T, W.V2T_bf, d * d);
     tobf(W.V1aT, W.V1aT_bf, d * d); tobf(W.V1bT, W.V1bT_bf, d * d); tobf(W.W1abT, W.W1abT_bf, 2 * d * d);
     // operand images of the fused edge kernels (tc_images.cuh documents the layouts)

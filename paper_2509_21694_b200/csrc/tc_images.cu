@@ -7,13 +7,12 @@ __global__ void k_edge_images(const float* __restrict__ W2, const float* __restr
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < d * d) {
     const int o = idx / d, i = idx % d;
-    W2img[tc_sw128_index(d, o, i)] = __float2bfloat16_rn(W2[idx]);
+    W2img[tc_sw128_index(d, o, i)] = __float2bfloat16_rn(0.5f * W2[idx]);  // exact: power of two
   }
   if (idx < d * 16) {
     const int c = idx / 16, k = idx % 16;
-    const __nv_bfloat16 v = __float2bfloat16_rn(W1c[idx]);
-    W1cimg[tc_nosw_index(16, c, k)] = v;
-    W1cTimg[tc_sw128_index(16, k, c)] = v;
+    W1cimg[tc_nosw_index(16, c, k)] = __float2bfloat16_rn(0.5f * W1c[idx]);
+    W1cTimg[tc_sw128_index(16, k, c)] = __float2bfloat16_rn(W1c[idx]);
   }
 }
 }  // namespace

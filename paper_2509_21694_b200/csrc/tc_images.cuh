@@ -22,8 +22,10 @@ __host__ __device__ inline int tc_nosw_index(int K, int r, int k) {
   return (r >> 3) * (K >> 3) * 64 + (k >> 3) * 64 + (r & 7) * 8 + (k & 7);
 }
 
-// W2 [d,d] row-major [out,in] -> W2img  : SW128 K-major, rows = out, K = in
-// W1c [d,16] (padded)         -> W1cimg : no-swizzle K-major, rows = channel, K = 16
-//                             -> W1cTimg: SW128 K-major, rows = rbf index (16), K = channel
+// The edge kernels evaluate SiLU(2x) = x + x tanh(x) on HALVED pre-activations, so the operands
+// that produce pre-activations carry an exact factor 1/2:
+// W2 [d,d] row-major [out,in] -> W2img  : SW128 K-major, rows = out, K = in, values W2/2
+// W1c [d,16] (padded)         -> W1cimg : no-swizzle K-major, rows = channel, K = 16, values W1c/2
+//                             -> W1cTimg: SW128 K-major, rows = rbf index (16), K = channel, values W1c
 void mlip_make_edge_images(cudaStream_t st, const float* W2, const float* W1c, int d,
                            __nv_bfloat16* W2img, __nv_bfloat16* W1cimg, __nv_bfloat16* W1cTimg);
