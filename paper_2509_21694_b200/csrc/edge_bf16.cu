@@ -6,8 +6,9 @@
 //   warps 0..15  epilogue: thread = (edge row, 16 of every 64 channels); TMEM -> registers -> SiLU ->
 //                bf16 operand slab in shared memory, chunk by chunk (64 channels = one SW128 slab)
 //   warp 16      one thread issues every tcgen05.mma as soon as the slab it needs is published
-//   warp 17      producer, one tile ahead: edge metadata, envelope, radial basis (A6), the bf16 e_hat
-//                operand, the receiver-selector operand of the segmented sum
+//   warp 17      segment producer: receivers of the next tile, the 0/1 selector operand of the segmented sum
+//   warps 18,19  feature producers, up to two tiles ahead: edge metadata, envelope, radial basis (A6), the
+//                bf16 e_hat operand of G1
 // Per tile (all factors 1/2 of the SiLU arguments are folded into the weight images, so that
 // SiLU(2x) = x + x tanh(x) costs one MUFU and one FMA):
 //   G1  X[edge, c]  = e_hat . (W1c/2)^T                                  M128 N=d K16
@@ -32,16 +33,18 @@
 namespace {
 constexpr int TE = 128;          // edges per tile = MMA M
 constexpr int N_EPI_WARPS = 16;  // 4 lane quarters x 4 column groups
-constexpr int WARP_MMA = 16, WARP_PROD = 17;
-constexpr int N_THREADS = 18 * 32;
+constexpr int WARP_MMA = 16, WARP_SEG = 17, WARP_FEAT = 18, N_FEAT_WARPS = 2;
+constexpr int N_THREADS = 20 * 32;
 constexpr int SLOT_BYTES = TE * 128;  // one [128 x 64] bf16 SW128 slab
 constexpr int MAX_SEG = 16;           // receivers per tile handled by the selector MMA
 
-struct TileMeta {       // written by the producer warp, double buffered
+struct TileMeta {       // written by the feature producers, double buffered
   int recv[TE];         // local receiver (-1 beyond E)
   int send[TE];
   float w[TE];          // alpha * u(r_e)   (0 beyond E)
   float r[TE], u[TE], du[TE];
+};
+struct TileSeg {        // written by the segment producer, double buffered
   int rid[MAX_SEG];     // receivers of the tile in order of appearance
   int cls[MAX_SEG];     // 0: segment complete inside the tile, 1: continues from an earlier tile, 2: into a later one
   int R;                // number of distinct receivers in the tile
@@ -59,7 +62,8 @@ struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
   static constexpr uint32_t sel = ehat + TE * 16 * 2;                 // [16 x 128] bf16, K-major no swizzle
   static constexpr uint32_t b2 = sel + MAX_SEG * TE * 2;              // [D] fp32 (b2/2)
   static constexpr uint32_t meta = b2 + D * 4;                        // TileMeta[2]
-  static constexpr uint32_t ubar = meta + 2 * sizeof(TileMeta);       // [4][128] fp32 (backward)
+  static constexpr uint32_t seg = meta + 2 * sizeof(TileMeta);        // TileSeg[2]
+  static constexpr uint32_t ubar = seg + 2 * sizeof(TileSeg);         // [4][128] fp32 (backward)
   static constexpr uint32_t bars = ubar + (BWD ? 4 * TE * 4 : 0);     // mbarriers
   static constexpr uint32_t slot = bars + 32 * 8;                     // TMEM base address
   static constexpr uint32_t bytes = slot + 16 + 1024;                 // + alignment slack
@@ -68,7 +72,7 @@ struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
 
 // barrier indices
 enum { B_META_FULL = 0, B_META_EMPTY = 2, B_EHAT_FULL = 4, B_SEL_FULL = 5, B_D1_FULL = 6, B_D2_FULL = 7,
-       B_D3_FULL = 8, B_SEG_FULL = 9, B_X_FREE = 10, B_S_READY = 11 /* .. +NCH */ };
+       B_D3_FULL = 8, B_SEG_FULL = 9, B_SPILL_DONE = 10, B_X_FREE = 11, B_S_READY = 12 /* .. +NCH */ };
 
 __device__ __forceinline__ float tanh_mufu(float x) {
   float y;
@@ -77,6 +81,17 @@ __device__ __forceinline__ float tanh_mufu(float x) {
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// read-only global load that keeps its place among the other asm volatile statements (prefetch distance)
+__device__ __forceinline__ uint4 ldg_nc_v4(const void* p) {
+  uint4 v;
+  asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
 }
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&r)[16]) {
@@ -128,6 +143,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
   const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
   unsigned char* gen = smem_raw + (base - tc::smem_u32(smem_raw));
   TileMeta* meta = reinterpret_cast<TileMeta*>(gen + SM::meta);
+  TileSeg* seg = reinterpret_cast<TileSeg*>(gen + SM::seg);
   float* b2_s = reinterpret_cast<float*>(gen + SM::b2);
   float* ubar_s = reinterpret_cast<float*>(gen + SM::ubar);
   uint32_t* slot = reinterpret_cast<uint32_t*>(gen + SM::slot);
@@ -151,11 +167,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
     for (int i = tid; i < D; i += N_THREADS) b2_s[i] = 0.5f * a.b2[i];
   }
   if (tid == 0) {
-    tc::mbar_init(bar(B_META_FULL), 1); tc::mbar_init(bar(B_META_FULL + 1), 1);
-    tc::mbar_init(bar(B_META_EMPTY), N_EPI_WARPS + 1); tc::mbar_init(bar(B_META_EMPTY + 1), N_EPI_WARPS + 1);
-    tc::mbar_init(bar(B_EHAT_FULL), 1); tc::mbar_init(bar(B_SEL_FULL), 1);
+    tc::mbar_init(bar(B_META_FULL), N_FEAT_WARPS); tc::mbar_init(bar(B_META_FULL + 1), N_FEAT_WARPS);
+    tc::mbar_init(bar(B_META_EMPTY), N_EPI_WARPS); tc::mbar_init(bar(B_META_EMPTY + 1), N_EPI_WARPS);
+    tc::mbar_init(bar(B_EHAT_FULL), N_FEAT_WARPS); tc::mbar_init(bar(B_SEL_FULL), 1);
     tc::mbar_init(bar(B_D1_FULL), 1); tc::mbar_init(bar(B_D2_FULL), 1); tc::mbar_init(bar(B_D3_FULL), 1);
-    tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
+    tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_SPILL_DONE), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
     for (int s = 0; s < NCH; ++s) tc::mbar_init(bar(B_S_READY + s), N_EPI_WARPS);
     tc::fence_mbar_init();
   }
@@ -167,75 +183,96 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
   const uint32_t tmem = *slot;
   const uint32_t TX = tmem, TY = tmem + D;  // accumulator regions: X = D1 / D3, Y = D2 / (segment sums, D4)
 
-  if (warp == WARP_PROD) {
-    // =========================== producer: tile metadata, e_hat, selector ===========================
+  if (warp >= WARP_FEAT) {
+    // ============ feature producers: tile metadata (two tiles ahead) and the e_hat operand ============
     const float delta = a.r_cut / (float)(a.n_rbf - 1);
     const float ngl2 = -(0.5f / (delta * delta)) * 1.4426950408889634f;  // -gamma log2(e)
+    const float inv_rc = 1.0f / a.r_cut;
+    const int ebase = (warp - WARP_FEAT) * 64 + lane;  // this lane's edges: ebase, ebase + 32
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
       TileMeta& M = meta[b];
+      const int64_t e0 = tile * TE;
+      int rc[2], sd[2];
+      float rr[2];
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int64_t ge = e0 + ebase + 32 * k;
+        rc[k] = -1; sd[k] = 0; rr[k] = 0.f;
+        if (ge < a.E) { rc[k] = a.recv[ge]; sd[k] = a.send[ge]; rr[k] = a.rvec[ge].w; }
+      }
       tc::mbar_wait(bar(B_META_EMPTY + b), (uint32_t)(((it >> 1) & 1) ^ 1));
+      uint32_t pk[2][8];
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int e = ebase + 32 * k;
+        float u = 0.f, du = 0.f;
+        if (rc[k] >= 0) {
+          float sn, cs;
+          __sincosf(3.14159265358979f * rr[k] * inv_rc, &sn, &cs);  // argument in [0, pi]
+          u = 0.5f * (cs + 1.0f);
+          du = -(1.5707963267948966f * inv_rc) * sn;
+        }
+        M.recv[e] = rc[k]; M.send[e] = sd[k]; M.w[e] = a.alpha * u;
+        M.r[e] = rr[k]; M.u[e] = u; M.du[e] = du;
+#pragma unroll
+        for (int j = 0; j < 16; j += 2) {
+          const float d0 = rr[k] - (float)j * delta, d1 = rr[k] - (float)(j + 1) * delta;
+          const float g0 = j < a.n_rbf ? u * ex2_approx(ngl2 * d0 * d0) : 0.f;
+          const float g1 = j + 1 < a.n_rbf ? u * ex2_approx(ngl2 * d1 * d1) : 0.f;
+          pk[k][j >> 1] = tc::pack_bf16(g0, g1);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_META_FULL + b));
+      // e_hat operand of G1: K-major, no swizzle: (row, k) -> (row/8)*256 + (k/8)*128 + (row%8)*16 + (k%8)*2
+      if (it > 0) tc::mbar_wait(bar(B_D1_FULL), (uint32_t)((it - 1) & 1));  // G1 of the previous tile has read it
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        const int e = ebase + 32 * k;
+        unsigned char* dst = gen + SM::ehat + (e >> 3) * 256 + (e & 7) * 16;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(pk[k][0], pk[k][1], pk[k][2], pk[k][3]);
+        *reinterpret_cast<uint4*>(dst + 128) = make_uint4(pk[k][4], pk[k][5], pk[k][6], pk[k][7]);
+      }
+      tc::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_EHAT_FULL));
+    }
+  } else if (warp == WARP_SEG) {
+    // ============ segment producer: receivers of the tile and the selector operand of GS ============
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int b = it & 1;
+      TileSeg& G = seg[b];
       const int64_t e0 = tile * TE;
       int rc[4];
-      float rr[4], uu[4];
       uint32_t fm[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int e = lane + 32 * k;
         const int64_t ge = e0 + e;
-        int sd = 0;
-        float du = 0.f;
         bool flag = false;
-        rc[k] = -1; rr[k] = 0.f; uu[k] = 0.f;
+        rc[k] = -1;
         if (ge < a.E) {
-          rc[k] = a.recv[ge]; sd = a.send[ge]; rr[k] = a.rvec[ge].w;
-          envelope_f(rr[k], a.r_cut, uu[k], du);
+          rc[k] = a.recv[ge];
           flag = e == 0 || a.recv[ge - 1] != rc[k];
         }
-        M.recv[e] = rc[k]; M.send[e] = sd; M.w[e] = a.alpha * uu[k];
-        M.r[e] = rr[k]; M.u[e] = uu[k]; M.du[e] = du;
         fm[k] = __ballot_sync(0xffffffffu, flag);
       }
-      int rloc[4];
+      int rloc[4], cls[4];
       int before = 0;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         rloc[k] = before + __popc(fm[k] & (0xffffffffu >> (31 - lane))) - 1;
+        cls[k] = -1;
         if (((fm[k] >> lane) & 1u) && rloc[k] < MAX_SEG) {
           const int64_t s0 = a.rowptr[rc[k]], s1 = a.rowptr[rc[k] + 1];
-          M.rid[rloc[k]] = rc[k];
-          M.cls[rloc[k]] = (s0 >= e0 && s1 <= e0 + TE) ? 0 : (s0 < e0 ? 1 : 2);
+          cls[k] = (s0 >= e0 && s1 <= e0 + TE) ? 0 : (s0 < e0 ? 1 : 2);
         }
         before += __popc(fm[k]);
       }
-      if (lane == 0) M.R = before;
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_META_FULL + b));
-
-      // e_hat operand of G1: K-major, no swizzle: (row, k) -> (row/8)*256 + (k/8)*128 + (row%8)*16 + (k%8)*2
-      if (it > 0) tc::mbar_wait(bar(B_D1_FULL), (uint32_t)((it - 1) & 1));
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int e = lane + 32 * k;
-        uint32_t pk[8];
-#pragma unroll
-        for (int j = 0; j < 16; j += 2) {
-          const float d0 = rr[k] - (float)j * delta, d1 = rr[k] - (float)(j + 1) * delta;
-          const float g0 = (rc[k] >= 0 && j < a.n_rbf) ? uu[k] * exp2f(ngl2 * d0 * d0) : 0.f;
-          const float g1 = (rc[k] >= 0 && j + 1 < a.n_rbf) ? uu[k] * exp2f(ngl2 * d1 * d1) : 0.f;
-          pk[j >> 1] = tc::pack_bf16(g0, g1);
-        }
-        unsigned char* dst = gen + SM::ehat + (e >> 3) * 256 + (e & 7) * 16;
-        *reinterpret_cast<uint4*>(dst) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
-        *reinterpret_cast<uint4*>(dst + 128) = make_uint4(pk[4], pk[5], pk[6], pk[7]);
-      }
-      tc::fence_proxy_async();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_EHAT_FULL));
-
-      // selector operand of GS: Sel[r][e] = 1 if edge e belongs to the r-th receiver of the tile;
-      // K-major (K = edge), no swizzle: (r, e) -> (r/8)*2048 + (e/8)*128 + (r%8)*16 + (e%8)*2
+      // the selector buffer (and seg[b], last read two tiles ago) is free once GS of the previous tile is done
       if (it > 0) tc::mbar_wait(bar(B_SEG_FULL), (uint32_t)((it - 1) & 1));
       {
         uint4* z = reinterpret_cast<uint4*>(gen + SM::sel);
@@ -243,13 +280,17 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         for (int i = 0; i < MAX_SEG * TE * 2 / 16 / 32; ++i) z[lane + 32 * i] = make_uint4(0u, 0u, 0u, 0u);
       }
       __syncwarp();
+      // Sel[r][e] = 1 if edge e belongs to the r-th receiver of the tile; K-major (K = edge), no swizzle:
+      // (r, e) -> (r/8)*2048 + (e/8)*128 + (r%8)*16 + (e%8)*2
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int e = lane + 32 * k;
+        if (cls[k] >= 0) { G.rid[rloc[k]] = rc[k]; G.cls[rloc[k]] = cls[k]; }
         if (rc[k] >= 0 && rloc[k] < MAX_SEG)
           *reinterpret_cast<unsigned short*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 +
                                              (e & 7) * 2) = (unsigned short)0x3F80;  // bf16 1.0
       }
+      if (lane == 0) G.R = before;
       tc::fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_SEL_FULL));
@@ -267,16 +308,19 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         srp ^= 1u << s;
         tc::fence_after_sync();
       };
-      int it = 0;
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        const int b = it & 1;
-        tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)(it & 1));
-        tc::mbar_wait(bar(B_X_FREE), (uint32_t)((it & 1) ^ 1));
+      auto issue_g1 = [&](int jt) {  // G1 of this CTA's jt-th tile: needs its e_hat and region X released by tile jt-1
+        tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)(jt & 1));
+        tc::mbar_wait(bar(B_X_FREE), (uint32_t)((jt & 1) ^ 1));
         tc::fence_after_sync();
-        // G1
         tc::mma_bf16(TX, tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE),
                      tc::smem_desc(base + SM::w1c, 128, 256, tc::LAYOUT_NONE), IDESC_ND, false);
         tc::mma_commit(bar(B_D1_FULL));
+      };
+      int it = 0;
+      issue_g1(0);
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int b = it & 1;
+        const bool has_next = tile + gridDim.x < n_tiles;
         // G2, one K slab at a time
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
@@ -288,6 +332,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
                          (s | kk) != 0);
         }
         tc::mma_commit(bar(B_D2_FULL));
+        if (!BWD && has_next) issue_g1(it + 1);  // forward: X is dead after E1, run G1 of the next tile under E2
         if (BWD) {
           // G3: X = pbar . W2 (W2 image as MN-major B: LBO = slab stride, 16 k-rows = 2 KB)
 #pragma unroll
@@ -302,7 +347,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           tc::mma_commit(bar(B_D3_FULL));
         }
         tc::mbar_wait(bar(B_SEL_FULL), (uint32_t)(it & 1));
-        const bool seg_mma = *reinterpret_cast<volatile int*>(&meta[b].R) <= MAX_SEG;
+        const bool seg_mma = *reinterpret_cast<volatile int*>(&seg[b].R) <= MAX_SEG;
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           wait_slab(s);
@@ -322,12 +367,13 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
                            tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
           }
         }
+        tc::mma_commit(bar(B_SEG_FULL));
         if (BWD) {
+          if (has_next) issue_g1(it + 1);  // backward: X (D3) is released by the last E3 read
           tc::bulk_commit();
           tc::bulk_wait_read0();  // the spill has finished reading the slabs
+          mbar_arrive(bar(B_SPILL_DONE));
         }
-        tc::mma_commit(bar(B_SEG_FULL));
-        mbar_arrive(bar(B_META_EMPTY + b));
       }
       if (BWD) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
@@ -356,20 +402,24 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           make_uint4(tc::pack_bf16(v[8], v[9]), tc::pack_bf16(v[10], v[11]), tc::pack_bf16(v[12], v[13]), tc::pack_bf16(v[14], v[15]));
     };
 
+    // row metadata and the first Q chunk of a tile are fetched while the previous tile drains
+    tc::mbar_wait(bar(B_META_FULL), 0u);
+    int rc = meta[0].recv[row];
+    float w = meta[0].w[row];
+    const __nv_bfloat16* Qrow = a.Qbf + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
+    uint4 qn0 = ldg_nc_v4(Qrow), qn1 = ldg_nc_v4(Qrow + 8);
+
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
       const uint32_t par = (uint32_t)(it & 1);
       const TileMeta& M = meta[b];
+      const TileSeg& G = seg[b];
       const int64_t e0 = tile * TE;
-      tc::mbar_wait(bar(B_META_FULL + b), (uint32_t)((it >> 1) & 1));
-      const int rc = M.recv[row];
+      const bool has_next = tile + gridDim.x < n_tiles;
       const bool valid = rc >= 0;
-      const float w = M.w[row];
       const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
-      const __nv_bfloat16* Qrow = a.Qbf + (size_t)(valid ? M.send[row] : 0) * D + 16 * g;
-      uint4 qn0 = __ldg(reinterpret_cast<const uint4*>(Qrow));
-      uint4 qn1 = __ldg(reinterpret_cast<const uint4*>(Qrow + 8));
+      if (BWD && it > 0) tc::mbar_wait(bar(B_SPILL_DONE), (uint32_t)((it - 1) & 1));  // slabs of the previous tile spilled
 
       // ---- E1: a' = X + P'_i + Q'_j ; s = a' + a' tanh(a') ----
       tc::mbar_wait(bar(B_D1_FULL), par);
@@ -380,8 +430,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
         const uint4 q0 = qn0, q1 = qn1;
         if (s + 1 < NCH) {
-          qn0 = __ldg(reinterpret_cast<const uint4*>(Qrow + 64 * (s + 1)));
-          qn1 = __ldg(reinterpret_cast<const uint4*>(Qrow + 64 * (s + 1) + 8));
+          qn0 = ldg_nc_v4(Qrow + 64 * (s + 1));
+          qn1 = ldg_nc_v4(Qrow + 64 * (s + 1) + 8);
         }
         float pv[16];
 #pragma unroll
@@ -487,10 +537,22 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         if (lane == 0) mbar_arrive(bar(B_X_FREE));
       }
 
+      // ---- next tile: row metadata and first Q chunk (in flight during the read-out below) ----
+      int rc_n = -1;
+      float w_n = 0.f;
+      if (has_next) {
+        tc::mbar_wait(bar(B_META_FULL + (b ^ 1)), (uint32_t)(((it + 1) >> 1) & 1));
+        rc_n = meta[b ^ 1].recv[row];
+        w_n = meta[b ^ 1].w[row];
+        Qrow = a.Qbf + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
+        qn0 = ldg_nc_v4(Qrow);
+        qn1 = ldg_nc_v4(Qrow + 8);
+      }
+
       // ---- segment sums (and E4) out of Y ----
       tc::mbar_wait(bar(B_SEG_FULL), par);
       tc::fence_after_sync();
-      const int R = M.R;
+      const int R = G.R;
       if (R <= MAX_SEG) {
         if (g >= 1 && g <= NCH / 2) {
           const int h = g - 1;
@@ -501,8 +563,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
 #pragma unroll
           for (int r = 0; r < MAX_SEG; ++r) {
             if (r < R) {
-              const int cls = M.cls[r];
-              float* dst = cls == 0 ? out + (size_t)M.rid[r] * D : (cls == 1 ? a.head : a.tail) + (size_t)tile * D;
+              const int cls = G.cls[r];
+              float* dst = cls == 0 ? out + (size_t)G.rid[r] * D : (cls == 1 ? a.head : a.tail) + (size_t)tile * D;
               dst[pos] = __uint_as_float(acc[r]);
             }
           }
@@ -533,6 +595,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
       tc::fence_before_sync();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_META_EMPTY + b));
+      rc = rc_n;
+      w = w_n;
     }
   }
 
