@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 #include <string>
 #include <vector>
@@ -108,7 +109,7 @@ struct LayerWeights {
   float* b1pad;   // [2d] = [b1 | 0]
   float* b1h;     // [d] = b1 / 2 (bias of the halved receiver pre-projection of the bf16 path)
   // bf16 operand images for the tensor-core path (device, owned); see tc_common.cuh
-  __nv_bfloat16 *W2img, *W1cimg, *W1cTimg;
+  __half *W2img, *W1cimg;
   __nv_bfloat16 *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;
 };
 
@@ -195,6 +196,7 @@ struct GemmArgs {
   const float* residual = nullptr; int ldr = 0;   // epilogue: y += R[row, col] (may alias Y)
   float* Y = nullptr; int ldy = 0;                // fp32 output (or)
   __nv_bfloat16* Ybf = nullptr;                   // bf16 output (same ldy)
+  __half* Yh = nullptr;                           // f16 output (same ldy)
   int64_t n = 0; int N = 0;
 };
 int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a);

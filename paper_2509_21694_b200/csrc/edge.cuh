@@ -1,5 +1,6 @@
 // Argument block and launchers of the fused edge kernels (fp32 CUDA-core and bf16 tcgen05 paths).
 #pragma once
+#include <cuda_fp16.h>
 #include "common.cuh"
 
 struct EdgeArgs {
@@ -9,13 +10,14 @@ struct EdgeArgs {
   const int32_t* send = nullptr;
   const int32_t* rev = nullptr;
   const float4* rvec = nullptr;
-  const float* P = nullptr; int ldp = 0;           // receiver pre-projection W1a h_i + b1 (fp32)
+  const float* P = nullptr; int ldp = 0;           // receiver pre-projection W1a h_i + b1 (fp32 path)
+  const __half* Ph = nullptr;                      // halved receiver pre-projection (tensor-core path, f16), ld = d
   const float* Q = nullptr; int ldq = 0;           // sender pre-projection W1b h_j (fp32 path)
-  const __nv_bfloat16* Qbf = nullptr;              // sender pre-projection (bf16 path), ld = d
+  const __half* Qh = nullptr;                      // halved sender pre-projection (tensor-core path, f16), ld = d
   const float* W1c = nullptr;                      // [d,16] fp32
   const float* W2T = nullptr;                      // [in,out] fp32
   const float* W2 = nullptr;                       // [out,in] fp32
-  const __nv_bfloat16 *W2img = nullptr, *W1cimg = nullptr, *W1cTimg = nullptr;  // tc_images.cuh
+  const __half *W2img = nullptr, *W1cimg = nullptr;  // f16 operand images, tc_images.cuh
   const float* b2 = nullptr;
   float r_cut = 0.f, alpha = 0.f;
   int n_rbf = 0;
@@ -23,7 +25,7 @@ struct EdgeArgs {
   float *head = nullptr, *tail = nullptr;          // per-tile partial rows [tiles,d]
   const float* mbar = nullptr;                     // backward in [n,d]
   float* abar = nullptr;                           // backward spill [E,d] fp32
-  __nv_bfloat16* abar_bf = nullptr;                // backward spill [E,d] bf16
+  __half* abar_h = nullptr;                        // backward spill, f16 tile images [tiles,128,d]
   float* Pbar = nullptr;                           // backward out [n,d]
   float* rbar = nullptr;                           // [E] accumulated over layers
 };
@@ -34,8 +36,8 @@ int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
                         const float* abar, float* Qbar);
 
-int64_t mlip_edge_bf16_tiles(int64_t E);
-int mlip_edge_forward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a);
-int mlip_edge_backward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a);
-int mlip_gather_rev_bf16(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
-                         const __nv_bfloat16* abar, float* Qbar);
+int64_t mlip_edge_tc_tiles(int64_t E);
+int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
+int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
+                       const __half* abar, float* Qbar);

@@ -1,30 +1,41 @@
-// MLIP_BF16 path of the fused edge kernels (steps A6, A7 and the edge part of A10) on the sm_100a
-// tensor cores: bf16 operands, fp32 accumulation in TMEM.
+// Tensor-core path (precision MLIP_BF16) of the fused edge kernels: steps A6, A7 and the edge part
+// of A10 on the sm_100a tensor cores. 16-bit operands, fp32 accumulation in TMEM.
+//
+// Operand type: IEEE half (f16), not bf16. Same tcgen05 rate and bytes, three more mantissa bits, and
+// -- the reason -- the epilogues can then run in packed f16x2 arithmetic (HADD2/HFMA2, one
+// instruction per two elements) straight from the accumulators to the next operand with no
+// unpack/convert/pack sequence per element: the epilogues, not the MMAs, bound this kernel (MUFU:
+// one tanh per element at 16/clk/SM = 4096 cycles per 128x256 tile pair of epilogues against 2048
+// cycles of tcgen05 per GEMM). Range: |pre-activations| and |adjoints| must stay below 6.5e4.
 //
 // One persistent, warp-specialised CTA per SM walks over tiles of 128 consecutive receiver-sorted
-// edges. The bf16 image of W2 (and the small W1c images) stays resident in shared memory.
+// edges. The f16 image of W2 (and the small W1c image) stays resident in shared memory.
 //   warps 0..15  epilogue: thread = (edge row, 16 of every 64 channels); TMEM -> registers -> SiLU ->
-//                bf16 operand slab in shared memory, chunk by chunk (64 channels = one SW128 slab)
+//                f16 operand slab in shared memory, chunk by chunk (64 channels = one SW128 slab)
 //   warp 16      one thread issues every tcgen05.mma as soon as the slab it needs is published
-//   warp 17      segment producer: receivers of the next tile, the 0/1 selector operand of the segmented sum
+//   warp 17      segment producer: receivers of the tile, the selector operand of the segmented sum,
+//                and the per-tile staging of the receiver rows P_i (and mbar_i) in shared memory
 //   warps 18,19  feature producers, up to two tiles ahead: edge metadata, envelope, radial basis (A6), the
-//                bf16 e_hat operand of G1
+//                f16 e_hat operand of G1
 // Per tile (all factors 1/2 of the SiLU arguments are folded into the weight images, so that
 // SiLU(2x) = x + x tanh(x) costs one MUFU and one FMA):
 //   G1  X[edge, c]  = e_hat . (W1c/2)^T                                  M128 N=d K16
 //   E1  a' = X + P'_i + Q'_j ; s = SiLU(2a') -> slab c/64 ; backward keeps 2 SiLU'(2a') in registers
 //   G2  Y[edge, o] += s . (W2/2)^T      issued per 64-channel K slab while E1 works on the next one
-//   E2  forward : alpha u_e SiLU(2(Y + b2/2)) -> slabs
+//   E2  forward : phi = SiLU(2(Y + b2/2)) -> slabs (the weight alpha u_e rides in the selector of GS)
 //       backward: pbar = alpha u_e mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
 //   G3  X[edge, i] += pbar . (W2/2)     (backward; the SAME W2 image read MN-major), per slab
 //   E3  abar = X * 2 SiLU'(2a') -> slabs -> (i) bulk copy to the spill buffer (read back through
-//       rev[] by k_gather_rev_bf16), (ii) segmented sum, (iii) G4
+//       rev[] by k_gather_rev_tc), (ii) segmented sum, (iii) G4
 //   GS  segmented sum over runs of equal receiver as an MMA: Yseg[channel, r] = slab^T . Sel with the
-//       0/1 selector Sel[edge, r] (M = 128 channels, N = 16 receivers, K = 128 edges); its result is
-//       m_i (forward) / Pbar_i (backward). Tiles with more than 16 receivers take a shared-memory loop.
-//   G4  ebar[edge, k] = abar . W1c  (N = 16) ; E4  rbar_e += ubar_e u' + sum_k ebar_k (u' g_k + u g'_k)
-// Segments that straddle tiles go through per-tile head/tail rows and k_segment_fixup_bf16: no
+//       selector Sel[edge, r] = weight of edge if it belongs to receiver slot r (M = 128 channels,
+//       N = 16 receivers, K = 128 edges); its result is m_i (forward) / Pbar_i (backward). Tiles with
+//       more than 16 receivers take a shared-memory loop.
+//   G4  ebar[edge, k] = abar . (W1c/2)  (N = 16, the W1c image read MN-major)
+//   E4  rbar_e += ubar_e u' + sum_k 2 ebar_k (u' g_k + u g'_k)
+// Segments that straddle tiles go through per-tile head/tail rows and k_segment_fixup_tc: no
 // floating-point atomics anywhere, results are bitwise reproducible.
+#include <cuda_fp16.h>
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
@@ -35,50 +46,53 @@ constexpr int TE = 128;          // edges per tile = MMA M
 constexpr int N_EPI_WARPS = 16;  // 4 lane quarters x 4 column groups
 constexpr int WARP_MMA = 16, WARP_SEG = 17, WARP_FEAT = 18, N_FEAT_WARPS = 2;
 constexpr int N_THREADS = 20 * 32;
-constexpr int SLOT_BYTES = TE * 128;  // one [128 x 64] bf16 SW128 slab
+constexpr int SLOT_BYTES = TE * 128;  // one [128 x 64] f16 SW128 slab
 constexpr int MAX_SEG = 16;           // receivers per tile handled by the selector MMA
+constexpr int NSLOT = 8;              // receivers per tile whose P_i / mbar_i rows are staged in shared memory
 
+template <bool BWD>
 struct TileMeta {       // written by the feature producers, double buffered
   int recv[TE];         // local receiver (-1 beyond E)
   int send[TE];
   float w[TE];          // alpha * u(r_e)   (0 beyond E)
-  float r[TE], u[TE], du[TE];
+  float r[BWD ? TE : 1], u[BWD ? TE : 1], du[BWD ? TE : 1];
 };
 struct TileSeg {        // written by the segment producer, double buffered
   int rid[MAX_SEG];     // receivers of the tile in order of appearance
   int cls[MAX_SEG];     // 0: segment complete inside the tile, 1: continues from an earlier tile, 2: into a later one
   int R;                // number of distinct receivers in the tile
   int pad[3];
+  unsigned char slot[TE];  // receiver slot of every edge row (valid when R <= NSLOT)
 };
 
 template <int D, bool BWD>
 struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
   static constexpr int NCH = D / 64;
-  static constexpr uint32_t w2 = 0;                                   // [D x D] bf16, K-major SW128 image of W2/2
-  static constexpr uint32_t ring = w2 + D * D * 2;                    // NCH slabs [128 x 64] bf16, K-major SW128
-  static constexpr uint32_t w1c = ring + NCH * SLOT_BYTES;            // [D x 16] bf16, K-major no swizzle (W1c/2)
-  static constexpr uint32_t w1cT = w1c + D * 16 * 2;                  // [16 x D] bf16, K-major SW128 (backward)
-  static constexpr uint32_t ehat = w1cT + (BWD ? 16 * D * 2 : 0);     // [128 x 16] bf16, K-major no swizzle
-  static constexpr uint32_t sel = ehat + TE * 16 * 2;                 // [16 x 128] bf16, K-major no swizzle
-  static constexpr uint32_t b2 = sel + MAX_SEG * TE * 2;              // [D] fp32 (b2/2)
-  static constexpr uint32_t meta = b2 + D * 4;                        // TileMeta[2]
-  static constexpr uint32_t seg = meta + 2 * sizeof(TileMeta);        // TileSeg[2]
+  static constexpr uint32_t w2 = 0;                                   // [D x D] f16, K-major SW128 image of W2/2
+  static constexpr uint32_t ring = w2 + D * D * 2;                    // NCH slabs [128 x 64] f16, K-major SW128
+  static constexpr uint32_t w1c = ring + NCH * SLOT_BYTES;            // [D x 16] f16, K-major no swizzle (W1c/2)
+  static constexpr uint32_t ehat = w1c + D * 16 * 2;                  // [128 x 16] f16, K-major no swizzle
+  static constexpr uint32_t sel = ehat + TE * 16 * 2;                 // [16 x 128] f16, K-major no swizzle
+  static constexpr uint32_t ptile = sel + MAX_SEG * TE * 2;           // [NSLOT x D] f16: P'_i of the tile's receivers
+  static constexpr uint32_t mtile = ptile + NSLOT * D * 2;            // [NSLOT x D] f16: mbar_i (backward)
+  static constexpr uint32_t b2 = mtile + (BWD ? NSLOT * D * 2 : 0);   // [D] f16 (b2/2)
+  static constexpr uint32_t meta = b2 + D * 2;                        // TileMeta[2]
+  static constexpr uint32_t seg = meta + 2 * sizeof(TileMeta<BWD>);   // TileSeg[2]
   static constexpr uint32_t ubar = seg + 2 * sizeof(TileSeg);         // [4][128] fp32 (backward)
   static constexpr uint32_t bars = ubar + (BWD ? 4 * TE * 4 : 0);     // mbarriers
   static constexpr uint32_t slot = bars + 32 * 8;                     // TMEM base address
   static constexpr uint32_t bytes = slot + 16 + 1024;                 // + alignment slack
   static constexpr int tmem_cols = 2 * D;                             // X | Y
+  static_assert(bytes <= 232448, "shared memory budget of one SM exceeded");
 };
 
 // barrier indices
 enum { B_META_FULL = 0, B_META_EMPTY = 2, B_EHAT_FULL = 4, B_SEL_FULL = 5, B_D1_FULL = 6, B_D2_FULL = 7,
-       B_D3_FULL = 8, B_SEG_FULL = 9, B_SPILL_DONE = 10, B_X_FREE = 11, B_S_READY = 12 /* .. +NCH */ };
+       B_D3_FULL = 8, B_SEG_FULL = 9, B_SPILL_DONE = 10, B_X_FREE = 11, B_P_FULL = 12, B_P_FREE = 13,
+       B_MB_FULL = 14, B_MB_FREE = 15, B_S_READY = 16 /* .. +NCH */ };
 
-__device__ __forceinline__ float tanh_mufu(float x) {
-  float y;
-  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
+constexpr uint32_t H2_ONE = 0x3C003C00u, H2_HALF = 0x38003800u, H2_NEG_ONE = 0xBC00BC00u, H2_NEG_HALF = 0xB800B800u;
+
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
@@ -104,14 +118,14 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&r)[1
 }
 
 // Shared-memory fallback of the segmented sum (tiles with more than MAX_SEG receivers): column sums
-// of the bf16 slabs over runs of equal receiver (thread = channel). Complete segments go to
-// out[recv], segments continuing from an earlier tile to head[tile], segments continuing into a
-// later tile to tail[tile].
+// of the f16 slabs over runs of equal receiver (thread = channel), each row weighted by wrow[e] when
+// given. Complete segments go to out[recv], segments continuing from an earlier tile to head[tile],
+// segments continuing into a later tile to tail[tile].
 template <int D>
-__device__ __forceinline__ void segmented_store_bf16(const unsigned char* __restrict__ S, const int* __restrict__ recv_s,
-                                                     const int32_t* __restrict__ rowptr, int64_t e0, int64_t tile,
-                                                     float* __restrict__ out, float* __restrict__ head,
-                                                     float* __restrict__ tail, int c) {
+__device__ __forceinline__ void segmented_store_tc(const unsigned char* __restrict__ S, const int* __restrict__ recv_s,
+                                                   const float* __restrict__ wrow, const int32_t* __restrict__ rowptr,
+                                                   int64_t e0, int64_t tile, float* __restrict__ out,
+                                                   float* __restrict__ head, float* __restrict__ tail, int c) {
   int cur = recv_s[0];
   float sum = 0.f;
   const uint32_t coff = (uint32_t)((c >> 6) * SLOT_BYTES + (c & 7) * 2);
@@ -129,22 +143,22 @@ __device__ __forceinline__ void segmented_store_bf16(const unsigned char* __rest
       sum = 0.f;
     }
     if (e < TE && rcv >= 0) {
-      const unsigned short v = *reinterpret_cast<const unsigned short*>(S + coff + e * 128 + ((cc ^ (e & 7)) << 4));
-      sum += __uint_as_float((uint32_t)v << 16);
+      const __half v = *reinterpret_cast<const __half*>(S + coff + e * 128 + ((cc ^ (e & 7)) << 4));
+      sum = fmaf(wrow ? wrow[e] : 1.0f, __half2float(v), sum);
     }
   }
 }
 
 template <int D, bool BWD>
-__global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t n_tiles) {
+__global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_tiles) {
   extern __shared__ unsigned char smem_raw[];
   using SM = ES<D, BWD>;
+  using Meta = TileMeta<BWD>;
   constexpr int NCH = SM::NCH;
   const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
   unsigned char* gen = smem_raw + (base - tc::smem_u32(smem_raw));
-  TileMeta* meta = reinterpret_cast<TileMeta*>(gen + SM::meta);
+  Meta* meta = reinterpret_cast<Meta*>(gen + SM::meta);
   TileSeg* seg = reinterpret_cast<TileSeg*>(gen + SM::seg);
-  float* b2_s = reinterpret_cast<float*>(gen + SM::b2);
   float* ubar_s = reinterpret_cast<float*>(gen + SM::ubar);
   uint32_t* slot = reinterpret_cast<uint32_t*>(gen + SM::slot);
   auto bar = [&](int i) -> uint32_t { return base + SM::bars + 8u * (uint32_t)i; };
@@ -159,12 +173,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
     src = reinterpret_cast<const uint4*>(a.W1cimg);
     dst = reinterpret_cast<uint4*>(gen + SM::w1c);
     for (int i = tid; i < D * 16 * 2 / 16; i += N_THREADS) dst[i] = src[i];
-    if (BWD) {
-      src = reinterpret_cast<const uint4*>(a.W1cTimg);
-      dst = reinterpret_cast<uint4*>(gen + SM::w1cT);
-      for (int i = tid; i < 16 * D * 2 / 16; i += N_THREADS) dst[i] = src[i];
-    }
-    for (int i = tid; i < D; i += N_THREADS) b2_s[i] = 0.5f * a.b2[i];
+    __half* b2h = reinterpret_cast<__half*>(gen + SM::b2);
+    for (int i = tid; i < D; i += N_THREADS) b2h[i] = __float2half_rn(0.5f * a.b2[i]);
+    // staged rows start finite: a stale slot is never read, but keep the buffers defined
+    uint4* z = reinterpret_cast<uint4*>(gen + SM::ptile);
+    for (int i = tid; i < (BWD ? 2 : 1) * NSLOT * D * 2 / 16; i += N_THREADS) z[i] = make_uint4(0u, 0u, 0u, 0u);
   }
   if (tid == 0) {
     tc::mbar_init(bar(B_META_FULL), N_FEAT_WARPS); tc::mbar_init(bar(B_META_FULL + 1), N_FEAT_WARPS);
@@ -172,6 +185,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
     tc::mbar_init(bar(B_EHAT_FULL), N_FEAT_WARPS); tc::mbar_init(bar(B_SEL_FULL), 1);
     tc::mbar_init(bar(B_D1_FULL), 1); tc::mbar_init(bar(B_D2_FULL), 1); tc::mbar_init(bar(B_D3_FULL), 1);
     tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_SPILL_DONE), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
+    tc::mbar_init(bar(B_P_FULL), 1); tc::mbar_init(bar(B_P_FREE), N_EPI_WARPS);
+    tc::mbar_init(bar(B_MB_FULL), 1); tc::mbar_init(bar(B_MB_FREE), N_EPI_WARPS);
     for (int s = 0; s < NCH; ++s) tc::mbar_init(bar(B_S_READY + s), N_EPI_WARPS);
     tc::fence_mbar_init();
   }
@@ -192,7 +207,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
-      TileMeta& M = meta[b];
+      Meta& M = meta[b];
       const int64_t e0 = tile * TE;
       int rc[2], sd[2];
       float rr[2];
@@ -215,13 +230,13 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           du = -(1.5707963267948966f * inv_rc) * sn;
         }
         M.recv[e] = rc[k]; M.send[e] = sd[k]; M.w[e] = a.alpha * u;
-        M.r[e] = rr[k]; M.u[e] = u; M.du[e] = du;
+        if (BWD) { M.r[e] = rr[k]; M.u[e] = u; M.du[e] = du; }
 #pragma unroll
         for (int j = 0; j < 16; j += 2) {
           const float d0 = rr[k] - (float)j * delta, d1 = rr[k] - (float)(j + 1) * delta;
           const float g0 = j < a.n_rbf ? u * ex2_approx(ngl2 * d0 * d0) : 0.f;
           const float g1 = j + 1 < a.n_rbf ? u * ex2_approx(ngl2 * d1 * d1) : 0.f;
-          pk[k][j >> 1] = tc::pack_bf16(g0, g1);
+          pk[k][j >> 1] = tc::pack_f16(g0, g1);
         }
       }
       __syncwarp();
@@ -240,7 +255,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
       if (lane == 0) mbar_arrive(bar(B_EHAT_FULL));
     }
   } else if (warp == WARP_SEG) {
-    // ============ segment producer: receivers of the tile and the selector operand of GS ============
+    // ===== segment producer: receivers of the tile, staged P_i / mbar_i rows, selector operand of GS =====
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
@@ -272,7 +287,55 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         }
         before += __popc(fm[k]);
       }
-      // the selector buffer (and seg[b], last read two tiles ago) is free once GS of the previous tile is done
+      const int R = before;
+      const bool fast = R <= NSLOT;
+      // ---- receiver list, row slots and the P'_i rows: free once E1 of the previous tile is done ----
+      if (it > 0) tc::mbar_wait(bar(B_P_FREE), (uint32_t)((it - 1) & 1));
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        if (cls[k] >= 0) { G.rid[rloc[k]] = rc[k]; G.cls[rloc[k]] = cls[k]; }
+        G.slot[lane + 32 * k] = (unsigned char)(rloc[k] < 0 ? 0 : (rloc[k] & 15));
+      }
+      if (lane == 0) G.R = R;
+      __syncwarp();
+      if (fast) {
+        if (lane < D / 8) {  // one row = D/8 chunks of 16 bytes
+          uint4 pr[NSLOT];
+#pragma unroll
+          for (int r = 0; r < NSLOT; ++r)
+            if (r < R) pr[r] = ldg_nc_v4(a.Ph + (size_t)G.rid[r] * D + lane * 8);
+#pragma unroll
+          for (int r = 0; r < NSLOT; ++r)
+            if (r < R) *reinterpret_cast<uint4*>(gen + SM::ptile + r * D * 2 + lane * 16) = pr[r];
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_P_FULL));
+      if (BWD) {
+        // ---- mbar_i rows (fp32 in global -> f16): free once E2 of the previous tile is done ----
+        if (it > 0) tc::mbar_wait(bar(B_MB_FREE), (uint32_t)((it - 1) & 1));
+        if (fast) {
+#pragma unroll 2
+          for (int r = 0; r < R; ++r) {
+            const float* src = a.mbar + (size_t)G.rid[r] * D;
+#pragma unroll
+            for (int hf = 0; hf < D / 128; ++hf) {
+              const float4 v = __ldg(reinterpret_cast<const float4*>(src + hf * 128 + lane * 4));
+              *reinterpret_cast<uint2*>(gen + SM::mtile + r * D * 2 + (hf * 128 + lane * 4) * 2) =
+                  make_uint2(tc::pack_f16(v.x, v.y), tc::pack_f16(v.z, v.w));
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_MB_FULL));
+      }
+      // ---- selector: the buffer is free once GS of the previous tile is done ----
+      float wsel[4];
+      if (!BWD) {
+        tc::mbar_wait(bar(B_META_FULL + b), (uint32_t)((it >> 1) & 1));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) wsel[k] = meta[b].w[lane + 32 * k];
+      }
       if (it > 0) tc::mbar_wait(bar(B_SEG_FULL), (uint32_t)((it - 1) & 1));
       {
         uint4* z = reinterpret_cast<uint4*>(gen + SM::sel);
@@ -280,17 +343,15 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         for (int i = 0; i < MAX_SEG * TE * 2 / 16 / 32; ++i) z[lane + 32 * i] = make_uint4(0u, 0u, 0u, 0u);
       }
       __syncwarp();
-      // Sel[r][e] = 1 if edge e belongs to the r-th receiver of the tile; K-major (K = edge), no swizzle:
-      // (r, e) -> (r/8)*2048 + (e/8)*128 + (r%8)*16 + (e%8)*2
+      // Sel[r][e] = weight of edge e if it belongs to the r-th receiver of the tile; K-major (K = edge), no
+      // swizzle: (r, e) -> (r/8)*2048 + (e/8)*128 + (r%8)*16 + (e%8)*2
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int e = lane + 32 * k;
-        if (cls[k] >= 0) { G.rid[rloc[k]] = rc[k]; G.cls[rloc[k]] = cls[k]; }
         if (rc[k] >= 0 && rloc[k] < MAX_SEG)
-          *reinterpret_cast<unsigned short*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 +
-                                             (e & 7) * 2) = (unsigned short)0x3F80;  // bf16 1.0
+          *reinterpret_cast<__half*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 + (e & 7) * 2) =
+              __float2half_rn(BWD ? 1.0f : wsel[k]);
       }
-      if (lane == 0) G.R = before;
       tc::fence_proxy_async();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_SEL_FULL));
@@ -298,10 +359,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
   } else if (warp == WARP_MMA) {
     // =========================== MMA issuer (one thread) ===========================
     if (lane == 0) {
-      constexpr uint32_t IDESC_ND = tc::idesc_bf16(128, D, 0, 0);     // K-major A and B, N = D
-      constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);  // B read MN-major
-      constexpr uint32_t IDESC_N16 = tc::idesc_bf16(128, 16, 0, 0);
-      constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);   // A read MN-major (M = channel, K = edge)
+      constexpr uint32_t IDESC_ND = tc::idesc_f16(128, D, 0, 0);     // K-major A and B, N = D
+      constexpr uint32_t IDESC_ND_BT = tc::idesc_f16(128, D, 0, 1);  // B read MN-major
+      constexpr uint32_t IDESC_N16_BT = tc::idesc_f16(128, 16, 0, 1);
+      constexpr uint32_t IDESC_SEG = tc::idesc_f16(128, 16, 1, 0);   // A read MN-major (M = channel, K = edge)
       uint32_t srp = 0;  // bit s: parity of the next completion of S_READY[s]
       auto wait_slab = [&](int s) {
         tc::mbar_wait(bar(B_S_READY + s), (srp >> s) & 1u);
@@ -352,11 +413,13 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         for (int s = 0; s < NCH; ++s) {
           wait_slab(s);
           if (BWD) {
-            tc::bulk_s2g(a.abar_bf + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
+            tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
+            // G4: ebar/2 = abar . (W1c/2). B = the G1 image [channel][16] read MN-major (N = rbf index, K = channel),
+            // no swizzle: N-direction core-matrix stride (SBO) 128 B, K-direction 8-channel group stride (LBO) 256 B
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk)  // G4: ebar = abar . W1c
+            for (int kk = 0; kk < 4; ++kk)
               tc::mma_bf16(TY + 32, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
-                           tc::smem_desc(base + SM::w1cT + s * 2048 + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC_N16,
+                           tc::smem_desc(base + SM::w1c + (4 * s + kk) * 512, 256, 128, tc::LAYOUT_NONE), IDESC_N16_BT,
                            (s | kk) != 0);
           }
           if ((s & 1) && seg_mma) {  // GS over the 128 channels of slabs s-1, s
@@ -386,8 +449,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
     const uint32_t so0 = (uint32_t)(row * 128 + (((2 * g) ^ (row & 7)) << 4));
     const uint32_t so1 = (uint32_t)(row * 128 + (((2 * g + 1) ^ (row & 7)) << 4));
     unsigned char* ring = gen + SM::ring;
+    const unsigned char* b2h = gen + SM::b2 + 32 * g;  // this thread's 16 channels of b2/2 inside a 64-channel block
     float* out = BWD ? a.Pbar : a.m;
-    uint32_t ds2[BWD ? NCH * 8 : 1];  // 2 SiLU'(a) of this thread's channels, packed bf16x2
+    uint32_t ds2[BWD ? NCH * 8 : 1];  // 2 SiLU'(2a') of this thread's channels, f16x2
 
     auto publish = [&](int s) {  // slab s written by this warp: visible to the async proxy, then signal
       tc::fence_proxy_async();
@@ -395,31 +459,36 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_S_READY + s));
     };
-    auto store_slab = [&](int s, const float (&v)[16]) {
-      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so0) =
-          make_uint4(tc::pack_bf16(v[0], v[1]), tc::pack_bf16(v[2], v[3]), tc::pack_bf16(v[4], v[5]), tc::pack_bf16(v[6], v[7]));
-      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so1) =
-          make_uint4(tc::pack_bf16(v[8], v[9]), tc::pack_bf16(v[10], v[11]), tc::pack_bf16(v[12], v[13]), tc::pack_bf16(v[14], v[15]));
+    auto store_slab = [&](int s, const uint32_t (&v)[8]) {
+      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so0) = make_uint4(v[0], v[1], v[2], v[3]);
+      *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so1) = make_uint4(v[4], v[5], v[6], v[7]);
     };
 
     // row metadata and the first Q chunk of a tile are fetched while the previous tile drains
     tc::mbar_wait(bar(B_META_FULL), 0u);
     int rc = meta[0].recv[row];
     float w = meta[0].w[row];
-    const __nv_bfloat16* Qrow = a.Qbf + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
+    const __half* Qrow = a.Qh + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
     uint4 qn0 = ldg_nc_v4(Qrow), qn1 = ldg_nc_v4(Qrow + 8);
 
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
       const uint32_t par = (uint32_t)(it & 1);
-      const TileMeta& M = meta[b];
+      const Meta& M = meta[b];
       const TileSeg& G = seg[b];
       const int64_t e0 = tile * TE;
       const bool has_next = tile + gridDim.x < n_tiles;
       const bool valid = rc >= 0;
-      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
       if (BWD && it > 0) tc::mbar_wait(bar(B_SPILL_DONE), (uint32_t)((it - 1) & 1));  // slabs of the previous tile spilled
+
+      // receiver rows of the tile: staged in shared memory (R <= NSLOT) or read from global memory
+      tc::mbar_wait(bar(B_P_FULL), par);
+      const int R = G.R;
+      const bool fast = R <= NSLOT;
+      const int myslot = G.slot[row];
+      const unsigned char* prow = fast ? gen + SM::ptile + myslot * (D * 2) + 32 * g
+                                       : reinterpret_cast<const unsigned char*>(a.Ph + (size_t)(valid ? rc : 0) * D + 16 * g);
 
       // ---- E1: a' = X + P'_i + Q'_j ; s = a' + a' tanh(a') ----
       tc::mbar_wait(bar(B_D1_FULL), par);
@@ -433,91 +502,107 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           qn0 = ldg_nc_v4(Qrow + 64 * (s + 1));
           qn1 = ldg_nc_v4(Qrow + 64 * (s + 1) + 8);
         }
-        float pv[16];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const float4 p = __ldg(reinterpret_cast<const float4*>(Prow + 64 * s + 4 * j));
-          pv[4 * j] = p.x; pv[4 * j + 1] = p.y; pv[4 * j + 2] = p.z; pv[4 * j + 3] = p.w;
+        uint4 p0, p1;
+        if (fast) {
+          p0 = *reinterpret_cast<const uint4*>(prow + 128 * s);
+          p1 = *reinterpret_cast<const uint4*>(prow + 128 * s + 16);
+        } else {
+          p0 = ldg_nc_v4(prow + 128 * s);
+          p1 = ldg_nc_v4(prow + 128 * s + 16);
         }
         const uint32_t qw[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
-        tc::tmem_wait_ld();
-        float v[16];
+        const uint32_t pw[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
+        uint32_t pq[8];
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const float qf = (j & 1) ? tc::bf16_hi(qw[j >> 1]) : tc::bf16_lo(qw[j >> 1]);
-          const float x = __uint_as_float(acc[j]) + pv[j] + qf;
-          const float t = tanh_mufu(x);
-          v[j] = fmaf(x, t, x);
-          if (BWD) pv[j] = fmaf(v[j], 1.0f - t, 1.0f + t);  // 2 SiLU'(2x) = (1 + t) + s (1 - t)
+        for (int j = 0; j < 8; ++j) pq[j] = tc::h2_add(pw[j], qw[j]);
+        tc::tmem_wait_ld();
+        uint32_t v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const uint32_t x = tc::h2_add(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), pq[j]);
+          const uint32_t t = tc::h2_tanh(x);
+          v[j] = tc::h2_fma(x, t, x);
+          if (BWD)  // 2 SiLU'(2x) = (1 + t) + s (1 - t)
+            ds2[s * 8 + j] = tc::h2_fma(v[j], tc::h2_fma(t, H2_NEG_ONE, H2_ONE), tc::h2_add(t, H2_ONE));
         }
         store_slab(s, v);
-        if (BWD) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) ds2[s * 8 + j] = tc::pack_bf16(pv[2 * j], pv[2 * j + 1]);
-        }
         publish(s);
       }
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
+      if (lane == 0) mbar_arrive(bar(B_P_FREE));           // staged P rows may be replaced
 
       // ---- E2 ----
-      tc::mbar_wait(bar(B_D2_FULL), par);
-      tc::fence_after_sync();
       if (!BWD) {
-        // forward: alpha u_e SiLU(p) -> slabs
+        // forward: phi = SiLU(p) -> slabs (weighted by alpha u_e inside the selector of GS)
+        tc::mbar_wait(bar(B_D2_FULL), par);
+        tc::fence_after_sync();
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           uint32_t acc[16];
           tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
-          float bv[16];
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const float4 p = *reinterpret_cast<const float4*>(b2_s + 64 * s + 16 * g + 4 * j);
-            bv[4 * j] = p.x; bv[4 * j + 1] = p.y; bv[4 * j + 2] = p.z; bv[4 * j + 3] = p.w;
-          }
+          const uint4 c0 = *reinterpret_cast<const uint4*>(b2h + 128 * s);
+          const uint4 c1 = *reinterpret_cast<const uint4*>(b2h + 128 * s + 16);
+          const uint32_t bw[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
           tc::tmem_wait_ld();
-          float v[16];
+          uint32_t v[8];
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const float x = __uint_as_float(acc[j]) + bv[j];
-            const float t = tanh_mufu(x);
-            v[j] = w * fmaf(x, t, x);
+          for (int j = 0; j < 8; ++j) {
+            const uint32_t x = tc::h2_add(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), bw[j]);
+            v[j] = tc::h2_fma(x, tc::h2_tanh(x), x);
           }
           store_slab(s, v);
           publish(s);
         }
       } else {
         // backward: pbar = alpha u mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
-        const float* mrow = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        tc::mbar_wait(bar(B_MB_FULL), par);
+        const unsigned char* mrow = gen + SM::mtile + myslot * (D * 2) + 32 * g;
+        const float* mrow_g = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        const uint32_t w2 = tc::pack_f16(w, w);
         float ub = 0.f;
+        tc::mbar_wait(bar(B_D2_FULL), par);
+        tc::fence_after_sync();
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           uint32_t acc[16];
           tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
-          float bv[16], mb[16];
+          const uint4 c0 = *reinterpret_cast<const uint4*>(b2h + 128 * s);
+          const uint4 c1 = *reinterpret_cast<const uint4*>(b2h + 128 * s + 16);
+          const uint32_t bw[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+          uint32_t mb[8];
+          if (fast) {
+            const uint4 m0 = *reinterpret_cast<const uint4*>(mrow + 128 * s);
+            const uint4 m1 = *reinterpret_cast<const uint4*>(mrow + 128 * s + 16);
+            mb[0] = m0.x; mb[1] = m0.y; mb[2] = m0.z; mb[3] = m0.w; mb[4] = m1.x; mb[5] = m1.y; mb[6] = m1.z; mb[7] = m1.w;
+          } else {
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const float4 p = *reinterpret_cast<const float4*>(b2_s + 64 * s + 16 * g + 4 * j);
-            bv[4 * j] = p.x; bv[4 * j + 1] = p.y; bv[4 * j + 2] = p.z; bv[4 * j + 3] = p.w;
-            const float4 m4 = __ldg(reinterpret_cast<const float4*>(mrow + 64 * s + 4 * j));
-            mb[4 * j] = m4.x; mb[4 * j + 1] = m4.y; mb[4 * j + 2] = m4.z; mb[4 * j + 3] = m4.w;
+            for (int j = 0; j < 4; ++j) {
+              const float4 m4 = __ldg(reinterpret_cast<const float4*>(mrow_g + 64 * s + 4 * j));
+              mb[2 * j] = tc::pack_f16(m4.x, m4.y);
+              mb[2 * j + 1] = tc::pack_f16(m4.z, m4.w);
+            }
           }
           tc::tmem_wait_ld();
-          float v[16];
+          uint32_t v[8];
+          uint32_t ubp = 0u;
 #pragma unroll
-          for (int j = 0; j < 16; ++j) {
-            const float x = __uint_as_float(acc[j]) + bv[j];
-            const float t = tanh_mufu(x);
-            const float phi = fmaf(x, t, x);
-            const float dphi = fmaf(phi, fmaf(-0.5f, t, 0.5f), fmaf(0.5f, t, 0.5f));  // sigma + phi (1 - sigma)
-            ub = fmaf(mb[j], phi, ub);
-            v[j] = (w * mb[j]) * dphi;
+          for (int j = 0; j < 8; ++j) {
+            const uint32_t x = tc::h2_add(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), bw[j]);
+            const uint32_t t = tc::h2_tanh(x);
+            const uint32_t phi = tc::h2_fma(x, t, x);
+            // SiLU'(p) = sigma + phi (1 - sigma), sigma = (1 + t)/2
+            const uint32_t dphi = tc::h2_fma(phi, tc::h2_fma(t, H2_NEG_HALF, H2_HALF), tc::h2_fma(t, H2_HALF, H2_HALF));
+            ubp = tc::h2_fma(mb[j], phi, ubp);
+            v[j] = tc::h2_mul(tc::h2_mul(mb[j], w2), dphi);
           }
+          ub += tc::h2_lo(ubp) + tc::h2_hi(ubp);
           store_slab(s, v);
           publish(s);
         }
+        if (lane == 0) mbar_arrive(bar(B_MB_FREE));
         ubar_s[g * TE + row] = ub;
 
-        // ---- E3: abar = X * 2 SiLU'(a) -> slabs ----
+        // ---- E3: abar = X * 2 SiLU'(2a') -> slabs ----
         tc::mbar_wait(bar(B_D3_FULL), par);
         tc::fence_after_sync();
 #pragma unroll
@@ -525,12 +610,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           uint32_t acc[16];
           tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
           tc::tmem_wait_ld();
-          float v[16];
+          uint32_t v[8];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            v[2 * j] = __uint_as_float(acc[2 * j]) * tc::bf16_lo(ds2[s * 8 + j]);
-            v[2 * j + 1] = __uint_as_float(acc[2 * j + 1]) * tc::bf16_hi(ds2[s * 8 + j]);
-          }
+          for (int j = 0; j < 8; ++j)
+            v[j] = tc::h2_mul(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), ds2[s * 8 + j]);
           store_slab(s, v);
           publish(s);
         }
@@ -544,7 +627,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         tc::mbar_wait(bar(B_META_FULL + (b ^ 1)), (uint32_t)(((it + 1) >> 1) & 1));
         rc_n = meta[b ^ 1].recv[row];
         w_n = meta[b ^ 1].w[row];
-        Qrow = a.Qbf + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
+        Qrow = a.Qh + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
         qn0 = ldg_nc_v4(Qrow);
         qn1 = ldg_nc_v4(Qrow + 8);
       }
@@ -552,7 +635,6 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
       // ---- segment sums (and E4) out of Y ----
       tc::mbar_wait(bar(B_SEG_FULL), par);
       tc::fence_after_sync();
-      const int R = G.R;
       if (R <= MAX_SEG) {
         if (g >= 1 && g <= NCH / 2) {
           const int h = g - 1;
@@ -571,11 +653,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
         }
       } else {
         named_bar_sync(1, N_EPI_WARPS * 32);
-        if (tid < D) segmented_store_bf16<D>(ring, M.recv, a.rowptr, e0, tile, out, a.head, a.tail, tid);
+        if (tid < D) segmented_store_tc<D>(ring, M.recv, BWD ? nullptr : M.w, a.rowptr, e0, tile, out, a.head, a.tail, tid);
         named_bar_sync(1, N_EPI_WARPS * 32);
       }
       if (BWD && g == 0) {
-        // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k) ----
+        // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k); G4 used the halved W1c image ----
         uint32_t eb[16];
         tmem_ld16_nowait(TY + tlane + 32u, eb);
         tc::tmem_wait_ld();
@@ -590,7 +672,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
           }
         }
         const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
-        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, part);
+        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, 2.0f * part);
       }
       tc::fence_before_sync();
       __syncwarp();
@@ -606,9 +688,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_bf16(EdgeArgs a, int64_t 
 }
 
 // out[i] = tail[t] + head[t+1] + ... for the segment that starts in tile t and continues beyond it
-__global__ void k_segment_fixup_bf16(int64_t E, int D, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ recv,
-                                     const float* __restrict__ head, const float* __restrict__ tail,
-                                     float* __restrict__ out) {
+__global__ void k_segment_fixup_tc(int64_t E, int D, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ recv,
+                                   const float* __restrict__ head, const float* __restrict__ tail, float* __restrict__ out) {
   const int64_t t = blockIdx.x;
   const int64_t e0 = t * TE, e1 = e0 + TE;
   if (e1 >= E) return;
@@ -622,11 +703,11 @@ __global__ void k_segment_fixup_bf16(int64_t E, int D, const int32_t* __restrict
   }
 }
 
-// Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled tile images written by E3
+// Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled f16 tile images written by E3
 template <int D>
-__global__ void __launch_bounds__(256) k_gather_rev_bf16(int64_t n, const int32_t* __restrict__ rowptr,
-                                                         const int32_t* __restrict__ rev,
-                                                         const __nv_bfloat16* __restrict__ abar, float* __restrict__ Qbar) {
+__global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, const int32_t* __restrict__ rowptr,
+                                                       const int32_t* __restrict__ rev, const __half* __restrict__ abar,
+                                                       float* __restrict__ Qbar) {
   constexpr int CH = D / 8;        // 16-byte chunks per row
   constexpr int NSUB = 32 / CH;    // edges handled concurrently by one warp
   const int lane = threadIdx.x & 31;
@@ -640,8 +721,12 @@ __global__ void __launch_bounds__(256) k_gather_rev_bf16(int64_t n, const int32_
     const int re = rev[e];
     const int t = re >> 7, rw = re & 127;
     const uint4 v = *reinterpret_cast<const uint4*>(base + (size_t)t * TE * D * 2 + tc::sw128_chunk_off(TE, rw, ch));
-    acc[0] += tc::bf16_lo(v.x); acc[1] += tc::bf16_hi(v.x); acc[2] += tc::bf16_lo(v.y); acc[3] += tc::bf16_hi(v.y);
-    acc[4] += tc::bf16_lo(v.z); acc[5] += tc::bf16_hi(v.z); acc[6] += tc::bf16_lo(v.w); acc[7] += tc::bf16_hi(v.w);
+    const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
+    const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+    const float2 f2 = __half22float2(*reinterpret_cast<const __half2*>(&v.z));
+    const float2 f3 = __half22float2(*reinterpret_cast<const __half2*>(&v.w));
+    acc[0] += f0.x; acc[1] += f0.y; acc[2] += f1.x; acc[3] += f1.y;
+    acc[4] += f2.x; acc[5] += f2.y; acc[6] += f3.x; acc[7] += f3.y;
   }
   if (NSUB > 1) {
 #pragma unroll
@@ -660,37 +745,37 @@ int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   if (tiles == 0) return MLIP_OK;
   const size_t smem = ES<D, BWD>::bytes;
   const unsigned grid = (unsigned)(tiles < ctx->num_sms ? tiles : ctx->num_sms);
-  MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_bf16<D, BWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_edge_bf16<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
-  k_segment_fixup_bf16<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
-                                                                               BWD ? a.Pbar : a.m);
+  MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_tc<D, BWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  k_edge_tc<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
+  k_segment_fixup_tc<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
+                                                                             BWD ? a.Pbar : a.m);
   ctx->launches += 2;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
 }
 }  // namespace
 
-int64_t mlip_edge_bf16_tiles(int64_t E) { return (E + TE - 1) / TE; }
+int64_t mlip_edge_tc_tiles(int64_t E) { return (E + TE - 1) / TE; }
 
-int mlip_edge_forward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a) {
+int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   if (d == 256) return launch_edge_dir<256, false>(ctx, a);
   if (d == 128) return launch_edge_dir<128, false>(ctx, a);
-  ctx->set_error("bf16 edge kernels need d = 128 or 256");
+  ctx->set_error("tensor-core edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_edge_backward_bf16(mlip_ctx* ctx, int d, const EdgeArgs& a) {
+int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   if (d == 256) return launch_edge_dir<256, true>(ctx, a);
   if (d == 128) return launch_edge_dir<128, true>(ctx, a);
-  ctx->set_error("bf16 edge kernels need d = 128 or 256");
+  ctx->set_error("tensor-core edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_gather_rev_bf16(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
-                         const __nv_bfloat16* abar, float* Qbar) {
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev, const __half* abar,
+                       float* Qbar) {
   if (n <= 0) return MLIP_OK;
   const unsigned grid = (unsigned)((n * 32 + 255) / 256);
-  if (d == 256) k_gather_rev_bf16<256><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
-  else if (d == 128) k_gather_rev_bf16<128><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
-  else { ctx->set_error("bf16 gather needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
+  if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
+  else if (d == 128) k_gather_rev_tc<128><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
+  else { ctx->set_error("tensor-core gather needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
   ctx->launches++;
   return MLIP_OK;
 }

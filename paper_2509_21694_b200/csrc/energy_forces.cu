@@ -124,7 +124,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   cudaStream_t st = ctx->stream;
   auto gemm_raw = bf ? mlip_gemm_bf16 : mlip_gemm_f32;
   auto gemm = [&](mlip_ctx* c, const GemmArgs& ga) { ProfScope p(c, MLIP_PROF_NODE_GEMM); return gemm_raw(c, ga); };
-  const int64_t tiles = bf ? mlip_edge_bf16_tiles(E) : mlip_edge_f32_tiles(E);
+  const int64_t tiles = bf ? mlip_edge_tc_tiles(E) : mlip_edge_f32_tiles(E);
 
   std::vector<void*> ws;
   auto release = [&]() { for (void* p : ws) ctx->free(p); };
@@ -138,21 +138,21 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
 
   std::vector<float*> h(L + 1), P(L), c(L);
   std::vector<float*> Qf(L, nullptr);
-  std::vector<__nv_bfloat16*> Qb(L, nullptr);
+  std::vector<__half*> Ph(L, nullptr), Qh(L, nullptr);
   for (int l = 0; l <= L; ++l) W_ALLOC(h[l], float, n * d);
   for (int l = 0; l < L; ++l) {
-    if (bf) { W_ALLOC(P[l], float, n * d); W_ALLOC(Qb[l], __nv_bfloat16, n * d); }
+    if (bf) { W_ALLOC(Ph[l], __half, n * d); W_ALLOC(Qh[l], __half, n * d); }
     else { W_ALLOC(P[l], float, n * 2 * d); Qf[l] = P[l] + d; }
     W_ALLOC(c[l], float, n * d);
   }
   float *m = nullptr, *o = nullptr, *hbar = nullptr, *cbar = nullptr, *PQbar = nullptr, *head = nullptr, *tail = nullptr,
         *rbar = nullptr, *E_i = nullptr, *abar = nullptr;
-  __nv_bfloat16* abar_bf = nullptr;
+  __half* abar_h = nullptr;
   double* partial = nullptr;
   W_ALLOC(m, float, n * d); W_ALLOC(o, float, n * d); W_ALLOC(hbar, float, n * d); W_ALLOC(cbar, float, n * d);
   W_ALLOC(PQbar, float, n * 2 * d); W_ALLOC(head, float, (tiles + 1) * d); W_ALLOC(tail, float, (tiles + 1) * d);
   W_ALLOC(rbar, float, E + 1); W_ALLOC(E_i, float, n);
-  if (L > 0) { if (bf) W_ALLOC(abar_bf, __nv_bfloat16, tiles * 128 * d); else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
+  if (L > 0) { if (bf) W_ALLOC(abar_h, __half, tiles * 128 * d); else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
   const int64_t n_part = (n + 255) / 256;
   W_ALLOC(partial, double, n_part);
   float* mbar = m;           // m is dead after the forward pass
@@ -171,18 +171,18 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
 
   auto set_layer = [&](int l) {
     const LayerWeights& W = M->layers[l];
-    ea.P = P[l]; ea.ldp = bf ? d : 2 * d; ea.Q = Qf[l]; ea.ldq = 2 * d; ea.Qbf = Qb[l];
+    ea.P = P[l]; ea.ldp = 2 * d; ea.Q = Qf[l]; ea.ldq = 2 * d; ea.Ph = Ph[l]; ea.Qh = Qh[l];
     ea.W1c = W.W1c; ea.W2T = W.W2T; ea.W2 = W.W2; ea.b2 = W.b2;
-    ea.W2img = W.W2img; ea.W1cimg = W.W1cimg; ea.W1cTimg = W.W1cTimg;
+    ea.W2img = W.W2img; ea.W1cimg = W.W1cimg;
   };
 
   for (int l = 0; l < L; ++l) {
     const LayerWeights& W = M->layers[l];
     GemmArgs a;
     if (bf) {
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Y = P[l]; a.ldy = d; a.n = n; a.N = d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = n; a.N = d;
       W_TRY(gemm(ctx, a));
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Ybf = Qb[l]; a.ldy = d; a.n = n; a.N = d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = n; a.N = d;
       W_TRY(gemm(ctx, a));
     } else {
       a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1ab; a.bias = W.b1pad; a.Y = P[l]; a.ldy = 2 * d; a.n = n; a.N = 2 * d;
@@ -193,7 +193,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     ea.m = m;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
-      W_TRY(bf ? mlip_edge_forward_bf16(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
+      W_TRY(bf ? mlip_edge_forward_tc(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
     }
     a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.X2 = m; a.ld2 = d; a.K2 = d;
     a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = n; a.N = d;
@@ -238,14 +238,14 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     W_TRY(gemm(ctx, a));
     cudaMemsetAsync(Pbar, 0, sizeof(float) * n * d, st);
     set_layer(l);
-    ea.mbar = mbar; ea.abar = abar; ea.abar_bf = abar_bf; ea.Pbar = Pbar; ea.rbar = rbar;
+    ea.mbar = mbar; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
-      W_TRY(bf ? mlip_edge_backward_bf16(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
+      W_TRY(bf ? mlip_edge_backward_tc(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
     }
     {
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
-      W_TRY(bf ? mlip_gather_rev_bf16(ctx, n, d, g.rowptr, g.rev, abar_bf, Qbar)
+      W_TRY(bf ? mlip_gather_rev_tc(ctx, n, d, g.rowptr, g.rev, abar_h, Qbar)
                : mlip_gather_rev_f32(ctx, n, d, g.rowptr, g.rev, abar, Qbar));
     }
     a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.X2 = Qbar; a.ld2 = d; a.K2 = d;

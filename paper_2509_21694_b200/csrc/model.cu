@@ -183,16 +183,15 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     M_ALLOC(W.V1_bf, __nv_bfloat16, 2 * d * d); M_ALLOC(W.V2_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V2T_bf, __nv_bfloat16, d * d); M_ALLOC(W.V1aT_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V1bT_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1abT_bf, __nv_bfloat16, 2 * d * d);
-    // the bf16 edge kernels consume HALVED pre-projections P' = (W1a h + b1)/2, Q' = (W1b h)/2 (exact scaling)
+    // the tensor-core edge kernels consume HALVED pre-projections P' = (W1a h + b1)/2, Q' = (W1b h)/2 (exact scaling)
     tobf(W.W1ab, W.W1a_bf, d * d, 0.5f); tobf(W.W1ab + (size_t)d * d, W.W1b_bf, d * d, 0.5f);
     M_ALLOC(W.b1h, float, d);
     k_scale<<<(d + 255) / 256, 256, 0, st>>>(W.b1, W.b1h, d, 0.5f);
     tobf(W.V1, W.V1_bf, 2 * d * d); tobf(W.V2, W.V2_bf, d * d); tobf(W.V2T, W.V2T_bf, d * d);
     tobf(W.V1aT, W.V1aT_bf, d * d); tobf(W.V1bT, W.V1bT_bf, d * d); tobf(W.W1abT, W.W1abT_bf, 2 * d * d);
     // operand images of the fused edge kernels (tc_images.cuh documents the layouts)
-    M_ALLOC(W.W2img, __nv_bfloat16, d * d); M_ALLOC(W.W1cimg, __nv_bfloat16, d * 16);
-    M_ALLOC(W.W1cTimg, __nv_bfloat16, 16 * d);
-    mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg, W.W1cTimg);
+    M_ALLOC(W.W2img, __half, d * d); M_ALLOC(W.W1cimg, __half, d * 16);
+    mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg);
   }
   M->Wo = p; p += (size_t)d * d;
   M->bo = p; p += d;

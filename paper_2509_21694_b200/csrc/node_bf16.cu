@@ -134,6 +134,15 @@ __global__ void __launch_bounds__(256) k_gemm_bf16(GemmArgs a) {
         for (int j = 0; j < 32; j += 4)
           *reinterpret_cast<float4*>(a.Y + r * a.ldy + c0 + j) = make_float4(y[j], y[j + 1], y[j + 2], y[j + 3]);
       }
+      if (a.Yh) {
+#pragma unroll
+        for (int j = 0; j < 32; j += 8) {
+          uint4 pk;
+          pk.x = tc::pack_f16(y[j], y[j + 1]); pk.y = tc::pack_f16(y[j + 2], y[j + 3]);
+          pk.z = tc::pack_f16(y[j + 4], y[j + 5]); pk.w = tc::pack_f16(y[j + 6], y[j + 7]);
+          *reinterpret_cast<uint4*>(a.Yh + r * a.ldy + c0 + j) = pk;
+        }
+      }
       if (a.Ybf) {
 #pragma unroll
         for (int j = 0; j < 32; j += 8) {
