@@ -23,7 +23,8 @@ struct EdgeArgs {
   int n_rbf = 0;
   float* m = nullptr;                              // forward out [n,d]
   float *head = nullptr, *tail = nullptr;          // per-tile partial rows [tiles,d]
-  const float* mbar = nullptr;                     // backward in [n,d]
+  const float* mbar = nullptr;                     // backward in [n,d] (fp32 path)
+  const __half* mbar_h = nullptr;                  // backward in [n,d] (tensor-core path, f16)
   float* abar = nullptr;                           // backward spill [E,d] fp32
   __half* abar_h = nullptr;                        // backward spill, f16 tile images [tiles,128,d]
   float* Pbar = nullptr;                           // backward out [n,d]

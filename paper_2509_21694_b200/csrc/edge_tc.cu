@@ -58,8 +58,9 @@ struct TileMeta {       // written by the feature producers, double buffered
   float r[BWD ? TE : 1], u[BWD ? TE : 1], du[BWD ? TE : 1];
 };
 struct TileSeg {        // written by the segment producer, double buffered
+  float* dst[MAX_SEG];  // where the sum of receiver slot r goes: out[rid] if its segment is complete inside the tile,
+                        // head[tile] if it continues from an earlier tile, tail[tile] if it continues into a later one
   int rid[MAX_SEG];     // receivers of the tile in order of appearance
-  int cls[MAX_SEG];     // 0: segment complete inside the tile, 1: continues from an earlier tile, 2: into a later one
   int R;                // number of distinct receivers in the tile
   int pad[3];
   unsigned char slot[TE];  // receiver slot of every edge row (valid when R <= NSLOT)
@@ -89,7 +90,7 @@ struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
 // barrier indices
 enum { B_META_FULL = 0, B_META_EMPTY = 2, B_EHAT_FULL = 4, B_SEL_FULL = 5, B_D1_FULL = 6, B_D2_FULL = 7,
        B_D3_FULL = 8, B_SEG_FULL = 9, B_SPILL_DONE = 10, B_X_FREE = 11, B_P_FULL = 12, B_P_FREE = 13,
-       B_MB_FULL = 14, B_MB_FREE = 15, B_S_READY = 16 /* .. +NCH */ };
+       B_MB_FULL = 14, B_MB_FREE = 15, B_D2B_FULL = 16, B_D3B_FULL = 17, B_S_READY = 18 /* .. +NCH */ };
 
 constexpr uint32_t H2_ONE = 0x3C003C00u, H2_HALF = 0x38003800u, H2_NEG_ONE = 0xBC00BC00u, H2_NEG_HALF = 0xB800B800u;
 
@@ -115,6 +116,21 @@ __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&r)[1
         "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
       : "r"(taddr)
       : "memory");
+}
+
+template <int N>
+__device__ __forceinline__ void tmem_ld_nowait(uint32_t taddr, uint32_t (&r)[N]) {
+  static_assert(N == 4 || N == 8, "4 or 8 columns");
+  if constexpr (N == 8)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+  else
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(taddr)
+                 : "memory");
 }
 
 // Shared-memory fallback of the segmented sum (tiles with more than MAX_SEG receivers): column sums
@@ -187,6 +203,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_SPILL_DONE), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
     tc::mbar_init(bar(B_P_FULL), 1); tc::mbar_init(bar(B_P_FREE), N_EPI_WARPS);
     tc::mbar_init(bar(B_MB_FULL), 1); tc::mbar_init(bar(B_MB_FREE), N_EPI_WARPS);
+    tc::mbar_init(bar(B_D2B_FULL), 1); tc::mbar_init(bar(B_D3B_FULL), 1);
     for (int s = 0; s < NCH; ++s) tc::mbar_init(bar(B_S_READY + s), N_EPI_WARPS);
     tc::fence_mbar_init();
   }
@@ -293,7 +310,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       if (it > 0) tc::mbar_wait(bar(B_P_FREE), (uint32_t)((it - 1) & 1));
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        if (cls[k] >= 0) { G.rid[rloc[k]] = rc[k]; G.cls[rloc[k]] = cls[k]; }
+        if (cls[k] >= 0) {
+          G.rid[rloc[k]] = rc[k];
+          G.dst[rloc[k]] = cls[k] == 0 ? (BWD ? a.Pbar : a.m) + (size_t)rc[k] * D
+                                       : (cls[k] == 1 ? a.head : a.tail) + (size_t)tile * D;
+        }
         G.slot[lane + 32 * k] = (unsigned char)(rloc[k] < 0 ? 0 : (rloc[k] & 15));
       }
       if (lane == 0) G.R = R;
@@ -312,19 +333,18 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_P_FULL));
       if (BWD) {
-        // ---- mbar_i rows (fp32 in global -> f16): free once E2 of the previous tile is done ----
-        if (it > 0) tc::mbar_wait(bar(B_MB_FREE), (uint32_t)((it - 1) & 1));
-        if (fast) {
-#pragma unroll 2
-          for (int r = 0; r < R; ++r) {
-            const float* src = a.mbar + (size_t)G.rid[r] * D;
+        // ---- mbar_i rows: the buffer is free once E2 of the previous tile is done; the loads do not wait for it ----
+        uint4 mr[NSLOT];
+        if (fast && lane < D / 8) {
 #pragma unroll
-            for (int hf = 0; hf < D / 128; ++hf) {
-              const float4 v = __ldg(reinterpret_cast<const float4*>(src + hf * 128 + lane * 4));
-              *reinterpret_cast<uint2*>(gen + SM::mtile + r * D * 2 + (hf * 128 + lane * 4) * 2) =
-                  make_uint2(tc::pack_f16(v.x, v.y), tc::pack_f16(v.z, v.w));
-            }
-          }
+          for (int r = 0; r < NSLOT; ++r)
+            if (r < R) mr[r] = ldg_nc_v4(a.mbar_h + (size_t)G.rid[r] * D + lane * 8);
+        }
+        if (it > 0) tc::mbar_wait(bar(B_MB_FREE), (uint32_t)((it - 1) & 1));
+        if (fast && lane < D / 8) {
+#pragma unroll
+          for (int r = 0; r < NSLOT; ++r)
+            if (r < R) *reinterpret_cast<uint4*>(gen + SM::mtile + r * D * 2 + lane * 16) = mr[r];
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar(B_MB_FULL));
@@ -361,6 +381,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     if (lane == 0) {
       constexpr uint32_t IDESC_ND = tc::idesc_f16(128, D, 0, 0);     // K-major A and B, N = D
       constexpr uint32_t IDESC_ND_BT = tc::idesc_f16(128, D, 0, 1);  // B read MN-major
+      // the last K slab of G2 / G3 is issued as two N halves with a commit each, so that the epilogue of
+      // the first half of the columns starts while the tensor core finishes the second
+      constexpr uint32_t IDESC_NH = tc::idesc_f16(128, D / 2, 0, 0);
+      constexpr uint32_t IDESC_NH_BT = tc::idesc_f16(128, D / 2, 0, 1);
       constexpr uint32_t IDESC_N16_BT = tc::idesc_f16(128, 16, 0, 1);
       constexpr uint32_t IDESC_SEG = tc::idesc_f16(128, 16, 1, 0);   // A read MN-major (M = channel, K = edge)
       uint32_t srp = 0;  // bit s: parity of the next completion of S_READY[s]
@@ -386,26 +410,50 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           wait_slab(s);
+          if (s < NCH - 1) {
 #pragma unroll
-          for (int kk = 0; kk < 4; ++kk)
-            tc::mma_bf16(TY, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
-                         tc::smem_desc(base + SM::w2 + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC_ND,
-                         (s | kk) != 0);
+            for (int kk = 0; kk < 4; ++kk)
+              tc::mma_f16_ts(TY, TX + (uint32_t)(64 * s + 16 * kk),  // A = s, written in place over X by E1
+                             tc::smem_desc(base + SM::w2 + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC_ND,
+                             (s | kk) != 0);
+          } else {
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk)
+                tc::mma_f16_ts(TY + (uint32_t)(hf * (D / 2)), TX + (uint32_t)(64 * s + 16 * kk),
+                               tc::smem_desc(base + SM::w2 + s * (D * 128) + hf * (D / 2) * 128 + kk * 32, 16, 1024,
+                                             tc::LAYOUT_SW128),
+                               IDESC_NH, true);
+              tc::mma_commit(bar(hf == 0 ? B_D2_FULL : B_D2B_FULL));
+            }
+          }
         }
-        tc::mma_commit(bar(B_D2_FULL));
         if (!BWD && has_next) issue_g1(it + 1);  // forward: X is dead after E1, run G1 of the next tile under E2
         if (BWD) {
           // G3: X = pbar . W2 (W2 image as MN-major B: LBO = slab stride, 16 k-rows = 2 KB)
 #pragma unroll
           for (int s = 0; s < NCH; ++s) {
             wait_slab(s);
+            if (s < NCH - 1) {
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk)
-              tc::mma_bf16(TX, tc::smem_desc(base + SM::ring + s * SLOT_BYTES + kk * 32, 16, 1024, tc::LAYOUT_SW128),
-                           tc::smem_desc(base + SM::w2 + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128), IDESC_ND_BT,
-                           (s | kk) != 0);
+              for (int kk = 0; kk < 4; ++kk)
+                tc::mma_f16_ts(TX, TY + (uint32_t)(64 * s + 16 * kk),  // A = pbar, written in place over Y by E2
+                               tc::smem_desc(base + SM::w2 + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128),
+                               IDESC_ND_BT, (s | kk) != 0);
+            } else {
+#pragma unroll
+              for (int hf = 0; hf < 2; ++hf) {
+#pragma unroll
+                for (int kk = 0; kk < 4; ++kk)
+                  tc::mma_f16_ts(TX + (uint32_t)(hf * (D / 2)), TY + (uint32_t)(64 * s + 16 * kk),
+                                 tc::smem_desc(base + SM::w2 + (4 * s + kk) * 2048 + hf * (D / 128) * (D * 128), D * 128, 1024,
+                                               tc::LAYOUT_SW128),
+                                 IDESC_NH_BT, true);
+                tc::mma_commit(bar(hf == 0 ? B_D3_FULL : B_D3B_FULL));
+              }
+            }
           }
-          tc::mma_commit(bar(B_D3_FULL));
         }
         tc::mbar_wait(bar(B_SEL_FULL), (uint32_t)(it & 1));
         const bool seg_mma = *reinterpret_cast<volatile int*>(&seg[b].R) <= MAX_SEG;
@@ -459,6 +507,14 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_S_READY + s));
     };
+    // operand chunk kept in tensor memory: this thread's 16 f16 (8 columns) over the first half of the 16 fp32
+    // accumulator columns it has just read; no proxy fence, so loads in flight are not waited for
+    auto publish_tmem = [&](int s) {
+      tc::tmem_wait_st();
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_S_READY + s));
+    };
     auto store_slab = [&](int s, const uint32_t (&v)[8]) {
       *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so0) = make_uint4(v[0], v[1], v[2], v[3]);
       *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so1) = make_uint4(v[4], v[5], v[6], v[7]);
@@ -469,7 +525,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     int rc = meta[0].recv[row];
     float w = meta[0].w[row];
     const __half* Qrow = a.Qh + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
-    uint4 qn0 = ldg_nc_v4(Qrow), qn1 = ldg_nc_v4(Qrow + 8);
+    // Q'_j chunks of the row, fetched two slabs ahead of their use (rolling buffer of three)
+    uint4 qb[3][2];
+    qb[0][0] = ldg_nc_v4(Qrow); qb[0][1] = ldg_nc_v4(Qrow + 8);
+    qb[1][0] = ldg_nc_v4(Qrow + 64); qb[1][1] = ldg_nc_v4(Qrow + 72);
 
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
@@ -497,10 +556,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       for (int s = 0; s < NCH; ++s) {
         uint32_t acc[16];
         tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
-        const uint4 q0 = qn0, q1 = qn1;
-        if (s + 1 < NCH) {
-          qn0 = ldg_nc_v4(Qrow + 64 * (s + 1));
-          qn1 = ldg_nc_v4(Qrow + 64 * (s + 1) + 8);
+        const uint4 q0 = qb[s % 3][0], q1 = qb[s % 3][1];
+        if (s + 2 < NCH) {
+          qb[(s + 2) % 3][0] = ldg_nc_v4(Qrow + 64 * (s + 2));
+          qb[(s + 2) % 3][1] = ldg_nc_v4(Qrow + 64 * (s + 2) + 8);
         }
         uint4 p0, p1;
         if (fast) {
@@ -525,8 +584,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           if (BWD)  // 2 SiLU'(2x) = (1 + t) + s (1 - t)
             ds2[s * 8 + j] = tc::h2_fma(v[j], tc::h2_fma(t, H2_NEG_ONE, H2_ONE), tc::h2_add(t, H2_ONE));
         }
-        store_slab(s, v);
-        publish(s);
+        tc::tmem_st8(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
+        publish_tmem(s);
       }
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
       if (lane == 0) mbar_arrive(bar(B_P_FREE));           // staged P rows may be replaced
@@ -538,6 +597,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         tc::fence_after_sync();
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
+          if (s == NCH / 2) { tc::mbar_wait(bar(B_D2B_FULL), par); tc::fence_after_sync(); }
           uint32_t acc[16];
           tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
           const uint4 c0 = *reinterpret_cast<const uint4*>(b2h + 128 * s);
@@ -557,13 +617,14 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         // backward: pbar = alpha u mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
         tc::mbar_wait(bar(B_MB_FULL), par);
         const unsigned char* mrow = gen + SM::mtile + myslot * (D * 2) + 32 * g;
-        const float* mrow_g = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        const __half* mrow_g = a.mbar_h + (size_t)(valid ? rc : 0) * D + 16 * g;
         const uint32_t w2 = tc::pack_f16(w, w);
         float ub = 0.f;
         tc::mbar_wait(bar(B_D2_FULL), par);
         tc::fence_after_sync();
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
+          if (s == NCH / 2) { tc::mbar_wait(bar(B_D2B_FULL), par); tc::fence_after_sync(); }
           uint32_t acc[16];
           tmem_ld16_nowait(TY + tlane + (uint32_t)(64 * s + 16 * g), acc);
           const uint4 c0 = *reinterpret_cast<const uint4*>(b2h + 128 * s);
@@ -575,12 +636,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
             const uint4 m1 = *reinterpret_cast<const uint4*>(mrow + 128 * s + 16);
             mb[0] = m0.x; mb[1] = m0.y; mb[2] = m0.z; mb[3] = m0.w; mb[4] = m1.x; mb[5] = m1.y; mb[6] = m1.z; mb[7] = m1.w;
           } else {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 m4 = __ldg(reinterpret_cast<const float4*>(mrow_g + 64 * s + 4 * j));
-              mb[2 * j] = tc::pack_f16(m4.x, m4.y);
-              mb[2 * j + 1] = tc::pack_f16(m4.z, m4.w);
-            }
+            const uint4 m0 = ldg_nc_v4(mrow_g + 64 * s), m1 = ldg_nc_v4(mrow_g + 64 * s + 8);
+            mb[0] = m0.x; mb[1] = m0.y; mb[2] = m0.z; mb[3] = m0.w; mb[4] = m1.x; mb[5] = m1.y; mb[6] = m1.z; mb[7] = m1.w;
           }
           tc::tmem_wait_ld();
           uint32_t v[8];
@@ -596,8 +653,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
             v[j] = tc::h2_mul(tc::h2_mul(mb[j], w2), dphi);
           }
           ub += tc::h2_lo(ubp) + tc::h2_hi(ubp);
-          store_slab(s, v);
-          publish(s);
+          tc::tmem_st8(TY + tlane + (uint32_t)(64 * s + 16 * g), v);
+          publish_tmem(s);
         }
         if (lane == 0) mbar_arrive(bar(B_MB_FREE));
         ubar_s[g * TE + row] = ub;
@@ -607,6 +664,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         tc::fence_after_sync();
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
+          if (s == NCH / 2) { tc::mbar_wait(bar(B_D3B_FULL), par); tc::fence_after_sync(); }
           uint32_t acc[16];
           tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
           tc::tmem_wait_ld();
@@ -628,28 +686,25 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         rc_n = meta[b ^ 1].recv[row];
         w_n = meta[b ^ 1].w[row];
         Qrow = a.Qh + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
-        qn0 = ldg_nc_v4(Qrow);
-        qn1 = ldg_nc_v4(Qrow + 8);
+        qb[0][0] = ldg_nc_v4(Qrow); qb[0][1] = ldg_nc_v4(Qrow + 8);
+        qb[1][0] = ldg_nc_v4(Qrow + 64); qb[1][1] = ldg_nc_v4(Qrow + 72);
       }
 
       // ---- segment sums (and E4) out of Y ----
       tc::mbar_wait(bar(B_SEG_FULL), par);
       tc::fence_after_sync();
       if (R <= MAX_SEG) {
-        if (g >= 1 && g <= NCH / 2) {
-          const int h = g - 1;
-          uint32_t acc[16];
-          tmem_ld16_nowait(TY + tlane + (uint32_t)(16 * h), acc);
+        // Yseg: 16 columns (receiver slots) per 128 channels; warp group g reads 2 NCH of the 8 NCH columns
+        constexpr int NR = 2 * NCH;
+        const int h = (g * NR) >> 4, r0 = (g * NR) & 15;
+        if (r0 < R) {
+          uint32_t acc[NR];
+          tmem_ld_nowait<NR>(TY + tlane + (uint32_t)(g * NR), acc);
           tc::tmem_wait_ld();
           const int pos = 128 * h + row;
 #pragma unroll
-          for (int r = 0; r < MAX_SEG; ++r) {
-            if (r < R) {
-              const int cls = G.cls[r];
-              float* dst = cls == 0 ? out + (size_t)G.rid[r] * D : (cls == 1 ? a.head : a.tail) + (size_t)tile * D;
-              dst[pos] = __uint_as_float(acc[r]);
-            }
-          }
+          for (int r = 0; r < NR; ++r)
+            if (r0 + r < R) G.dst[r0 + r][pos] = __uint_as_float(acc[r]);
         }
       } else {
         named_bar_sync(1, N_EPI_WARPS * 32);
@@ -661,14 +716,19 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         uint32_t eb[16];
         tmem_ld16_nowait(TY + tlane + 32u, eb);
         tc::tmem_wait_ld();
+        // u' g_k + u g'_k = g_k (u' - 2 gamma u (r - k Delta)), g_k through ex2.approx as in the feature producers
         const float r = M.r[row], u = M.u[row], du = M.du[row];
+        const float delta = a.r_cut / (float)(a.n_rbf - 1);
+        const float gamma = 0.5f / (delta * delta);
+        const float ngl2 = -gamma * 1.4426950408889634f;
+        const float c1 = -2.0f * gamma * u;
         float part = 0.f;
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
           if (k < a.n_rbf) {
-            float gk, dgk;
-            rbf_f(r, a.r_cut, a.n_rbf, k, gk, dgk);
-            part = fmaf(__uint_as_float(eb[k]), fmaf(du, gk, u * dgk), part);
+            const float dk = r - (float)k * delta;
+            const float gk = ex2_approx(ngl2 * dk * dk);
+            part = fmaf(__uint_as_float(eb[k]), gk * fmaf(c1, dk, du), part);
           }
         }
         const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));

@@ -147,12 +147,12 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   }
   float *m = nullptr, *o = nullptr, *hbar = nullptr, *cbar = nullptr, *PQbar = nullptr, *head = nullptr, *tail = nullptr,
         *rbar = nullptr, *E_i = nullptr, *abar = nullptr;
-  __half* abar_h = nullptr;
+  __half *abar_h = nullptr, *mbar_h = nullptr;
   double* partial = nullptr;
   W_ALLOC(m, float, n * d); W_ALLOC(o, float, n * d); W_ALLOC(hbar, float, n * d); W_ALLOC(cbar, float, n * d);
   W_ALLOC(PQbar, float, n * 2 * d); W_ALLOC(head, float, (tiles + 1) * d); W_ALLOC(tail, float, (tiles + 1) * d);
   W_ALLOC(rbar, float, E + 1); W_ALLOC(E_i, float, n);
-  if (L > 0) { if (bf) W_ALLOC(abar_h, __half, tiles * 128 * d); else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
+  if (L > 0) { if (bf) { W_ALLOC(abar_h, __half, tiles * 128 * d); W_ALLOC(mbar_h, __half, n * d); } else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
   const int64_t n_part = (n + 255) / 256;
   W_ALLOC(partial, double, n_part);
   float* mbar = m;           // m is dead after the forward pass
@@ -231,14 +231,15 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     a.mul_dsilu = c[l]; a.ldz = d; a.Y = cbar; a.ldy = d; a.n = n; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1bT_bf : (const void*)W.V1bT;
-    a.Y = mbar; a.ldy = d; a.n = n; a.N = d;
+    if (bf) a.Yh = mbar_h; else a.Y = mbar;
+    a.ldy = d; a.n = n; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
     a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = n; a.N = d;
     W_TRY(gemm(ctx, a));
     cudaMemsetAsync(Pbar, 0, sizeof(float) * n * d, st);
     set_layer(l);
-    ea.mbar = mbar; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
+    ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
       W_TRY(bf ? mlip_edge_backward_tc(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
