@@ -190,7 +190,7 @@ struct GemmArgs {
   const float* X1 = nullptr; int ld1 = 0; int K1 = 0;
   const float* X2 = nullptr; int ld2 = 0; int K2 = 0;
   int act_in = 0;                 // 1: SiLU applied to X on load
-  const void* B = nullptr;        // [N, K1+K2] row-major (fp32 path) / bf16 row-major (tensor path)
+  const void* B = nullptr;        // [N, K1+K2] row-major (fp32 path) / bf16 SW128 operand image (tensor path)
   const float* bias = nullptr;    // [N]
   const float* mul_dsilu = nullptr; int ldz = 0;  // epilogue: y *= SiLU'(Z[row, col])
   const float* residual = nullptr; int ldr = 0;   // epilogue: y += R[row, col] (may alias Y)
@@ -200,7 +200,8 @@ struct GemmArgs {
   int64_t n = 0; int N = 0;
 };
 int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a);
-int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a);
+int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a);  // B = image built by mlip_make_gemm_image
+void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, __nv_bfloat16* img);
 
 // energy_forces.cu
 int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* m, int L, const SubGraph& g, int precision,

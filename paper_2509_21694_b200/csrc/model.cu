@@ -14,10 +14,6 @@ __global__ void k_copy_sub(const float* __restrict__ src, int ld, int r0, int c0
   const int sr = r0 + (transpose ? c : r), sc = c0 + (transpose ? r : c);
   dst[(size_t)r * ld_dst + c] = src[(size_t)sr * ld + sc];
 }
-__global__ void k_to_bf16(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, int n, float scale) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) dst[i] = __float2bfloat16_rn(scale * src[i]);
-}
 __global__ void k_scale(const float* __restrict__ src, float* __restrict__ dst, int n, float scale) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) dst[i] = scale * src[i];
@@ -148,8 +144,9 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   auto sub = [&](const float* src, int ld, int r0, int c0, int tr, float* dst, int ld_dst, int rows, int cols) {
     k_copy_sub<<<(rows * cols + 255) / 256, 256, 0, st>>>(src, ld, r0, c0, tr, dst, ld_dst, rows, cols);
   };
-  auto tobf = [&](const float* src, __nv_bfloat16* dst, int cnt, float scale = 1.0f) {
-    k_to_bf16<<<(cnt + 255) / 256, 256, 0, st>>>(src, dst, cnt, scale);
+  // bf16 SWIZZLE_128B operand image of a row-major [N, K] weight (node_bf16.cu streams it slab by slab)
+  auto toimg = [&](const float* src, __nv_bfloat16* dst, int N, int K, float scale = 1.0f) {
+    mlip_make_gemm_image(st, src, N, K, scale, dst);
   };
   for (int l = 0; l < L; ++l) {
     LayerWeights& W = M->layers[l];
@@ -178,17 +175,17 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     sub(W.V1, 2 * d, 0, d, 1, W.V1bT, d, d, d);
     cudaMemsetAsync(W.b1pad, 0, sizeof(float) * 2 * d, st);
     cudaMemcpyAsync(W.b1pad, W.b1, sizeof(float) * d, cudaMemcpyDeviceToDevice, st);
-    // bf16 row-major copies for the tensor-core node GEMMs (B operands are [N, K] row-major)
+    // bf16 operand images for the tensor-core node GEMMs (B operands are [N, K])
     M_ALLOC(W.W1a_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1b_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V1_bf, __nv_bfloat16, 2 * d * d); M_ALLOC(W.V2_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V2T_bf, __nv_bfloat16, d * d); M_ALLOC(W.V1aT_bf, __nv_bfloat16, d * d);
     M_ALLOC(W.V1bT_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1abT_bf, __nv_bfloat16, 2 * d * d);
     // the tensor-core edge kernels consume HALVED pre-projections P' = (W1a h + b1)/2, Q' = (W1b h)/2 (exact scaling)
-    tobf(W.W1ab, W.W1a_bf, d * d, 0.5f); tobf(W.W1ab + (size_t)d * d, W.W1b_bf, d * d, 0.5f);
+    toimg(W.W1ab, W.W1a_bf, d, d, 0.5f); toimg(W.W1ab + (size_t)d * d, W.W1b_bf, d, d, 0.5f);
     M_ALLOC(W.b1h, float, d);
     k_scale<<<(d + 255) / 256, 256, 0, st>>>(W.b1, W.b1h, d, 0.5f);
-    tobf(W.V1, W.V1_bf, 2 * d * d); tobf(W.V2, W.V2_bf, d * d); tobf(W.V2T, W.V2T_bf, d * d);
-    tobf(W.V1aT, W.V1aT_bf, d * d); tobf(W.V1bT, W.V1bT_bf, d * d); tobf(W.W1abT, W.W1abT_bf, 2 * d * d);
+    toimg(W.V1, W.V1_bf, d, 2 * d); toimg(W.V2, W.V2_bf, d, d); toimg(W.V2T, W.V2T_bf, d, d);
+    toimg(W.V1aT, W.V1aT_bf, d, d); toimg(W.V1bT, W.V1bT_bf, d, d); toimg(W.W1abT, W.W1abT_bf, d, 2 * d);
     // operand images of the fused edge kernels (tc_images.cuh documents the layouts)
     M_ALLOC(W.W2img, __half, d * d); M_ALLOC(W.W1cimg, __half, d * 16);
     mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg);
@@ -200,7 +197,7 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   M_ALLOC(M->WoT, float, d * d);
   sub(M->Wo, d, 0, 0, 1, M->WoT, d, d, d);
   M_ALLOC(M->Wo_bf, __nv_bfloat16, d * d); M_ALLOC(M->WoT_bf, __nv_bfloat16, d * d);
-  tobf(M->Wo, M->Wo_bf, d * d); tobf(M->WoT, M->WoT_bf, d * d);
+  toimg(M->Wo, M->Wo_bf, d, d); toimg(M->WoT, M->WoT_bf, d, d);
 #undef M_ALLOC
   if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
     ctx->set_error("model preparation kernels failed");

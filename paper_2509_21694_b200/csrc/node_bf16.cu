@@ -1,174 +1,242 @@
 // bf16 tensor-core node-level GEMM with fused prologue / epilogue (steps A8, A9 and their adjoints
 // in the MLIP_BF16 path): Y[n,N] = epi( act(X)[n,K] . B^T + bias ), X = [X1 | X2] fp32 in global.
 //
-// One CTA owns 128 rows and the full output width N (= d). K is streamed in chunks of 64: the
-// threads convert the fp32 activations to bf16 (optionally through SiLU) straight into a K-major
-// SWIZZLE_128B operand slab, the matching [N x 64] slab of the bf16 weight is staged with
-// cp.async, and one thread issues four tcgen05.mma (M=128, N, K=16) into a TMEM accumulator.
-// Two stages: the conversion of chunk k+1 overlaps the MMAs of chunk k (tcgen05.commit -> mbarrier
-// frees a stage). Epilogue: tcgen05.ld -> bias / SiLU' / residual -> fp32 or bf16 rows.
+// The node GEMMs are HBM bound (fp32 activations in and out, 2 d^2 flop per 8..12 bytes per element),
+// so the kernel is built to keep loads in flight, not to feed the tensor pipe: one persistent,
+// warp-specialised CTA per SM walks over 128-row tiles;
+//   warps 0..7   epilogue: TMEM -> registers -> per-warp 32x32 transpose through shared memory, so that
+//                every global access of the epilogue (bias, SiLU' factor, residual, output) is a
+//                full 128-byte row segment -> fp32 / f16 / bf16 rows
+//   warp  8      one thread issues the tcgen05.mma (M=128, N, K=16) into one of TWO accumulators in
+//                tensor memory, so the epilogue of tile t overlaps the main loop of tile t+1
+//   warp  9      one thread streams the [N x 64] SWIZZLE_128B weight slabs (pre-built images, see
+//                mlip_make_gemm_image) with cp.async.bulk
+//   warps 10..17 activation producers: fp32 rows -> (SiLU) -> bf16 -> K-major SWIZZLE_128B slab, with
+//                the loads of the next K chunk (also across tiles) in flight before the current one
+//                is stored
+// through a ring of STAGES (A slab | B slab) buffers guarded by full / empty mbarriers.
 #include "common.cuh"
 #include "mathfn.cuh"
+#include "tc_images.cuh"
 #include "tc_ptx.cuh"
 
 namespace {
 constexpr int BM = 128, BK = 64;
+constexpr int N_EPI = 8, WARP_MMA = 8, WARP_B = 9, WARP_A0 = 10, N_AW = 8;
+constexpr int N_THREADS = (WARP_A0 + N_AW) * 32;  // 576
 
 template <int N>
 struct NodeSmem {
+  static constexpr int STAGES = N == 256 ? 4 : 6;
   static constexpr uint32_t a_bytes = BM * BK * 2;  // 16 KB
   static constexpr uint32_t b_bytes = N * BK * 2;   // 32 KB at N = 256
-  static constexpr uint32_t a_off(int s) { return s * a_bytes; }
-  static constexpr uint32_t b_off(int s) { return 2 * a_bytes + s * b_bytes; }
-  static constexpr uint32_t bar_off = 2 * a_bytes + 2 * b_bytes;
-  static constexpr uint32_t bytes = bar_off + 64 + 1024;  // + alignment slack
+  static constexpr uint32_t stage_bytes = a_bytes + b_bytes;
+  static constexpr uint32_t a_off(int s) { return s * stage_bytes; }
+  static constexpr uint32_t b_off(int s) { return s * stage_bytes + a_bytes; }
+  static constexpr uint32_t xpose = STAGES * stage_bytes;       // 8 warps x [32 x 32] fp32, chunk-swizzled
+  static constexpr uint32_t bars = xpose + N_EPI * 4096;
+  static constexpr uint32_t slot = bars + 8 * (2 * STAGES + 4);
+  static constexpr uint32_t bytes = slot + 16 + 1024;           // + alignment slack
+  static_assert(bytes <= 232448, "shared memory budget of one SM exceeded");
 };
 
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ float4 ldg_stream_f4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+
 template <int N>
-__global__ void __launch_bounds__(256) k_gemm_bf16(GemmArgs a) {
+__global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int64_t n_tiles) {
   extern __shared__ unsigned char smem_raw[];
   using SM = NodeSmem<N>;
-  // SWIZZLE_128B operands need 1024-byte aligned slabs
-  const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
+  constexpr int STAGES = SM::STAGES;
+  const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;  // SWIZZLE_128B slabs need 1024-byte alignment
   unsigned char* gen = smem_raw + (base - tc::smem_u32(smem_raw));
-  const uint32_t bar0 = base + SM::bar_off, bar1 = bar0 + 8;
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(gen + SM::bar_off + 16);
+  auto full = [&](int s) -> uint32_t { return base + SM::bars + 8u * (uint32_t)s; };
+  auto empty = [&](int s) -> uint32_t { return base + SM::bars + 8u * (uint32_t)(STAGES + s); };
+  auto acc_full = [&](int b) -> uint32_t { return base + SM::bars + 8u * (uint32_t)(2 * STAGES + b); };
+  auto acc_empty = [&](int b) -> uint32_t { return base + SM::bars + 8u * (uint32_t)(2 * STAGES + 2 + b); };
+  uint32_t* slot = reinterpret_cast<uint32_t*>(gen + SM::slot);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int64_t row0 = (int64_t)blockIdx.x * BM;
   const int K = a.K1 + a.K2;
   const int nk = K / BK;
-  const __nv_bfloat16* Bw = (const __nv_bfloat16*)a.B;
+  const int64_t my_tiles = (n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
+  const int64_t total = my_tiles * nk;  // K chunks this CTA walks through
 
   if (tid == 0) {
-    tc::mbar_init(bar0, 1);
-    tc::mbar_init(bar1, 1);
+    for (int s = 0; s < STAGES; ++s) { tc::mbar_init(full(s), N_AW + 1); tc::mbar_init(empty(s), 1); }
+    for (int b = 0; b < 2; ++b) { tc::mbar_init(acc_full(b), 1); tc::mbar_init(acc_empty(b), N_EPI); }
     tc::fence_mbar_init();
   }
-  if (warp == 0) tc::tmem_alloc<N>(tmem_slot);
+  if (warp == 0) tc::tmem_alloc<2 * N>(slot);
   tc::fence_before_sync();
   __syncthreads();
   tc::fence_after_sync();
-  const uint32_t tmem = *tmem_slot;
-  constexpr uint32_t IDESC = tc::idesc_bf16(128, N, 0, 0);
+  const uint32_t tmem = *slot;
 
-  for (int kc = 0; kc < nk; ++kc) {
-    const int s = kc & 1;
-    if (kc >= 2) tc::mbar_wait(s ? bar1 : bar0, (uint32_t)(((kc - 2) >> 1) & 1));  // MMAs of chunk kc-2 done
-    const int k0 = kc * BK;
-    // B slab: N rows x 128 B, 16-byte chunks via cp.async
+  if (warp >= WARP_A0) {
+    // ======================= activation producers =======================
+    const int pt = tid - WARP_A0 * 32;  // 0..255: thread = (16-byte column group c4, rows r0 + 16 i)
+    const int c4 = pt & 15, r0 = pt >> 4;
+    auto load = [&](float4 (&v)[8], int64_t g) {
+      if (g >= total) return;
+      const int64_t row0 = ((int64_t)blockIdx.x + (g / nk) * gridDim.x) * BM;
+      const int k0 = (int)(g % nk) * BK;
+      const float* X = k0 < a.K1 ? a.X1 : a.X2;
+      const int ld = k0 < a.K1 ? a.ld1 : a.ld2;
+      const int kx = (k0 < a.K1 ? k0 : k0 - a.K1) + c4 * 4;
 #pragma unroll
-    for (int i = 0; i < N * 8 / 256; ++i) {
-      const int idx = tid + 256 * i;
-      const int n = idx >> 3, ch = idx & 7;
-      tc::cp_async16(base + SM::b_off(s) + tc::sw128_chunk_off(N, n, ch), Bw + (size_t)n * K + k0 + ch * 8);
-    }
-    tc::cp_async_commit();
-    // A slab: 128 rows x 64 fp32 -> bf16
-    const float* X = k0 < a.K1 ? a.X1 : a.X2;
-    const int ld = k0 < a.K1 ? a.ld1 : a.ld2;
-    const int kx = k0 < a.K1 ? k0 : k0 - a.K1;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const int idx = tid + 256 * i;
-      const int r = idx >> 4, c4 = idx & 15;
-      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (row0 + r < a.n) {
-        v = *reinterpret_cast<const float4*>(X + (row0 + r) * ld + kx + c4 * 4);
-        if (a.act_in) { v.x = silu_f(v.x); v.y = silu_f(v.y); v.z = silu_f(v.z); v.w = silu_f(v.w); }
+      for (int i = 0; i < 8; ++i) {
+        const int64_t r = row0 + r0 + 16 * i;
+        v[i] = r < a.n ? ldg_stream_f4(X + r * ld + kx) : make_float4(0.f, 0.f, 0.f, 0.f);
       }
-      uint2 pk;
-      pk.x = tc::pack_bf16(v.x, v.y);
-      pk.y = tc::pack_bf16(v.z, v.w);
-      *reinterpret_cast<uint2*>(gen + SM::a_off(s) + tc::sw128_chunk_off(BM, r, c4 >> 1) + (c4 & 1) * 8) = pk;
+    };
+    auto store = [&](float4 (&v)[8], int64_t g) {
+      if (g >= total) return;
+      const int s = (int)(g % STAGES);
+      tc::mbar_wait(empty(s), (uint32_t)(((g / STAGES) & 1) ^ 1));
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int r = r0 + 16 * i;
+        float4 x = v[i];
+        if (a.act_in) { x.x = silu_f(x.x); x.y = silu_f(x.y); x.z = silu_f(x.z); x.w = silu_f(x.w); }
+        uint2 pk;
+        pk.x = tc::pack_bf16(x.x, x.y);
+        pk.y = tc::pack_bf16(x.z, x.w);
+        *reinterpret_cast<uint2*>(gen + SM::a_off(s) + tc::sw128_chunk_off(BM, r, c4 >> 1) + (c4 & 1) * 8) = pk;
+      }
+      tc::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(full(s));
+    };
+    float4 b0[8], b1[8];
+    load(b0, 0);
+    for (int64_t g = 0; g < total; g += 2) {
+      load(b1, g + 1); store(b0, g);
+      load(b0, g + 2); store(b1, g + 1);
     }
-    tc::cp_async_wait<0>();
-    tc::fence_proxy_async();
-    __syncthreads();
-    if (tid == 0) {
+  } else if (warp == WARP_B) {
+    // ======================= weight slab producer (one thread) =======================
+    if (lane == 0) {
+      const unsigned char* img = reinterpret_cast<const unsigned char*>(a.B);
+      for (int64_t g = 0; g < total; ++g) {
+        const int s = (int)(g % STAGES);
+        tc::mbar_wait(empty(s), (uint32_t)(((g / STAGES) & 1) ^ 1));
+        tc::mbar_expect_tx(full(s), SM::b_bytes);
+        tc::bulk_g2s(base + SM::b_off(s), img + (size_t)(g % nk) * SM::b_bytes, SM::b_bytes, full(s));
+      }
+    }
+  } else if (warp == WARP_MMA) {
+    // ======================= MMA issuer (one thread) =======================
+    if (lane == 0) {
+      constexpr uint32_t IDESC = tc::idesc_bf16(128, N, 0, 0);
+      int64_t g = 0;
+      for (int64_t it = 0; it < my_tiles; ++it) {
+        const int b = (int)(it & 1);
+        tc::mbar_wait(acc_empty(b), (uint32_t)(((it >> 1) & 1) ^ 1));
+        tc::fence_after_sync();
+        for (int kc = 0; kc < nk; ++kc, ++g) {
+          const int s = (int)(g % STAGES);
+          tc::mbar_wait(full(s), (uint32_t)((g / STAGES) & 1));
+          tc::fence_after_sync();
+#pragma unroll
+          for (int kk = 0; kk < BK / 16; ++kk)
+            tc::mma_bf16(tmem + (uint32_t)(b * N), tc::smem_desc(base + SM::a_off(s) + kk * 32, 16, 1024, tc::LAYOUT_SW128),
+                         tc::smem_desc(base + SM::b_off(s) + kk * 32, 16, 1024, tc::LAYOUT_SW128), IDESC, (kc | kk) != 0);
+          tc::mma_commit(empty(s));
+        }
+        tc::mma_commit(acc_full(b));
+      }
+    }
+  } else {
+    // ======================= epilogue warps =======================
+    const int q = warp & 3, hf = warp >> 2;
+    float* xp = reinterpret_cast<float*>(gen + SM::xpose + warp * 4096);
+    const int cj = lane & 7, rj = lane >> 3;  // after the transpose: thread = (row 4 i + rj, columns 4 cj .. 4 cj + 3)
+    for (int64_t it = 0; it < my_tiles; ++it) {
+      const int b = (int)(it & 1);
+      const int64_t row0 = ((int64_t)blockIdx.x + it * gridDim.x) * BM + q * 32;
+      tc::mbar_wait(acc_full(b), (uint32_t)((it >> 1) & 1));
       tc::fence_after_sync();
+#pragma unroll 1
+      for (int c0 = hf * (N / 2); c0 < (hf + 1) * (N / 2); c0 += 32) {
+        uint32_t y[32];
+        tc::tmem_ld32_nowait(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * N + c0), y);
+        float4 bias = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (a.bias) bias = *reinterpret_cast<const float4*>(a.bias + c0 + 4 * cj);
+        tc::tmem_wait_ld();
+        __syncwarp();  // the previous chunk has been read out of the staging tile
 #pragma unroll
-      for (int kk = 0; kk < BK / 16; ++kk) {
-        const uint64_t ad = tc::smem_desc(base + SM::a_off(s) + kk * 32, 16, 1024, tc::LAYOUT_SW128);
-        const uint64_t bd = tc::smem_desc(base + SM::b_off(s) + kk * 32, 16, 1024, tc::LAYOUT_SW128);
-        tc::mma_bf16(tmem, ad, bd, IDESC, (kc | kk) != 0);
+        for (int j = 0; j < 8; ++j)
+          *reinterpret_cast<uint4*>(xp + lane * 32 + ((j ^ (lane & 7)) << 2)) = make_uint4(y[4 * j], y[4 * j + 1], y[4 * j + 2], y[4 * j + 3]);
+        __syncwarp();
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const int rl = 4 * i + rj;
+          const int64_t r = row0 + rl;
+          float4 v = *reinterpret_cast<const float4*>(xp + rl * 32 + ((cj ^ (rl & 7)) << 2));
+          if (r < a.n) {
+            const int c = c0 + 4 * cj;
+            v.x += bias.x; v.y += bias.y; v.z += bias.z; v.w += bias.w;
+            if (a.mul_dsilu) {
+              const float4 z = ldg_stream_f4(a.mul_dsilu + r * a.ldz + c);
+              v.x *= dsilu_f(z.x); v.y *= dsilu_f(z.y); v.z *= dsilu_f(z.z); v.w *= dsilu_f(z.w);
+            }
+            if (a.residual) {
+              const float4 z = *reinterpret_cast<const float4*>(a.residual + r * a.ldr + c);
+              v.x += z.x; v.y += z.y; v.z += z.z; v.w += z.w;
+            }
+            if (a.Y) *reinterpret_cast<float4*>(a.Y + r * a.ldy + c) = v;
+            if (a.Yh) *reinterpret_cast<uint2*>(a.Yh + r * a.ldy + c) = make_uint2(tc::pack_f16(v.x, v.y), tc::pack_f16(v.z, v.w));
+            if (a.Ybf) *reinterpret_cast<uint2*>(a.Ybf + r * a.ldy + c) = make_uint2(tc::pack_bf16(v.x, v.y), tc::pack_bf16(v.z, v.w));
+          }
+        }
       }
-      tc::mma_commit(s ? bar1 : bar0);
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(acc_empty(b));
     }
-  }
-  {
-    const int kl = nk - 1;
-    tc::mbar_wait((kl & 1) ? bar1 : bar0, (uint32_t)((kl >> 1) & 1));
-    tc::fence_after_sync();
   }
 
-  // ---- epilogue: thread = (row, column half) ----
-  const int q = warp & 3, hf = warp >> 2;
-  const int64_t r = row0 + q * 32 + lane;
-  const bool valid = r < a.n;
-#pragma unroll 1
-  for (int c0 = hf * (N / 2); c0 < (hf + 1) * (N / 2); c0 += 32) {
-    float y[32];
-    tc::tmem_ld32(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, y);
-    if (valid) {
-      if (a.bias) {
-#pragma unroll
-        for (int j = 0; j < 32; ++j) y[j] += __ldg(a.bias + c0 + j);
-      }
-      if (a.mul_dsilu) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 z = *reinterpret_cast<const float4*>(a.mul_dsilu + r * a.ldz + c0 + j);
-          y[j] *= dsilu_f(z.x); y[j + 1] *= dsilu_f(z.y); y[j + 2] *= dsilu_f(z.z); y[j + 3] *= dsilu_f(z.w);
-        }
-      }
-      if (a.residual) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 z = *reinterpret_cast<const float4*>(a.residual + r * a.ldr + c0 + j);
-          y[j] += z.x; y[j + 1] += z.y; y[j + 2] += z.z; y[j + 3] += z.w;
-        }
-      }
-      if (a.Y) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4)
-          *reinterpret_cast<float4*>(a.Y + r * a.ldy + c0 + j) = make_float4(y[j], y[j + 1], y[j + 2], y[j + 3]);
-      }
-      if (a.Yh) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 8) {
-          uint4 pk;
-          pk.x = tc::pack_f16(y[j], y[j + 1]); pk.y = tc::pack_f16(y[j + 2], y[j + 3]);
-          pk.z = tc::pack_f16(y[j + 4], y[j + 5]); pk.w = tc::pack_f16(y[j + 6], y[j + 7]);
-          *reinterpret_cast<uint4*>(a.Yh + r * a.ldy + c0 + j) = pk;
-        }
-      }
-      if (a.Ybf) {
-#pragma unroll
-        for (int j = 0; j < 32; j += 8) {
-          uint4 pk;
-          pk.x = tc::pack_bf16(y[j], y[j + 1]); pk.y = tc::pack_bf16(y[j + 2], y[j + 3]);
-          pk.z = tc::pack_bf16(y[j + 4], y[j + 5]); pk.w = tc::pack_bf16(y[j + 6], y[j + 7]);
-          *reinterpret_cast<uint4*>(a.Ybf + r * a.ldy + c0 + j) = pk;
-        }
-      }
-    }
-  }
   tc::fence_before_sync();
   __syncthreads();
-  if (warp == 0) tc::tmem_dealloc<N>(tmem);
+  if (warp == 0) tc::tmem_dealloc<2 * N>(tmem);
+}
+
+// W [N, K] fp32 row-major -> scale * W as the bf16 SWIZZLE_128B K-major operand image the kernel streams:
+// K/64 slabs of [N x 64] (N * 128 bytes each), element (n, k) at tc_sw128_index(N, n, k)
+__global__ void k_gemm_image(const float* __restrict__ W, int N, int K, float scale, __nv_bfloat16* __restrict__ img) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= N * K) return;
+  const int n = idx / K, k = idx % K;
+  img[tc_sw128_index(N, n, k)] = __float2bfloat16_rn(scale * W[idx]);
 }
 
 template <int N>
 int launch(mlip_ctx* ctx, const GemmArgs& a) {
   const size_t smem = NodeSmem<N>::bytes;
-  MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_gemm_bf16<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_gemm_bf16<N><<<(unsigned)((a.n + BM - 1) / BM), 256, smem, ctx->stream>>>(a);
+  static bool configured = false;
+  if (!configured) {
+    MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_gemm_bf16<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = true;
+  }
+  const int64_t tiles = (a.n + BM - 1) / BM;
+  const unsigned grid = (unsigned)(tiles < ctx->num_sms ? tiles : ctx->num_sms);
+  k_gemm_bf16<N><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
   ctx->launches++;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
 }
 }  // namespace
+
+void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, __nv_bfloat16* img) {
+  k_gemm_image<<<(N * K + 255) / 256, 256, 0, st>>>(W, N, K, scale, img);
+}
 
 int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a) {
   if (a.n <= 0) return MLIP_OK;
