@@ -49,6 +49,12 @@ __device__ __forceinline__ float4 ldg_stream_f4(const float* p) {
   return v;
 }
 
+__device__ __forceinline__ float4 ldg_f4(const float* p) {  // ordered with the stores of the same thread (residual may alias Y)
+  float4 v;
+  asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+  return v;
+}
+
 template <int N>
 __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int64_t n_tiles) {
   extern __shared__ unsigned char smem_raw[];
@@ -158,6 +164,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int64_t 
     const int q = warp & 3, hf = warp >> 2;
     float* xp = reinterpret_cast<float*>(gen + SM::xpose + warp * 4096);
     const int cj = lane & 7, rj = lane >> 3;  // after the transpose: thread = (row 4 i + rj, columns 4 cj .. 4 cj + 3)
+    const float* zsrc = a.mul_dsilu ? a.mul_dsilu : a.residual;
+    const int zld = a.mul_dsilu ? a.ldz : a.ldr;
     for (int64_t it = 0; it < my_tiles; ++it) {
       const int b = (int)(it & 1);
       const int64_t row0 = ((int64_t)blockIdx.x + it * gridDim.x) * BM + q * 32;
@@ -167,8 +175,19 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int64_t 
       for (int c0 = hf * (N / 2); c0 < (hf + 1) * (N / 2); c0 += 32) {
         uint32_t y[32];
         tc::tmem_ld32_nowait(tmem + ((uint32_t)(q * 32) << 16) + (uint32_t)(b * N + c0), y);
+        const int c = c0 + 4 * cj;
         float4 bias = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (a.bias) bias = *reinterpret_cast<const float4*>(a.bias + c0 + 4 * cj);
+        if (a.bias) bias = *reinterpret_cast<const float4*>(a.bias + c);
+        // the epilogue operand (SiLU' argument or residual; no caller passes both) of the whole chunk is requested
+        // before anything is stored, so the eight row segments cost one round trip, not eight
+        float4 z[8];
+        if (zsrc) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int64_t r = row0 + 4 * i + rj;
+            z[i] = r < a.n ? ldg_f4(zsrc + r * zld + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+        }
         tc::tmem_wait_ld();
         __syncwarp();  // the previous chunk has been read out of the staging tile
 #pragma unroll
@@ -181,15 +200,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int64_t 
           const int64_t r = row0 + rl;
           float4 v = *reinterpret_cast<const float4*>(xp + rl * 32 + ((cj ^ (rl & 7)) << 2));
           if (r < a.n) {
-            const int c = c0 + 4 * cj;
             v.x += bias.x; v.y += bias.y; v.z += bias.z; v.w += bias.w;
             if (a.mul_dsilu) {
-              const float4 z = ldg_stream_f4(a.mul_dsilu + r * a.ldz + c);
-              v.x *= dsilu_f(z.x); v.y *= dsilu_f(z.y); v.z *= dsilu_f(z.z); v.w *= dsilu_f(z.w);
-            }
-            if (a.residual) {
-              const float4 z = *reinterpret_cast<const float4*>(a.residual + r * a.ldr + c);
-              v.x += z.x; v.y += z.y; v.z += z.z; v.w += z.w;
+              v.x *= dsilu_f(z[i].x); v.y *= dsilu_f(z[i].y); v.z *= dsilu_f(z[i].z); v.w *= dsilu_f(z[i].w);
+            } else if (a.residual) {
+              v.x += z[i].x; v.y += z[i].y; v.z += z[i].z; v.w += z[i].w;
             }
             if (a.Y) *reinterpret_cast<float4*>(a.Y + r * a.ldy + c) = v;
             if (a.Yh) *reinterpret_cast<uint2*>(a.Yh + r * a.ldy + c) = make_uint2(tc::pack_f16(v.x, v.y), tc::pack_f16(v.z, v.w));
@@ -241,6 +256,7 @@ void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float s
 int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a) {
   if (a.n <= 0) return MLIP_OK;
   if (a.K1 % BK || a.K2 % BK || a.K1 + a.K2 == 0) { ctx->set_error("gemm_bf16: K not a multiple of 64"); return MLIP_ERR_UNSUPPORTED; }
+  if (a.mul_dsilu && a.residual) { ctx->set_error("gemm_bf16: SiLU' factor and residual in one epilogue are not supported"); return MLIP_ERR_UNSUPPORTED; }
   if (a.N == 256) return launch<256>(ctx, a);
   if (a.N == 128) return launch<128>(ctx, a);
   ctx->set_error("gemm_bf16: N must be 128 or 256");
