@@ -15,7 +15,7 @@
 //   warp 16      one thread issues every tcgen05.mma as soon as the slab it needs is published
 //   warp 17      segment producer: receivers of the tile, the selector operand of the segmented sum,
 //                and the per-tile staging of the receiver rows P_i (and mbar_i) in shared memory
-//   warps 18,19  feature producers, up to two tiles ahead: edge metadata, envelope, radial basis (A6), the
+//   warp 18      feature producer, up to two tiles ahead: edge metadata, envelope, radial basis (A6), the
 //                f16 e_hat operand of G1
 // Per tile (all factors 1/2 of the SiLU arguments are folded into the weight images, so that
 // SiLU(2x) = x + x tanh(x) costs one MUFU and one FMA):
@@ -44,8 +44,8 @@
 namespace {
 constexpr int TE = 128;          // edges per tile = MMA M
 constexpr int N_EPI_WARPS = 16;  // 4 lane quarters x 4 column groups
-constexpr int WARP_MMA = 16, WARP_SEG = 17, WARP_FEAT = 18, N_FEAT_WARPS = 2;
-constexpr int N_THREADS = 20 * 32;
+constexpr int WARP_MMA = 16, WARP_SEG = 17, WARP_FEAT = 18, N_FEAT_WARPS = 1;
+constexpr int N_THREADS = 19 * 32;
 constexpr int SLOT_BYTES = TE * 128;  // one [128 x 64] f16 SW128 slab
 constexpr int MAX_SEG = 16;           // receivers per tile handled by the selector MMA
 constexpr int NSLOT = 8;              // receivers per tile whose P_i / mbar_i rows are staged in shared memory
@@ -103,10 +103,37 @@ __device__ __forceinline__ uint4 ldg_nc_v4(const void* p) {
   asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
   return v;
 }
+// 32 contiguous bytes (one sector) per thread in ONE 256-bit request: half the L1 wavefronts of two 128-bit loads
+__device__ __forceinline__ void ldg_nc_v8(const void* p, uint4& lo, uint4& hi) {
+  asm volatile("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(lo.x), "=r"(lo.y), "=r"(lo.z), "=r"(lo.w), "=r"(hi.x), "=r"(hi.y), "=r"(hi.z), "=r"(hi.w)
+               : "l"(p));
+}
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+// All 16 Gaussians g_k(r) = exp(-(r/Delta - k)^2 / 2) of one edge from THREE exponentials instead of sixteen (the
+// producers share the MUFU of their SM partition with four epilogue warps): with t = r/Delta - 8,
+// g_8 = exp(-t^2/2) and g_{8+-m} = g_{8+-(m-1)} exp(+-t) exp(1/2 - m). |t| <= 8, so every intermediate stays
+// within e^+-32 and the product of at most 8 factors keeps fp32 accuracy (the result is rounded to f16).
+__device__ __forceinline__ void gaussians16(float r_over_delta, float (&g)[16]) {
+  constexpr float L2E = 1.4426950408889634f;
+  const float t = r_over_delta - 8.0f;
+  float ex;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(-0.5f * L2E * t * t));
+  g[8] = ex;
+  float bp, bm;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(bp) : "f"(L2E * t));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(bm) : "f"(-L2E * t));
+  // exp(1/2 - m), m = 1..8
+  constexpr float C[9] = {0.f, 0.60653065971263342f, 0.22313016014842982f, 0.082084998623898800f, 0.030197383422318501f,
+                          0.011108996538242306f, 0.0040867714384640666f, 0.0015034391929775724f, 0.00055308437014783363f};
+#pragma unroll
+  for (int m = 1; m <= 7; ++m) g[8 + m] = g[8 + m - 1] * (bp * C[m]);
+#pragma unroll
+  for (int m = 1; m <= 8; ++m) g[8 - m] = g[8 - m + 1] * (bm * C[m]);
 }
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t (&r)[16]) {
@@ -218,26 +245,27 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
   if (warp >= WARP_FEAT) {
     // ============ feature producers: tile metadata (two tiles ahead) and the e_hat operand ============
     const float delta = a.r_cut / (float)(a.n_rbf - 1);
-    const float ngl2 = -(0.5f / (delta * delta)) * 1.4426950408889634f;  // -gamma log2(e)
+    const float inv_delta = 1.0f / delta;
     const float inv_rc = 1.0f / a.r_cut;
-    const int ebase = (warp - WARP_FEAT) * 64 + lane;  // this lane's edges: ebase, ebase + 32
+    constexpr int EPL = TE / (32 * N_FEAT_WARPS);  // edges per lane
+    const int ebase = (warp - WARP_FEAT) * (TE / N_FEAT_WARPS) + lane;  // this lane's edges: ebase + 32 k
     int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
       Meta& M = meta[b];
       const int64_t e0 = tile * TE;
-      int rc[2], sd[2];
-      float rr[2];
+      int rc[EPL], sd[EPL];
+      float rr[EPL];
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
+      for (int k = 0; k < EPL; ++k) {
         const int64_t ge = e0 + ebase + 32 * k;
         rc[k] = -1; sd[k] = 0; rr[k] = 0.f;
         if (ge < a.E) { rc[k] = a.recv[ge]; sd[k] = a.send[ge]; rr[k] = a.rvec[ge].w; }
       }
       tc::mbar_wait(bar(B_META_EMPTY + b), (uint32_t)(((it >> 1) & 1) ^ 1));
-      uint32_t pk[2][8];
+      uint32_t pk[EPL][8];
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
+      for (int k = 0; k < EPL; ++k) {
         const int e = ebase + 32 * k;
         float u = 0.f, du = 0.f;
         if (rc[k] >= 0) {
@@ -248,20 +276,18 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         }
         M.recv[e] = rc[k]; M.send[e] = sd[k]; M.w[e] = a.alpha * u;
         if (BWD) { M.r[e] = rr[k]; M.u[e] = u; M.du[e] = du; }
+        float gk[16];
+        gaussians16(rr[k] * inv_delta, gk);
 #pragma unroll
-        for (int j = 0; j < 16; j += 2) {
-          const float d0 = rr[k] - (float)j * delta, d1 = rr[k] - (float)(j + 1) * delta;
-          const float g0 = j < a.n_rbf ? u * ex2_approx(ngl2 * d0 * d0) : 0.f;
-          const float g1 = j + 1 < a.n_rbf ? u * ex2_approx(ngl2 * d1 * d1) : 0.f;
-          pk[k][j >> 1] = tc::pack_f16(g0, g1);
-        }
+        for (int j = 0; j < 16; j += 2)
+          pk[k][j >> 1] = tc::pack_f16(j < a.n_rbf ? u * gk[j] : 0.f, j + 1 < a.n_rbf ? u * gk[j + 1] : 0.f);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(B_META_FULL + b));
       // e_hat operand of G1: K-major, no swizzle: (row, k) -> (row/8)*256 + (k/8)*128 + (row%8)*16 + (k%8)*2
       if (it > 0) tc::mbar_wait(bar(B_D1_FULL), (uint32_t)((it - 1) & 1));  // G1 of the previous tile has read it
 #pragma unroll
-      for (int k = 0; k < 2; ++k) {
+      for (int k = 0; k < EPL; ++k) {
         const int e = ebase + 32 * k;
         unsigned char* dst = gen + SM::ehat + (e >> 3) * 256 + (e & 7) * 16;
         *reinterpret_cast<uint4*>(dst) = make_uint4(pk[k][0], pk[k][1], pk[k][2], pk[k][3]);
@@ -520,17 +546,74 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       *reinterpret_cast<uint4*>(ring + s * SLOT_BYTES + so1) = make_uint4(v[4], v[5], v[6], v[7]);
     };
 
+    // Read-out of a finished tile: segment sums out of Y (and E4). Deferred into E1 of the NEXT tile (after its first
+    // slab is computed, before that slab is published and G2 starts to overwrite Y), so that the selector MMAs and
+    // their completion latency hide under useful work instead of ending every tile with an idle wait.
+    auto read_out = [&](int itp, int64_t tile, bool valid) {
+      const int b = itp & 1;
+      const uint32_t par = (uint32_t)(itp & 1);
+      const Meta& M = meta[b];
+      const TileSeg& G = seg[b];
+      const int64_t e0 = tile * TE;
+      const int R = G.R;
+      tc::mbar_wait(bar(B_SEG_FULL), par);
+      tc::fence_after_sync();
+      if (R <= MAX_SEG) {
+        // Yseg: 16 columns (receiver slots) per 128 channels; warp group g reads 2 NCH of the 8 NCH columns
+        constexpr int NR = 2 * NCH;
+        const int h = (g * NR) >> 4, r0 = (g * NR) & 15;
+        if (r0 < R) {
+          uint32_t acc[NR];
+          tmem_ld_nowait<NR>(TY + tlane + (uint32_t)(g * NR), acc);
+          tc::tmem_wait_ld();
+          const int pos = 128 * h + row;
+#pragma unroll
+          for (int r = 0; r < NR; ++r)
+            if (r0 + r < R) G.dst[r0 + r][pos] = __uint_as_float(acc[r]);
+        }
+      } else {
+        named_bar_sync(1, N_EPI_WARPS * 32);
+        if (tid < D) segmented_store_tc<D>(ring, M.recv, BWD ? nullptr : M.w, a.rowptr, e0, tile, out, a.head, a.tail, tid);
+        named_bar_sync(1, N_EPI_WARPS * 32);
+      }
+      if (BWD && g == 0) {
+        // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k); G4 used the halved W1c image ----
+        uint32_t eb[16];
+        tmem_ld16_nowait(TY + tlane + 32u, eb);
+        tc::tmem_wait_ld();
+        // u' g_k + u g'_k = g_k (u' - 2 gamma u (r - k Delta)), g_k through ex2.approx as in the feature producers
+        const float r = M.r[row], u = M.u[row], du = M.du[row];
+        const float delta = a.r_cut / (float)(a.n_rbf - 1);
+        const float gamma = 0.5f / (delta * delta);
+        const float c1 = -2.0f * gamma * u;
+        float gk[16];
+        gaussians16(r / delta, gk);
+        float part = 0.f;
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+          if (k < a.n_rbf) part = fmaf(__uint_as_float(eb[k]), gk[k] * fmaf(c1, r - (float)k * delta, du), part);
+        const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
+        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, 2.0f * part);
+      }
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_META_EMPTY + b));
+    };
+
     // row metadata and the first Q chunk of a tile are fetched while the previous tile drains
     tc::mbar_wait(bar(B_META_FULL), 0u);
     int rc = meta[0].recv[row];
     float w = meta[0].w[row];
     const __half* Qrow = a.Qh + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
-    // Q'_j chunks of the row, fetched two slabs ahead of their use (rolling buffer of three)
-    uint4 qb[3][2];
-    qb[0][0] = ldg_nc_v4(Qrow); qb[0][1] = ldg_nc_v4(Qrow + 8);
-    qb[1][0] = ldg_nc_v4(Qrow + 64); qb[1][1] = ldg_nc_v4(Qrow + 72);
+    // Q'_j chunks of the row, fetched QD - 1 slabs ahead of their use (rolling buffer of QD; the reverse pass also
+    // keeps SiLU'(a) of the whole row in registers and affords one slab less)
+    constexpr int QD = BWD ? 2 : 3;
+    uint4 qb[QD][2];
+#pragma unroll
+    for (int s = 0; s < QD - 1; ++s) ldg_nc_v8(Qrow + 64 * s, qb[s][0], qb[s][1]);
 
     int it = 0;
+    bool valid_prev = false;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
       const uint32_t par = (uint32_t)(it & 1);
@@ -556,11 +639,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       for (int s = 0; s < NCH; ++s) {
         uint32_t acc[16];
         tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
-        const uint4 q0 = qb[s % 3][0], q1 = qb[s % 3][1];
-        if (s + 2 < NCH) {
-          qb[(s + 2) % 3][0] = ldg_nc_v4(Qrow + 64 * (s + 2));
-          qb[(s + 2) % 3][1] = ldg_nc_v4(Qrow + 64 * (s + 2) + 8);
-        }
+        const uint4 q0 = qb[s % QD][0], q1 = qb[s % QD][1];
+        if (s + QD - 1 < NCH) ldg_nc_v8(Qrow + 64 * (s + QD - 1), qb[(s + QD - 1) % QD][0], qb[(s + QD - 1) % QD][1]);
         uint4 p0, p1;
         if (fast) {
           p0 = *reinterpret_cast<const uint4*>(prow + 128 * s);
@@ -585,6 +665,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
             ds2[s * 8 + j] = tc::h2_fma(v[j], tc::h2_fma(t, H2_NEG_ONE, H2_ONE), tc::h2_add(t, H2_ONE));
         }
         tc::tmem_st8(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
+        if (s == 0 && it > 0) read_out(it - 1, tile - gridDim.x, valid_prev);  // Y of the previous tile, before G2 overwrites it
         publish_tmem(s);
       }
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
@@ -686,60 +767,15 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         rc_n = meta[b ^ 1].recv[row];
         w_n = meta[b ^ 1].w[row];
         Qrow = a.Qh + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
-        qb[0][0] = ldg_nc_v4(Qrow); qb[0][1] = ldg_nc_v4(Qrow + 8);
-        qb[1][0] = ldg_nc_v4(Qrow + 64); qb[1][1] = ldg_nc_v4(Qrow + 72);
+#pragma unroll
+        for (int s = 0; s < QD - 1; ++s) ldg_nc_v8(Qrow + 64 * s, qb[s][0], qb[s][1]);
       }
 
-      // ---- segment sums (and E4) out of Y ----
-      tc::mbar_wait(bar(B_SEG_FULL), par);
-      tc::fence_after_sync();
-      if (R <= MAX_SEG) {
-        // Yseg: 16 columns (receiver slots) per 128 channels; warp group g reads 2 NCH of the 8 NCH columns
-        constexpr int NR = 2 * NCH;
-        const int h = (g * NR) >> 4, r0 = (g * NR) & 15;
-        if (r0 < R) {
-          uint32_t acc[NR];
-          tmem_ld_nowait<NR>(TY + tlane + (uint32_t)(g * NR), acc);
-          tc::tmem_wait_ld();
-          const int pos = 128 * h + row;
-#pragma unroll
-          for (int r = 0; r < NR; ++r)
-            if (r0 + r < R) G.dst[r0 + r][pos] = __uint_as_float(acc[r]);
-        }
-      } else {
-        named_bar_sync(1, N_EPI_WARPS * 32);
-        if (tid < D) segmented_store_tc<D>(ring, M.recv, BWD ? nullptr : M.w, a.rowptr, e0, tile, out, a.head, a.tail, tid);
-        named_bar_sync(1, N_EPI_WARPS * 32);
-      }
-      if (BWD && g == 0) {
-        // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k); G4 used the halved W1c image ----
-        uint32_t eb[16];
-        tmem_ld16_nowait(TY + tlane + 32u, eb);
-        tc::tmem_wait_ld();
-        // u' g_k + u g'_k = g_k (u' - 2 gamma u (r - k Delta)), g_k through ex2.approx as in the feature producers
-        const float r = M.r[row], u = M.u[row], du = M.du[row];
-        const float delta = a.r_cut / (float)(a.n_rbf - 1);
-        const float gamma = 0.5f / (delta * delta);
-        const float ngl2 = -gamma * 1.4426950408889634f;
-        const float c1 = -2.0f * gamma * u;
-        float part = 0.f;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-          if (k < a.n_rbf) {
-            const float dk = r - (float)k * delta;
-            const float gk = ex2_approx(ngl2 * dk * dk);
-            part = fmaf(__uint_as_float(eb[k]), gk * fmaf(c1, dk, du), part);
-          }
-        }
-        const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
-        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, 2.0f * part);
-      }
-      tc::fence_before_sync();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_META_EMPTY + b));
+      valid_prev = valid;
       rc = rc_n;
       w = w_n;
     }
+    if (it > 0) read_out(it - 1, (int64_t)blockIdx.x + (int64_t)(it - 1) * gridDim.x, valid_prev);
   }
 
   tc::fence_before_sync();
