@@ -525,7 +525,6 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     unsigned char* ring = gen + SM::ring;
     const unsigned char* b2h = gen + SM::b2 + 32 * g;  // this thread's 16 channels of b2/2 inside a 64-channel block
     float* out = BWD ? a.Pbar : a.m;
-    uint32_t ds2[BWD ? NCH * 8 : 1];  // 2 SiLU'(2a') of this thread's channels, f16x2
 
     auto publish = [&](int s) {  // slab s written by this warp: visible to the async proxy, then signal
       tc::fence_proxy_async();
@@ -605,9 +604,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     int rc = meta[0].recv[row];
     float w = meta[0].w[row];
     const __half* Qrow = a.Qh + (size_t)(rc >= 0 ? meta[0].send[row] : 0) * D + 16 * g;
-    // Q'_j chunks of the row, fetched QD - 1 slabs ahead of their use (rolling buffer of QD; the reverse pass also
-    // keeps SiLU'(a) of the whole row in registers and affords one slab less)
-    constexpr int QD = BWD ? 2 : 3;
+    // Q'_j chunks of the row, fetched QD - 1 slabs ahead of their use (rolling buffer of QD)
+    constexpr int QD = 3;
     uint4 qb[QD][2];
 #pragma unroll
     for (int s = 0; s < QD - 1; ++s) ldg_nc_v8(Qrow + 64 * s, qb[s][0], qb[s][1]);
@@ -655,21 +653,39 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
 #pragma unroll
         for (int j = 0; j < 8; ++j) pq[j] = tc::h2_add(pw[j], qw[j]);
         tc::tmem_wait_ld();
-        uint32_t v[8];
+        uint32_t v[8], ds2[BWD ? 8 : 1];
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
           const uint32_t x = tc::h2_add(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), pq[j]);
           const uint32_t t = tc::h2_tanh(x);
           v[j] = tc::h2_fma(x, t, x);
           if (BWD)  // 2 SiLU'(2x) = (1 + t) + s (1 - t)
-            ds2[s * 8 + j] = tc::h2_fma(v[j], tc::h2_fma(t, H2_NEG_ONE, H2_ONE), tc::h2_add(t, H2_ONE));
+            ds2[j] = tc::h2_fma(v[j], tc::h2_fma(t, H2_NEG_ONE, H2_ONE), tc::h2_add(t, H2_ONE));
         }
         tc::tmem_st8(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
         if (s == 0 && it > 0) read_out(it - 1, tile - gridDim.x, valid_prev);  // Y of the previous tile, before G2 overwrites it
+        // 2 SiLU'(2a') waits for E3 in this thread's own two chunks of the slab E3 will overwrite with abar: the slab
+        // is free (spilled; read by GS / G4 of the previous tile, whose completion read_out has just waited for)
+        if constexpr (BWD) store_slab(s, ds2);
         publish_tmem(s);
       }
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
       if (lane == 0) mbar_arrive(bar(B_P_FREE));           // staged P rows may be replaced
+
+      // ---- next tile: row metadata and first Q chunk (forward: in flight while the tensor core
+      // finishes G2 and during E2; backward: requested between E2 and E3, when the registers of E2 are free) ----
+      int rc_n = -1;
+      float w_n = 0.f;
+      auto fetch_next = [&]() {
+        if (!has_next) return;
+        tc::mbar_wait(bar(B_META_FULL + (b ^ 1)), (uint32_t)(((it + 1) >> 1) & 1));
+        rc_n = meta[b ^ 1].recv[row];
+        w_n = meta[b ^ 1].w[row];
+        Qrow = a.Qh + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
+#pragma unroll
+        for (int s = 0; s < QD - 1; ++s) ldg_nc_v8(Qrow + 64 * s, qb[s][0], qb[s][1]);
+      };
+      if (!BWD) fetch_next();
 
       // ---- E2 ----
       if (!BWD) {
@@ -739,6 +755,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         }
         if (lane == 0) mbar_arrive(bar(B_MB_FREE));
         ubar_s[g * TE + row] = ub;
+        fetch_next();
 
         // ---- E3: abar = X * 2 SiLU'(2a') -> slabs ----
         tc::mbar_wait(bar(B_D3_FULL), par);
@@ -748,27 +765,18 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           if (s == NCH / 2) { tc::mbar_wait(bar(B_D3B_FULL), par); tc::fence_after_sync(); }
           uint32_t acc[16];
           tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
+          const uint4 d0 = *reinterpret_cast<const uint4*>(ring + s * SLOT_BYTES + so0);
+          const uint4 d1 = *reinterpret_cast<const uint4*>(ring + s * SLOT_BYTES + so1);
+          const uint32_t ds2[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
           tc::tmem_wait_ld();
           uint32_t v[8];
 #pragma unroll
           for (int j = 0; j < 8; ++j)
-            v[j] = tc::h2_mul(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), ds2[s * 8 + j]);
+            v[j] = tc::h2_mul(tc::pack_f16(__uint_as_float(acc[2 * j]), __uint_as_float(acc[2 * j + 1])), ds2[j]);
           store_slab(s, v);
           publish(s);
         }
         if (lane == 0) mbar_arrive(bar(B_X_FREE));
-      }
-
-      // ---- next tile: row metadata and first Q chunk (in flight during the read-out below) ----
-      int rc_n = -1;
-      float w_n = 0.f;
-      if (has_next) {
-        tc::mbar_wait(bar(B_META_FULL + (b ^ 1)), (uint32_t)(((it + 1) >> 1) & 1));
-        rc_n = meta[b ^ 1].recv[row];
-        w_n = meta[b ^ 1].w[row];
-        Qrow = a.Qh + (size_t)(rc_n >= 0 ? meta[b ^ 1].send[row] : 0) * D + 16 * g;
-#pragma unroll
-        for (int s = 0; s < QD - 1; ++s) ldg_nc_v8(Qrow + 64 * s, qb[s][0], qb[s][1]);
       }
 
       valid_prev = valid;
