@@ -89,8 +89,9 @@ struct ES {  // shared-memory carve-up, offsets from a 1024-byte aligned base
 
 // barrier indices
 enum { B_META_FULL = 0, B_META_EMPTY = 2, B_EHAT_FULL = 4, B_SEL_FULL = 5, B_D1_FULL = 6, B_D2_FULL = 7,
-       B_D3_FULL = 8, B_SEG_FULL = 9, B_SPILL_DONE = 10, B_X_FREE = 11, B_P_FULL = 12, B_P_FREE = 13,
-       B_MB_FULL = 14, B_MB_FREE = 15, B_D2B_FULL = 16, B_D3B_FULL = 17, B_S_READY = 18 /* .. +NCH */ };
+       B_D3_FULL = 8, B_SEG_FULL = 9, B_X_FREE = 11, B_P_FULL = 12, B_P_FREE = 13,
+       B_MB_FULL = 14, B_MB_FREE = 15, B_D2B_FULL = 16, B_D3B_FULL = 17, B_S_READY = 18 /* .. +NCH */,
+       B_SPILL_S = 22 /* .. +NCH: slab s of the previous tile has been read by its spill copy */ };
 
 constexpr uint32_t H2_ONE = 0x3C003C00u, H2_HALF = 0x38003800u, H2_NEG_ONE = 0xBC00BC00u, H2_NEG_HALF = 0xB800B800u;
 
@@ -227,7 +228,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     tc::mbar_init(bar(B_META_EMPTY), N_EPI_WARPS); tc::mbar_init(bar(B_META_EMPTY + 1), N_EPI_WARPS);
     tc::mbar_init(bar(B_EHAT_FULL), N_FEAT_WARPS); tc::mbar_init(bar(B_SEL_FULL), 1);
     tc::mbar_init(bar(B_D1_FULL), 1); tc::mbar_init(bar(B_D2_FULL), 1); tc::mbar_init(bar(B_D3_FULL), 1);
-    tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_SPILL_DONE), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
+    tc::mbar_init(bar(B_SEG_FULL), 1); tc::mbar_init(bar(B_X_FREE), N_EPI_WARPS);
+    for (int s = 0; s < NCH; ++s) tc::mbar_init(bar(B_SPILL_S + s), 1);
     tc::mbar_init(bar(B_P_FULL), 1); tc::mbar_init(bar(B_P_FREE), N_EPI_WARPS);
     tc::mbar_init(bar(B_MB_FULL), 1); tc::mbar_init(bar(B_MB_FREE), N_EPI_WARPS);
     tc::mbar_init(bar(B_D2B_FULL), 1); tc::mbar_init(bar(B_D3B_FULL), 1);
@@ -488,6 +490,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           wait_slab(s);
           if (BWD) {
             tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
+            tc::bulk_commit();  // one bulk group per slab: a slab is released as soon as ITS copy has read it
             // G4: ebar/2 = abar . (W1c/2). B = the G1 image [channel][16] read MN-major (N = rbf index, K = channel),
             // no swizzle: N-direction core-matrix stride (SBO) 128 B, K-direction 8-channel group stride (LBO) 256 B
 #pragma unroll
@@ -503,13 +506,16 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
                            tc::smem_desc(base + SM::ring + (s - 1) * SLOT_BYTES + j * 2048, SLOT_BYTES, 1024, tc::LAYOUT_SW128),
                            tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
           }
+          if (BWD && s > 0) {
+            tc::bulk_wait_read<1>();  // every spill copy but the newest has read its slab
+            mbar_arrive(bar(B_SPILL_S + s - 1));
+          }
         }
         tc::mma_commit(bar(B_SEG_FULL));
         if (BWD) {
           if (has_next) issue_g1(it + 1);  // backward: X (D3) is released by the last E3 read
-          tc::bulk_commit();
-          tc::bulk_wait_read0();  // the spill has finished reading the slabs
-          mbar_arrive(bar(B_SPILL_DONE));
+          tc::bulk_wait_read<0>();
+          mbar_arrive(bar(B_SPILL_S + NCH - 1));
         }
       }
       if (BWD) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -620,7 +626,6 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       const int64_t e0 = tile * TE;
       const bool has_next = tile + gridDim.x < n_tiles;
       const bool valid = rc >= 0;
-      if (BWD && it > 0) tc::mbar_wait(bar(B_SPILL_DONE), (uint32_t)((it - 1) & 1));  // slabs of the previous tile spilled
 
       // receiver rows of the tile: staged in shared memory (R <= NSLOT) or read from global memory
       tc::mbar_wait(bar(B_P_FULL), par);
@@ -665,8 +670,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         tc::tmem_st8(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
         if (s == 0 && it > 0) read_out(it - 1, tile - gridDim.x, valid_prev);  // Y of the previous tile, before G2 overwrites it
         // 2 SiLU'(2a') waits for E3 in this thread's own two chunks of the slab E3 will overwrite with abar: the slab
-        // is free (spilled; read by GS / G4 of the previous tile, whose completion read_out has just waited for)
-        if constexpr (BWD) store_slab(s, ds2);
+        // is free once its spill copy has read it (GS / G4 of the previous tile are done: read_out has waited for them)
+        if constexpr (BWD) {
+          if (it > 0) tc::mbar_wait(bar(B_SPILL_S + s), (uint32_t)((it - 1) & 1));
+          store_slab(s, ds2);
+        }
         publish_tmem(s);
       }
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
@@ -760,15 +768,19 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         // ---- E3: abar = X * 2 SiLU'(2a') -> slabs ----
         tc::mbar_wait(bar(B_D3_FULL), par);
         tc::fence_after_sync();
+        uint32_t accb[2][16];  // the accumulator columns of slab s + 1 are in flight while slab s is processed
+        tmem_ld16_nowait(TX + tlane + (uint32_t)(16 * g), accb[0]);
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
-          if (s == NCH / 2) { tc::mbar_wait(bar(B_D3B_FULL), par); tc::fence_after_sync(); }
-          uint32_t acc[16];
-          tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * s + 16 * g), acc);
           const uint4 d0 = *reinterpret_cast<const uint4*>(ring + s * SLOT_BYTES + so0);
           const uint4 d1 = *reinterpret_cast<const uint4*>(ring + s * SLOT_BYTES + so1);
           const uint32_t ds2[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
           tc::tmem_wait_ld();
+          if (s + 1 < NCH) {
+            if (s + 1 == NCH / 2) { tc::mbar_wait(bar(B_D3B_FULL), par); tc::fence_after_sync(); }
+            tmem_ld16_nowait(TX + tlane + (uint32_t)(64 * (s + 1) + 16 * g), accb[(s + 1) & 1]);
+          }
+          const uint32_t (&acc)[16] = accb[s & 1];
           uint32_t v[8];
 #pragma unroll
           for (int j = 0; j < 8; ++j)
