@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--precision", default="auto", choices=["auto", "fp32", "bf16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-active-sets", action="store_true",
+                    help="evaluate every layer on the whole extended sub-graph (A/B against the per-layer active sets)")
     ap.add_argument("--n-cells", type=int, default=None, help="shrink the fcc box (debugging only; not a bench line)")
     return ap.parse_args()
 
@@ -215,6 +217,7 @@ def run_ours(args):
         raise SystemExit("bench.py: --gpus > 1 needs a partitioned config (sub-domains are the unit that shards)")
 
     ctx = mlip.Context(local_rank)
+    ctx.set_active_sets(not args.no_active_sets)
     model = mlip.Model(ctx, m.n_species, m.d, m.n_rbf, m.L_max, m.r_cut, m.agg_scale, cfg.weights)
     pos = torch.tensor(s.pos, dtype=torch.float64, device=dev)
     species = torch.tensor(s.species, dtype=torch.int32, device=dev)
@@ -233,6 +236,9 @@ def run_ours(args):
             E, F, _ = mlip.energy_forces(ctx, model, cfg.L, g, part, prec, want_atom_energy=False, out=out)
         info["edges"] = g.num_edges
         info["subs"] = part.info() if part is not None else [dict(n_owned=N, n_ext=N, n_edges=g.num_edges)]
+        # edge evaluations per layer and sub-domain (per-layer active sets: mlip_part_layer_info)
+        info["layers"] = (part.layer_info(cfg.L) if part is not None
+                          else [[dict(n_recv=N, n_send=N, n_edges=g.num_edges)] * cfg.L])
         return E, F
 
     def barrier():
@@ -294,9 +300,11 @@ def run_ours(args):
     # ---- roofline of the dominant kernel group ----
     pk = peaks()
     edges_total = sum(x["n_edges"] for x in info["subs"][rank::world]) if world > 1 else sum(x["n_edges"] for x in info["subs"])
+    mine = info["layers"][rank::world] if world > 1 else info["layers"]
+    edge_layers = sum(r["n_edges"] for rows in mine for r in rows)   # edge-layer evaluations actually launched
     per_step = {k: v[0] / args.steps for k, v in groups.items()}
     dom = max(("edge_fwd", "edge_bwd"), key=lambda k: per_step[k])
-    flop = edges_total * cfg.L * flops_edge_layer(m.d, m.n_rbf)
+    flop = edge_layers * flops_edge_layer(m.d, m.n_rbf)
     achieved = flop / (per_step[dom] * 1e-3) / 1e12 if per_step[dom] > 0 else 0.0
     if prec_name == "bf16":
         bound, peak, peak_src = "tensor", pk["bf16_tflops_sustained"], pk["_source"] + " (sustained cuBLAS bf16)"
@@ -321,7 +329,8 @@ def run_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": "bf16" if prec_name == "bf16" else "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg, N), "n_atoms": N, "n_edges": info["edges"],
-                   "sub_domains": len(info["subs"]), "edges_evaluated_per_step": int(edges_total),
+                   "sub_domains": len(info["subs"]), "edges_in_subgraphs": int(edges_total),
+                   "edge_layers_evaluated_per_step": int(edge_layers), "active_sets": not args.no_active_sets,
                    "halo_growth_H": float(np.mean([(e - o) / max(o, 1) for o, e in zip(n_own, n_ext)])),
                    "l2": "256 MiB buffer rewritten between timed iterations; working set also exceeds the 126 MB L2"
                    if N > 200000 else "256 MiB buffer rewritten between timed iterations",

@@ -115,6 +115,16 @@ int mlip_part_count(const mlip_part* p, int* n_sub);
 /* Sizes of sub-domain s: root (owned) atoms, extended atoms, induced directed edges. The halo
  * growth factor of PAPER.md:289 is (n_ext - n_owned) / n_owned. */
 int mlip_part_info(const mlip_part* p, int s, int64_t* n_owned, int64_t* n_ext, int64_t* n_edges);
+/* Per-layer active sets of sub-domain s when the first L layers are evaluated. The extended atoms of a sub-domain are
+ * numbered by depth class (0 = root atoms; k >= 1 = halo atoms whose largest per-axis periodic distance to the bin lies
+ * in ((k-1) r_c, k r_c]). An edge is shorter than r_c, so the root energies of PAPER.md:169 and their gradient
+ * depend on layer l (0-based) only through receivers of class <= L-1-l and senders of class <= L-l:
+ * the K-hop neighbourhood of PAPER.md:165 shrinks by one hop per layer. mlip_energy_forces evaluates exactly those
+ * prefixes; the result is identical to evaluating every layer on the whole extended sub-graph.
+ *   n_recv  atoms whose h^{l+1} is computed, n_send atoms whose h^l is read, n_edges edges evaluated by layer l
+ * (with active sets switched off through mlip_ctx_set_active_sets: n_ext, n_ext, all induced edges). */
+int mlip_part_layer_info(const mlip_part* p, int s, int L, int l, int64_t* n_recv, int64_t* n_send,
+                         int64_t* n_edges);
 void mlip_part_destroy(mlip_part* p);
 
 /* Energy and forces with the first L of L_max layers (MPDP).
@@ -149,6 +159,10 @@ int mlip_step_host(mlip_ctx* ctx, const mlip_model* m, int L, const double* pos_
                    const double* cell_host, const int32_t* species_host, int64_t n_atoms,
                    const int grid[3], double halo, int precision, double* energy_host,
                    float* forces_host);
+
+/* Per-layer active sets inside sub-domains (see mlip_part_layer_info): on by default; enable = 0 makes every layer run
+ * on the whole extended sub-graph (same results; kept for A/B measurement and as a test control). */
+int mlip_ctx_set_active_sets(mlip_ctx* ctx, int enable);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);

@@ -403,6 +403,52 @@ def energy_forces_partitioned(model, L, pos, cell, species, parts, graph=None):
     return E, E_i, F, stats
 
 
+def khop_distance(graph, owned_idx, n_atoms, max_hops):
+    """Stage 2 of PAPER.md:165 as stated: breadth-first search over the radius graph from the root atoms
+    of a bin. Returns hops[n_atoms] = number of edges on the shortest path to the nearest root atom
+    (0 for root atoms, max_hops + 1 for atoms farther than max_hops)."""
+    recv, send, _ = graph
+    hops = np.full(n_atoms, max_hops + 1, np.int64)
+    hops[owned_idx] = 0
+    frontier = np.zeros(n_atoms, bool)
+    frontier[owned_idx] = True
+    for k in range(1, max_hops + 1):
+        reached = np.zeros(n_atoms, bool)
+        reached[send[frontier[recv]]] = True          # senders of edges into the frontier
+        new = reached & (hops > k)
+        hops[new] = k
+        frontier = new
+    return hops
+
+
+def halo_depth_classes(pos, cell, grid, halo, r_cut):
+    """Depth class of every atom of every extended set (same bins, same order as partition_grid):
+    0 for root atoms, else ceil(D / r_cut) clipped to [1, ceil(halo / r_cut)], D = the largest per-axis
+    periodic distance to the bin interval. An edge is shorter than r_cut, so a class-k atom is at least k
+    hops from the nearest root atom (pinned against khop_distance in tests/test_oracle_graph.py): layer l
+    of L (0-based) matters for the root energies of PAPER.md:169 only on receivers of class <= L-1-l.
+    Returns a list of int arrays aligned with the ext_idx of partition_grid."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    frac = pos @ np.linalg.inv(cell)
+    f = frac - np.floor(frac)
+    wk = perpendicular_widths(cell)
+    g = np.asarray(grid, int)
+    n_cls = max(2, 1 + int(np.ceil(halo / r_cut - 1e-9)))
+    out = []
+    for (owned, ext), b in zip(partition_grid(pos, cell, grid, halo), np.ndindex(*g)):
+        D = np.zeros(len(pos))
+        for k in range(3):
+            lo, hi = b[k] / g[k], (b[k] + 1) / g[k]
+            inside = (f[:, k] >= lo) & (f[:, k] < hi)
+            below = np.mod(lo - f[:, k], 1.0)
+            above = np.mod(f[:, k] - hi, 1.0)
+            D = np.maximum(D, np.where(inside, 0.0, np.minimum(below, above)) * wk[k])
+        cls = np.clip(np.ceil(D / r_cut - 1e-9).astype(np.int64), 1, n_cls - 1)
+        cls[owned] = 0
+        out.append(cls[ext])
+    return out
+
+
 def halo_growth_factor(parts):
     """H = (# atoms added by the halo) / (# root atoms), PAPER.md:289 (S1)."""
     return [(len(ext) - len(owned)) / max(len(owned), 1) for owned, ext in parts]

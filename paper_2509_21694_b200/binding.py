@@ -62,7 +62,9 @@ def load_library():
     lib.mlip_partition_grid.argtypes = [vp, vp, P(i32), dbl, P(vp)]
     lib.mlip_part_count.argtypes = [vp, P(i32)]
     lib.mlip_part_info.argtypes = [vp, i32, P(i64), P(i64), P(i64)]
+    lib.mlip_part_layer_info.argtypes = [vp, i32, i32, i32, P(i64), P(i64), P(i64)]
     lib.mlip_part_destroy.argtypes = [vp]; lib.mlip_part_destroy.restype = None
+    lib.mlip_ctx_set_active_sets.argtypes = [vp, i32]
     lib.mlip_energy_forces.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
     lib.mlip_energy_forces_shard.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.mlip_step_host.argtypes = [vp, vp, i32, vp, vp, vp, i64, P(i32), dbl, i32, vp, vp]
@@ -111,6 +113,10 @@ class Context:
     @property
     def launches(self) -> int:
         return int(self.lib.mlip_ctx_launch_count(self.h))
+
+    def set_active_sets(self, enable: bool):
+        """mlip_ctx_set_active_sets: per-layer active sets inside sub-domains (on by default)."""
+        self.check(self.lib.mlip_ctx_set_active_sets(self.h, 1 if enable else 0))
 
     def profile(self, enable: bool):
         """mlip_ctx_profile: start (clearing the counters) or stop per-kernel-group event timing."""
@@ -210,6 +216,20 @@ class Partition:
             a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
             self.ctx.check(self.ctx.lib.mlip_part_info(self.h, s, C.byref(a), C.byref(b), C.byref(c)))
             out.append(dict(n_owned=a.value, n_ext=b.value, n_edges=c.value))
+        return out
+
+    def layer_info(self, L: int):
+        """mlip_part_layer_info for every sub-domain and layer -> [[dict(n_recv, n_send, n_edges)] * L] * n_sub."""
+        n = C.c_int()
+        self.ctx.check(self.ctx.lib.mlip_part_count(self.h, C.byref(n)))
+        out = []
+        for s in range(n.value):
+            rows = []
+            for l in range(L):
+                a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+                self.ctx.check(self.ctx.lib.mlip_part_layer_info(self.h, s, int(L), l, C.byref(a), C.byref(b), C.byref(c)))
+                rows.append(dict(n_recv=a.value, n_send=b.value, n_edges=c.value))
+            out.append(rows)
         return out
 
     def __del__(self):

@@ -42,6 +42,7 @@ struct mlip_ctx {
   int num_sms = 148;
   std::string err;
   int64_t launches = 0;
+  bool active_sets = true;  // per-layer active sets inside sub-domains (mlip_ctx_set_active_sets)
   void set_error(const std::string& s) { err = s; }
   // ---- optional per-group timing ----
   struct ProfRec { int cat; int64_t launches; cudaEvent_t a, b; };
@@ -125,6 +126,7 @@ struct mlip_model {
 };
 
 // ---- graph --------------------------------------------------------------------------------
+constexpr int MLIP_MAX_CLS = 32;
 // A (sub)graph in the form the model kernels consume: atoms are numbered locally, edges are
 // sorted by receiver, rows sorted by (sender, shift).
 struct SubGraph {
@@ -139,6 +141,16 @@ struct SubGraph {
   const int32_t* send = nullptr;     // [E]
   const int32_t* rev = nullptr;      // [E] index of the reverse edge
   const float4* rvec = nullptr;      // [E] (r_x, r_y, r_z, |r|), float32 rounded from float64
+  // Depth classes (sub-domains only; n_cls == 0 means "no classes, every layer runs on all atoms"). Atoms are numbered
+  // by (class, cell order): class 0 = root atoms, class k >= 1 = halo atoms whose largest per-axis periodic distance to
+  // the bin lies in ((k-1) r_c, k r_c]. An edge is shorter than r_c, so an atom of class k only has neighbours of class
+  // >= k-1, and the root energies (and their gradient) need layer l only on receivers of class <= L-1-l with senders of
+  // class <= L-l (each root atom keeps its K-hop neighbourhood). Both sets are prefixes of the numbering.
+  int n_cls = 0;
+  int64_t n_le[MLIP_MAX_CLS] = {};   // atoms of class <= c
+  int64_t E_le[MLIP_MAX_CLS] = {};   // edges whose receiver has class <= c  (= rowptr[n_le[c]])
+  int64_t atoms_upto(int c) const { return n_cls == 0 ? n : n_le[c < 0 ? 0 : (c >= n_cls ? n_cls - 1 : c)]; }
+  int64_t edges_upto(int c) const { return n_cls == 0 ? E : E_le[c < 0 ? 0 : (c >= n_cls ? n_cls - 1 : c)]; }
 };
 
 struct mlip_graph {

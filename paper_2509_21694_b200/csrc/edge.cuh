@@ -34,11 +34,12 @@ struct EdgeArgs {
 int64_t mlip_edge_f32_tiles(int64_t E);
 int mlip_edge_forward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
-int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
+// Qbar_j = sum over in-edges e of j, j < n, with rev[e] < E_act, of abar[rev[e]]
+int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
                         const float* abar, float* Qbar);
 
 int64_t mlip_edge_tc_tiles(int64_t E);
 int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
-int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev,
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
                        const __half* abar, float* Qbar);

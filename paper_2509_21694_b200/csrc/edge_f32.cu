@@ -293,7 +293,7 @@ __global__ void k_segment_fixup(int64_t E, int D, const int32_t* __restrict__ ro
 }
 
 // Qbar_j = sum_{e in in(j)} abar[rev[e]]  (sender-side adjoint gathered through the reverse index)
-__global__ void __launch_bounds__(256) k_gather_rev_f32(int64_t n, int D, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_gather_rev_f32(int64_t n, int64_t E_act, int D, const int32_t* __restrict__ rowptr,
                                                         const int32_t* __restrict__ rev, const float* __restrict__ abar,
                                                         float* __restrict__ Qbar) {
   const int lane = threadIdx.x & 31;
@@ -305,7 +305,9 @@ __global__ void __launch_bounds__(256) k_gather_rev_f32(int64_t n, int D, const 
     const int c = c0 + lane * 4;
     if (c < D) {
       for (int e = lo; e < hi; ++e) {
-        const float4 v = *reinterpret_cast<const float4*>(abar + (size_t)rev[e] * D + c);
+        const int re = rev[e];
+        if (re >= E_act) continue;  // not evaluated by this layer: zero adjoint
+        const float4 v = *reinterpret_cast<const float4*>(abar + (size_t)re * D + c);
         s.x += v.x; s.y += v.y; s.z += v.z; s.w += v.w;
       }
       *reinterpret_cast<float4*>(Qbar + (size_t)j * D + c) = s;
@@ -351,10 +353,10 @@ int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   }
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev, const float* abar,
-                        float* Qbar) {
+int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
+                        const float* abar, float* Qbar) {
   if (n <= 0) return MLIP_OK;
-  k_gather_rev_f32<<<(unsigned)((n * 32 + 255) / 256), 256, 0, ctx->stream>>>(n, d, rowptr, rev, abar, Qbar);
+  k_gather_rev_f32<<<(unsigned)((n * 32 + 255) / 256), 256, 0, ctx->stream>>>(n, E_act, d, rowptr, rev, abar, Qbar);
   ctx->launches++;
   return MLIP_OK;
 }

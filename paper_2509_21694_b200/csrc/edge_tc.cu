@@ -821,7 +821,7 @@ __global__ void k_segment_fixup_tc(int64_t E, int D, const int32_t* __restrict__
 
 // Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled f16 tile images written by E3
 template <int D>
-__global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act, const int32_t* __restrict__ rowptr,
                                                        const int32_t* __restrict__ rev, const __half* __restrict__ abar,
                                                        float* __restrict__ Qbar) {
   constexpr int CH = D / 8;        // 16-byte chunks per row
@@ -835,6 +835,7 @@ __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, const int32_t*
   const unsigned char* base = reinterpret_cast<const unsigned char*>(abar);
   for (int e = lo + sub; e < hi; e += NSUB) {
     const int re = rev[e];
+    if (re >= E_act) continue;  // reverse edge outside this layer's active set: its adjoint is zero and was not written
     const int t = re >> 7, rw = re & 127;
     const uint4 v = *reinterpret_cast<const uint4*>(base + (size_t)t * TE * D * 2 + tc::sw128_chunk_off(TE, rw, ch));
     const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
@@ -885,12 +886,12 @@ int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   ctx->set_error("tensor-core edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int d, const int32_t* rowptr, const int32_t* rev, const __half* abar,
-                       float* Qbar) {
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
+                       const __half* abar, float* Qbar) {
   if (n <= 0) return MLIP_OK;
   const unsigned grid = (unsigned)((n * 32 + 255) / 256);
-  if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
-  else if (d == 128) k_gather_rev_tc<128><<<grid, 256, 0, ctx->stream>>>(n, rowptr, rev, abar, Qbar);
+  if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, E_act, rowptr, rev, abar, Qbar);
+  else if (d == 128) k_gather_rev_tc<128><<<grid, 256, 0, ctx->stream>>>(n, E_act, rowptr, rev, abar, Qbar);
   else { ctx->set_error("tensor-core gather needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
   ctx->launches++;
   return MLIP_OK;

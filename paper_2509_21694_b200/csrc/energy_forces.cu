@@ -176,69 +176,83 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     ea.W2img = W.W2img; ea.W1cimg = W.W1cimg;
   };
 
+  // Active sets (SubGraph depth classes): layer l runs on receivers [0, nr) = classes <= L-1-l, reads senders
+  // [0, ns) = classes <= L-l and therefore evaluates the edge prefix [0, Er). Rows beyond nr of h[l+1] are never read.
+  const bool act = ctx->active_sets;
+  auto n_recv = [&](int l) { return act ? g.atoms_upto(L - 1 - l) : n; };
+  auto n_send = [&](int l) { return act ? g.atoms_upto(L - l) : n; };
+  auto e_recv = [&](int l) { return act ? g.edges_upto(L - 1 - l) : E; };
+  const int64_t n0 = act ? g.atoms_upto(0) : n;  // root atoms (everything when there are no classes)
+
   for (int l = 0; l < L; ++l) {
     const LayerWeights& W = M->layers[l];
+    const int64_t nr = n_recv(l), ns = n_send(l);
     GemmArgs a;
     if (bf) {
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = n; a.N = d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = nr; a.N = d;
       W_TRY(gemm(ctx, a));
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = n; a.N = d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = ns; a.N = d;
       W_TRY(gemm(ctx, a));
     } else {
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1ab; a.bias = W.b1pad; a.Y = P[l]; a.ldy = 2 * d; a.n = n; a.N = 2 * d;
+      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1ab; a.bias = W.b1pad; a.Y = P[l]; a.ldy = 2 * d; a.n = ns; a.N = 2 * d;
       W_TRY(gemm(ctx, a));
     }
-    cudaMemsetAsync(m, 0, sizeof(float) * n * d, st);
+    cudaMemsetAsync(m, 0, sizeof(float) * nr * d, st);
     set_layer(l);
-    ea.m = m;
+    ea.m = m; ea.E = e_recv(l); ea.n = nr;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
       W_TRY(bf ? mlip_edge_forward_tc(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
     }
     a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.X2 = m; a.ld2 = d; a.K2 = d;
-    a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = n; a.N = d;
+    a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = c[l]; a.ld1 = d; a.K1 = d; a.act_in = 1;
     a.B = bf ? (const void*)W.V2_bf : (const void*)W.V2; a.bias = W.c2; a.residual = h[l]; a.ldr = d;
-    a.Y = h[l + 1]; a.ldy = d; a.n = n; a.N = d;
+    a.Y = h[l + 1]; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
   }
   {
     GemmArgs a;
     a.X1 = h[L]; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->Wo_bf : (const void*)M->Wo; a.bias = M->bo;
-    a.Y = o; a.ldy = d; a.n = n; a.N = d;
+    a.Y = o; a.ldy = d; a.n = n0; a.N = d;
     W_TRY(gemm(ctx, a));
   }
   float* obar = cbar;
   {
     ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
-    k_readout<<<nblk(n * 32, 256), 256, 0, st>>>(n, d, o, M->wo, M->bE, M->E0, g.species, g.omega, E_i, obar);
-    k_energy_partial<<<(unsigned)n_part, 256, 0, st>>>(n, E_i, g.omega, g.gid, partial, Ei_int);
-    k_energy_final<<<1, 256, 0, st>>>(n_part, partial, energy_accum);
+    k_readout<<<nblk(n0 * 32, 256), 256, 0, st>>>(n0, d, o, M->wo, M->bE, M->E0, g.species, g.omega, E_i, obar);
+    k_energy_partial<<<(unsigned)((n0 + 255) / 256), 256, 0, st>>>(n0, E_i, g.omega, g.gid, partial, Ei_int);
+    k_energy_final<<<1, 256, 0, st>>>((n0 + 255) / 256, partial, energy_accum);
     ctx->launches += 3;
   }
   {
     GemmArgs a;
     a.X1 = obar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->WoT_bf : (const void*)M->WoT;
-    a.Y = hbar; a.ldy = d; a.n = n; a.N = d;
+    a.Y = hbar; a.ldy = d; a.n = n0; a.N = d;
     W_TRY(gemm(ctx, a));
   }
+  // the adjoint of h^{l+1} is non-zero on the receivers of layer l only; the rows the sender-side GEMM of layer l adds
+  // ([nr, ns)) must start from zero
+  if (n > n0) cudaMemsetAsync(hbar + n0 * d, 0, sizeof(float) * (n - n0) * d, st);
   cudaMemsetAsync(rbar, 0, sizeof(float) * (E + 1), st);
   for (int l = L - 1; l >= 0; --l) {
     const LayerWeights& W = M->layers[l];
+    const int64_t nr = n_recv(l), ns = n_send(l), Er = e_recv(l);
     GemmArgs a;
     a = GemmArgs(); a.X1 = hbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V2T_bf : (const void*)W.V2T;
-    a.mul_dsilu = c[l]; a.ldz = d; a.Y = cbar; a.ldy = d; a.n = n; a.N = d;
+    a.mul_dsilu = c[l]; a.ldz = d; a.Y = cbar; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1bT_bf : (const void*)W.V1bT;
     if (bf) a.Yh = mbar_h; else a.Y = mbar;
-    a.ldy = d; a.n = n; a.N = d;
+    a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
-    a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = n; a.N = d;
+    a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
-    cudaMemsetAsync(Pbar, 0, sizeof(float) * n * d, st);
+    cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
     set_layer(l);
+    ea.E = Er; ea.n = nr;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
@@ -246,12 +260,13 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     }
     {
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
-      W_TRY(bf ? mlip_gather_rev_tc(ctx, n, d, g.rowptr, g.rev, abar_h, Qbar)
-               : mlip_gather_rev_f32(ctx, n, d, g.rowptr, g.rev, abar, Qbar));
+      // Qbar_j over the senders of this layer, summing only the reverse edges that were evaluated (rev[e] < Er)
+      W_TRY(bf ? mlip_gather_rev_tc(ctx, ns, Er, d, g.rowptr, g.rev, abar_h, Qbar)
+               : mlip_gather_rev_f32(ctx, ns, Er, d, g.rowptr, g.rev, abar, Qbar));
     }
     a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.X2 = Qbar; a.ld2 = d; a.K2 = d;
     a.B = bf ? (const void*)W.W1abT_bf : (const void*)W.W1abT; a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d;
-    a.n = n; a.N = d;
+    a.n = ns; a.N = d;
     W_TRY(gemm(ctx, a));
   }
   {

@@ -9,15 +9,20 @@ namespace {
 struct BinGeom {
   int grid[3];
   int bin[3];
-  double halo_frac[3];  // halo / perpendicular width
+  double halo_frac[3];      // halo / perpendicular width
+  double width_over_rc[3];  // perpendicular width / r_cut: fractional distance -> distance in units of r_c
 };
 
-// flag: 0 outside, 1 halo, 2 root (owned)
-__global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom b, int32_t* __restrict__ ext,
-                             int32_t* __restrict__ owned) {
+// Depth class of every atom for one bin: 0 = root (owned), k >= 1 = halo atom whose largest per-axis periodic distance
+// to the bin lies in ((k-1) r_c, k r_c] (clamped to n_cls-1), -1 = outside the extended set. The flag is written into
+// the class-major array ext[class * N + i], so that ONE exclusive scan over n_cls * N entries numbers the extended atoms
+// by (class, cell order). The 1e-9 slack only ever moves an atom to a LOWER class (more work, never a missing term).
+__global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom b, int n_cls, int32_t* __restrict__ ext,
+                             int32_t* __restrict__ cls) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   bool own = true, in_ext = true;
+  int depth = 0;
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     const double f = frac[3 * i + k];
@@ -32,25 +37,28 @@ __global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom
       dist = below < above ? below : above;
     }
     in_ext = in_ext && (dist <= b.halo_frac[k]);
+    const int dk = (int)ceil(dist * b.width_over_rc[k] - 1e-9);
+    depth = dk > depth ? dk : depth;
   }
-  in_ext = in_ext || own;
-  ext[i] = in_ext ? 1 : 0;
-  owned[i] = own ? 1 : 0;
+  int c = -1;
+  if (own) c = 0;
+  else if (in_ext) c = depth < 1 ? 1 : (depth > n_cls - 1 ? n_cls - 1 : depth);
+  cls[i] = c;
+  if (c >= 0) ext[(int64_t)c * N + i] = 1;
 }
 
-__global__ void k_part_compact(int64_t N, const int32_t* __restrict__ ext, const int32_t* __restrict__ owned,
-                               const int32_t* __restrict__ scan, const int32_t* __restrict__ species,
-                               int32_t* __restrict__ lid, int32_t* __restrict__ gid, float* __restrict__ omega,
-                               int32_t* __restrict__ species_l, unsigned long long* __restrict__ n_owned) {
+__global__ void k_part_compact(int64_t N, const int32_t* __restrict__ cls, const int32_t* __restrict__ scan,
+                               const int32_t* __restrict__ species, int32_t* __restrict__ lid,
+                               int32_t* __restrict__ gid, float* __restrict__ omega, int32_t* __restrict__ species_l) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  if (ext[i]) {
-    const int l = scan[i];
+  const int c = cls[i];
+  if (c >= 0) {
+    const int l = scan[(int64_t)c * N + i];
     lid[i] = l;
     gid[l] = (int32_t)i;
-    omega[l] = owned[i] ? 1.0f : 0.0f;
+    omega[l] = c == 0 ? 1.0f : 0.0f;
     species_l[l] = species[i];
-    if (owned[i]) atomicAdd(n_owned, 1ull);
   } else {
     lid[i] = -1;
   }
@@ -138,32 +146,44 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
   auto fail = [&](int code) { mlip_part_destroy(P); return code; };
   ProfScope prof(ctx, MLIP_PROF_PARTITION);
 #define P_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
-  int32_t *ext = nullptr, *owned = nullptr, *scan = nullptr, *lid = nullptr, *deg = nullptr, *geid = nullptr;
-  unsigned long long* n_owned_d = nullptr;
+  // depth classes 0 .. n_cls-1 (see SubGraph): the halo spans ceil(halo / r_c) shells of thickness r_c
+  int n_cls = 1 + (int)ceil(halo / G->r_cut - 1e-9);
+  if (n_cls < 2) n_cls = 2;
+  if (n_cls > MLIP_MAX_CLS) n_cls = MLIP_MAX_CLS;
+  const int64_t CN = (int64_t)n_cls * N;
+  if (CN >= (int64_t)1 << 31) { ctx->set_error("partition: n_cls * N >= 2^31"); return fail(MLIP_ERR_OVERFLOW); }
+  int32_t *ext = nullptr, *cls = nullptr, *scan = nullptr, *lid = nullptr, *deg = nullptr, *geid = nullptr;
   int* err_flag = nullptr;
-  P_TRY(ctx->alloc(&ext, N + 1)); P_TRY(ctx->alloc(&owned, N + 1)); P_TRY(ctx->alloc(&scan, N + 1));
-  P_TRY(ctx->alloc(&lid, N + 1)); P_TRY(ctx->alloc(&n_owned_d, 1)); P_TRY(ctx->alloc(&err_flag, 1));
+  P_TRY(ctx->alloc(&ext, CN + 1)); P_TRY(ctx->alloc(&cls, N + 1)); P_TRY(ctx->alloc(&scan, CN + 1));
+  P_TRY(ctx->alloc(&lid, N + 1)); P_TRY(ctx->alloc(&err_flag, 1));
   cudaMemsetAsync(err_flag, 0, sizeof(int), st);
   for (int bx = 0; bx < grid[0]; ++bx)
     for (int by = 0; by < grid[1]; ++by)
       for (int bz = 0; bz < grid[2]; ++bz) {
         BinGeom b;
         b.bin[0] = bx; b.bin[1] = by; b.bin[2] = bz;
-        for (int k = 0; k < 3; ++k) { b.grid[k] = grid[k]; b.halo_frac[k] = halo / G->width[k]; }
+        for (int k = 0; k < 3; ++k) {
+          b.grid[k] = grid[k]; b.halo_frac[k] = halo / G->width[k]; b.width_over_rc[k] = G->width[k] / G->r_cut;
+        }
         P->subs.emplace_back();
         PartSub& S = P->subs.back();
         int64_t n_ext = 0, E = 0;
-        cudaMemsetAsync(n_owned_d, 0, sizeof(unsigned long long), st);
+        int32_t cls_start[MLIP_MAX_CLS + 1] = {0}, E_at[MLIP_MAX_CLS] = {0};
+        cudaMemsetAsync(ext, 0, sizeof(int32_t) * (CN + 1), st);
         if (N > 0) {
-          k_part_flags<<<nblk(N, 256), 256, 0, st>>>(N, G->frac, b, ext, owned);
+          k_part_flags<<<nblk(N, 256), 256, 0, st>>>(N, G->frac, b, n_cls, ext, cls);
           ctx->launches++;
         }
-        P_TRY(mlip_exclusive_scan_i32(ctx, ext, scan, N, &n_ext));
+        P_TRY(mlip_exclusive_scan_i32(ctx, ext, scan, CN, nullptr));
+        // first local id of every class (scan[c * N]) and the total (scan[n_cls * N])
+        for (int c = 0; c <= n_cls && N > 0; ++c)
+          cudaMemcpyAsync(&cls_start[c], scan + (int64_t)c * N, sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) { ctx->set_error("partition: scan failed"); return fail(MLIP_ERR_CUDA); }
+        n_ext = N > 0 ? cls_start[n_cls] : 0;
         P_TRY(ctx->alloc(&S.gid, n_ext)); P_TRY(ctx->alloc(&S.omega, n_ext)); P_TRY(ctx->alloc(&S.species, n_ext));
         P_TRY(ctx->alloc(&S.rowptr, n_ext + 1)); P_TRY(ctx->alloc(&deg, n_ext + 1));
         if (N > 0) {
-          k_part_compact<<<nblk(N, 256), 256, 0, st>>>(N, ext, owned, scan, G->species, lid, S.gid, S.omega,
-                                                       S.species, n_owned_d);
+          k_part_compact<<<nblk(N, 256), 256, 0, st>>>(N, cls, scan, G->species, lid, S.gid, S.omega, S.species);
           ctx->launches++;
         }
         if (n_ext > 0) {
@@ -171,10 +191,12 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
                                                                      deg, nullptr, nullptr, nullptr, nullptr, nullptr);
           ctx->launches++;
         }
-        P_TRY(mlip_exclusive_scan_i32(ctx, deg, S.rowptr, n_ext, &E));
-        unsigned long long n_owned_h = 0;
-        cudaMemcpyAsync(&n_owned_h, n_owned_d, sizeof(n_owned_h), cudaMemcpyDeviceToHost, st);
-        cudaStreamSynchronize(st);
+        P_TRY(mlip_exclusive_scan_i32(ctx, deg, S.rowptr, n_ext, nullptr));
+        // E_le[c] = rowptr[n_le[c]], n_le[c] = first local id of class c+1
+        for (int c = 0; c < n_cls; ++c)
+          cudaMemcpyAsync(&E_at[c], S.rowptr + (N > 0 ? cls_start[c + 1] : 0), sizeof(int32_t), cudaMemcpyDeviceToHost, st);
+        if (cudaStreamSynchronize(st) != cudaSuccess) { ctx->set_error("partition: scan failed"); return fail(MLIP_ERR_CUDA); }
+        E = E_at[n_cls - 1];
         P_TRY(ctx->alloc(&S.recv, E)); P_TRY(ctx->alloc(&S.send, E)); P_TRY(ctx->alloc(&S.rev, E));
         P_TRY(ctx->alloc(&S.rvec, E)); P_TRY(ctx->alloc(&geid, E));
         if (E > 0) {
@@ -185,14 +207,16 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
         }
         ctx->free(deg); deg = nullptr;
         ctx->free(geid); geid = nullptr;
-        S.g.n = n_ext; S.g.n_owned = (int64_t)n_owned_h; S.g.E = E;
+        S.g.n = n_ext; S.g.n_owned = N > 0 ? cls_start[1] : 0; S.g.E = E;
+        S.g.n_cls = n_cls;
+        for (int c = 0; c < n_cls; ++c) { S.g.n_le[c] = N > 0 ? cls_start[c + 1] : 0; S.g.E_le[c] = E_at[c]; }
         S.g.gid = S.gid; S.g.omega = S.omega; S.g.species = S.species; S.g.rowptr = S.rowptr;
         S.g.recv = S.recv; S.g.send = S.send; S.g.rev = S.rev; S.g.rvec = S.rvec;
       }
   int err_h = 0;
   cudaMemcpyAsync(&err_h, err_flag, sizeof(int), cudaMemcpyDeviceToHost, st);
   cudaError_t e = cudaStreamSynchronize(st);
-  ctx->free(ext); ctx->free(owned); ctx->free(scan); ctx->free(lid); ctx->free(n_owned_d); ctx->free(err_flag);
+  ctx->free(ext); ctx->free(cls); ctx->free(scan); ctx->free(lid); ctx->free(err_flag);
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) {
     ctx->set_error(std::string("partition: ") + cudaGetErrorString(e));
     return fail(MLIP_ERR_CUDA);
@@ -224,5 +248,16 @@ extern "C" int mlip_part_info(const mlip_part* p, int s, int64_t* n_owned, int64
   if (n_owned) *n_owned = p->subs[s].g.n_owned;
   if (n_ext) *n_ext = p->subs[s].g.n;
   if (n_edges) *n_edges = p->subs[s].g.E;
+  return MLIP_OK;
+}
+
+extern "C" int mlip_part_layer_info(const mlip_part* p, int s, int L, int l, int64_t* n_recv, int64_t* n_send,
+                                    int64_t* n_edges) {
+  if (!p || s < 0 || s >= (int)p->subs.size() || L < 1 || l < 0 || l >= L) return MLIP_ERR_INVALID_ARG;
+  const SubGraph& g = p->subs[s].g;
+  const bool act = p->ctx->active_sets;
+  if (n_recv) *n_recv = act ? g.atoms_upto(L - 1 - l) : g.n;
+  if (n_send) *n_send = act ? g.atoms_upto(L - l) : g.n;
+  if (n_edges) *n_edges = act ? g.edges_upto(L - 1 - l) : g.E;
   return MLIP_OK;
 }

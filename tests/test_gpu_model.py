@@ -172,3 +172,79 @@ def test_bf16_rejects_d64():
     with pytest.raises(mlip.MlipError) as ei:
         mlip.energy_forces(ctx, model, cfg.L, g, None, 1)
     assert ei.value.code == -2
+
+
+# ---------------------------------------------------------------- per-layer active sets
+def _run_part(spec, blob, system, L, precision, grid, halo, active=True, n_sub=None):
+    mlip, ctx, model = gpu_setup(spec, blob)
+    ctx.set_active_sets(active)
+    g = gpu_graph(mlip, ctx, system, spec.r_cut)
+    part = mlip.Partition(ctx, g, halo, n_sub=n_sub) if n_sub else mlip.Partition(ctx, g, halo, grid=grid)
+    return gpu_energy_forces(mlip, ctx, model, L, g, part, precision), part.layer_info(L), part.info()
+
+
+def test_active_set_sizes_match_oracle_classes():
+    """mlip_part_layer_info against the oracle's depth classes: layer l runs on receivers of class
+    <= L-1-l, senders of class <= L-l, and the induced edges whose receiver is in the first set."""
+    import paper_2509_21694_b200 as mlip
+    ctx = mlip.Context(0)
+    r_cut, L = 3.0, 3
+    s = small_system(12, 0.08, seed=17)   # 43.2 A box
+    g = gpu_graph(mlip, ctx, s, r_cut)
+    graph = O.neighbor_list(s.pos, s.cell, r_cut)
+    for grid, halo in [((4, 1, 1), 9.0), ((2, 2, 1), 9.0), ((1, 3, 1), 7.5), ((2, 1, 1), 12.0)]:
+        part = mlip.Partition(ctx, g, halo, grid=grid)
+        info = part.layer_info(L)
+        parts = O.partition_grid(s.pos, s.cell, grid, halo)
+        classes = O.halo_depth_classes(s.pos, s.cell, grid, halo, r_cut)
+        for rows, (owned, ext), cls in zip(info, parts, classes):
+            lr, ls, _ = O.induced_subgraph(graph, ext, len(s.pos))
+            top = cls.max()
+            for l, row in enumerate(rows):
+                cr, cs = min(L - 1 - l, top), min(L - l, top)
+                assert row["n_recv"] == int((cls <= cr).sum())
+                assert row["n_send"] == int((cls <= cs).sum())
+                assert row["n_edges"] == int((cls[lr] <= cr).sum())
+            assert rows[L - 1]["n_recv"] == len(owned)
+        ctx.set_active_sets(False)
+        off = part.layer_info(L)
+        ctx.set_active_sets(True)
+        for rows, (owned, ext) in zip(off, parts):
+            assert all(r["n_recv"] == len(ext) and r["n_send"] == len(ext) for r in rows)
+
+
+@pytest.mark.parametrize("grid,n_sub,L,halo", [((4, 1, 1), None, 3, 9.0), ((2, 2, 2), None, 2, 6.0),
+                                                 (None, 3, 3, 9.0), ((3, 1, 1), None, 1, 9.0),
+                                                 ((2, 1, 1), None, 3, 10.5)])
+def test_fp32_active_sets_equal_full_subgraphs_and_oracle(grid, n_sub, L, halo):
+    """Skipping the layers' inactive atoms changes nothing: equal to evaluating every layer on the whole
+    extended sub-graph (the skipped adjoints are exact zeros), to the unpartitioned GPU result within
+    1e-5 RMS(F), and to the oracle's unpartitioned definition within the fp32 tolerances."""
+    spec = ModelSpec(4, 64, 8, 3, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 15)
+    s = small_system(12, 0.08, seed=41)   # 43.2 A box, 6912 atoms
+    ref = O.energy_forces(oracle_model(spec, blob), L, s.pos, s.cell, s.species)
+    E0, F0, Ei0 = _run(spec, blob, s, L)
+    (E, F, Ei), layers, info = _run_part(spec, blob, s, L, 0, grid, halo, active=True, n_sub=n_sub)
+    (Ef, Ff, Eif), layers_off, _ = _run_part(spec, blob, s, L, 0, grid, halo, active=False, n_sub=n_sub)
+    assert sum(r["n_edges"] for rows in layers for r in rows) < sum(r["n_edges"] for rows in layers_off for r in rows)
+    assert E == Ef and np.array_equal(Ei, Eif)
+    assert np.abs(F - Ff).max() <= 1e-6 * rms(F0)
+    assert np.abs(F - F0).max() <= 1e-5 * rms(F0)
+    assert abs(E - E0) <= 1e-5 * np.abs(Ei0).sum()
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+
+
+def test_bf16_active_sets_match_oracle():
+    spec = ModelSpec(4, 256, 16, 3, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 16)
+    s = small_system(12, 0.08, seed=42)
+    ref = O.energy_forces(oracle_model(spec, blob), 3, s.pos, s.cell, s.species)
+    for grid in [(4, 1, 1), (2, 2, 1)]:
+        (E, F, Ei), layers, info = _run_part(spec, blob, s, 3, 1, grid, 9.0, active=True)
+        (Ef, Ff, Eif), _, _ = _run_part(spec, blob, s, 3, 1, grid, 9.0, active=False)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        assert err["rms_F"] <= BF16_RMS_F
+        # same tiles of the same edge prefix, exact zeros skipped: the two evaluations agree far below bf16 accuracy
+        assert rms(F - Ff) <= 1e-3 * rms(Ff)

@@ -263,3 +263,56 @@ def test_nve_energy_error_is_second_order():
     e2 = O.nve_velocity_verlet(m, 2, s.pos, s.cell, s.species, masses, vel, 2.0, 40)
     f1 = np.abs(e1 - e1[0]).max(); f2 = np.abs(e2 - e2[0]).max()
     assert f1 > 0 and 2.5 < f1 / f2 < 6.0
+
+
+# ---------------------------------------------------------------- per-layer active sets
+@pytest.mark.parametrize("grid,L", [((4, 1, 1), 3), ((2, 2, 1), 2), ((1, 1, 3), 2)])
+def test_depth_class_never_exceeds_khop_distance(grid, L):
+    """The geometric depth class must be a LOWER bound of the breadth-first hop distance to the root
+    atoms (PAPER.md:165 Stage 2), otherwise an atom a root energy depends on through layer l could
+    be left out of that layer's active set. Pinned against a plain BFS over the radius graph."""
+    r_cut = 3.0
+    s = small_system(12 if max(grid) == 4 else 8, 0.08, seed=17)   # 43.2 / 28.8 A box
+    g = O.neighbor_list(s.pos, s.cell, r_cut)
+    halo = L * r_cut
+    parts = O.partition_grid(s.pos, s.cell, grid, halo)
+    classes = O.halo_depth_classes(s.pos, s.cell, grid, halo, r_cut)
+    some_halo_shell_is_populated = False
+    for (owned, ext), cls in zip(parts, classes):
+        hops = O.khop_distance(g, owned, len(s.pos), L + 2)[ext]
+        assert np.array_equal(cls == 0, np.isin(ext, owned))
+        assert np.all(cls <= hops)                    # class k  =>  at least k hops away
+        assert cls.max() <= L
+        # every edge changes the class by at most one (what makes the per-layer sets prefixes)
+        lr, ls, _ = O.induced_subgraph(g, ext, len(s.pos))
+        assert np.all(np.abs(cls[lr] - cls[ls]) <= 1)
+        some_halo_shell_is_populated |= bool(np.any(cls == L))
+        # the K-hop set of the paper is inside the geometric halo (reading R2)
+        assert np.all(np.isin(np.nonzero(O.khop_distance(g, owned, len(s.pos), L) <= L)[0], ext))
+    assert some_halo_shell_is_populated
+
+
+def test_outermost_shell_never_receives():
+    """With halo = L r_cut the atoms of class L only ever act as senders of layer 0: deleting every edge
+    they RECEIVE leaves the root energies and the gradient of their sum unchanged (to rounding), while
+    deleting the edges they SEND does not."""
+    spec, blob, m = make_model(r_cut=3.7, nbar=18.0)   # second fcc shell (a = 3.6) is inside: a hop spans ~r_cut
+    L = 2
+    s = small_system(8, 0.08, seed=23)
+    g = O.neighbor_list(s.pos, s.cell, spec.r_cut)
+    grid = (3, 1, 1)
+    parts = O.partition_grid(s.pos, s.cell, grid, L * spec.r_cut)
+    classes = O.halo_depth_classes(s.pos, s.cell, grid, L * spec.r_cut, spec.r_cut)
+    owned, ext = parts[1]
+    cls = classes[1]
+    lr, ls, lsh = O.induced_subgraph(g, ext, len(s.pos))
+    om = (cls == 0).astype(float)
+    E0, Ei0, F0 = O.energy_forces(m, L, s.pos[ext], s.cell, s.species[ext], (lr, ls, lsh), om)
+    keep = cls[lr] < L
+    assert 0 < keep.sum() < len(lr)
+    E1, Ei1, F1 = O.energy_forces(m, L, s.pos[ext], s.cell, s.species[ext], (lr[keep], ls[keep], lsh[keep]), om)
+    assert abs(E1 - E0) <= 1e-12 * np.abs(Ei0[om > 0]).sum()
+    assert np.abs(F1 - F0).max() <= 1e-12 * rms(F0)
+    keep2 = cls[ls] < L
+    E2, _, F2 = O.energy_forces(m, L, s.pos[ext], s.cell, s.species[ext], (lr[keep2], ls[keep2], lsh[keep2]), om)
+    assert np.abs(F2 - F0).max() > 1e-6 * rms(F0)
