@@ -105,8 +105,14 @@ void mlip_graph_destroy(mlip_graph* g);
 
 /* Spatial partition (PAPER.md:157 Stage 1: uniform grid of P bins on the scaled positions;
  * Stage 2: every bin is extended so that each root atom keeps its K-hop
- * neighbourhood -- here by the geometric halo: atoms whose periodic distance to the bin is
- * <= halo along every axis, a superset of the K-hop BFS set when halo >= K*r_c, reading R2).
+ * neighbourhood). K = ceil(halo / r_c). The extended set of a bin is found in two steps:
+ *   (a) the geometric box: atoms whose periodic distance to the bin is <= halo along every axis
+ *       (a superset of the K-hop set when halo >= K*r_c, reading R2);
+ *   (b) by default, a K-level breadth-first search over the radius graph from the root atoms inside
+ *       that box (the paper's own rule): atoms not reached within K hops leave the sub-domain, and
+ *       the hop count of the others is their depth class (see mlip_part_layer_info).
+ * mlip_ctx_set_khop_halo(ctx, 0) keeps the whole box of (a) and uses geometric shells of thickness r_c
+ * as depth classes instead. Results are identical either way; (b) evaluates fewer atoms and edges.
  * mlip_partition cuts n_sub slabs along the axis of largest perpendicular width (R3). */
 int mlip_partition(mlip_ctx* ctx, const mlip_graph* g, int n_sub, double halo, mlip_part** out);
 int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* g, const int grid[3], double halo,
@@ -116,11 +122,13 @@ int mlip_part_count(const mlip_part* p, int* n_sub);
  * growth factor of PAPER.md:289 is (n_ext - n_owned) / n_owned. */
 int mlip_part_info(const mlip_part* p, int s, int64_t* n_owned, int64_t* n_ext, int64_t* n_edges);
 /* Per-layer active sets of sub-domain s when the first L layers are evaluated. The extended atoms of a sub-domain are
- * numbered by depth class (0 = root atoms; k >= 1 = halo atoms whose largest per-axis periodic distance to the bin lies
- * in ((k-1) r_c, k r_c]). An edge is shorter than r_c, so the root energies of PAPER.md:169 and their gradient
- * depend on layer l (0-based) only through receivers of class <= L-1-l and senders of class <= L-l:
- * the K-hop neighbourhood of PAPER.md:165 shrinks by one hop per layer. mlip_energy_forces evaluates exactly those
- * prefixes; the result is identical to evaluating every layer on the whole extended sub-graph.
+ * numbered by depth class: 0 = root atoms; k >= 1 = halo atoms k hops away from the nearest root atom (K-hop search,
+ * default) or, with the geometric halo, atoms whose largest per-axis periodic distance to the bin lies in
+ * ((k-1) r_c, k r_c] -- a lower bound of the hop count because an edge is shorter than r_c. The root energies of
+ * PAPER.md:169 and their gradient depend on layer l (0-based) only through receivers of class <= L-1-l
+ * and senders of class <= L-l: the K-hop neighbourhood of PAPER.md:165 shrinks by one hop per layer.
+ * mlip_energy_forces evaluates exactly those prefixes; the result is identical to evaluating every layer on the whole
+ * extended sub-graph.
  *   n_recv  atoms whose h^{l+1} is computed, n_send atoms whose h^l is read, n_edges edges evaluated by layer l
  * (with active sets switched off through mlip_ctx_set_active_sets: n_ext, n_ext, all induced edges). */
 int mlip_part_layer_info(const mlip_part* p, int s, int L, int l, int64_t* n_recv, int64_t* n_send,
@@ -163,6 +171,9 @@ int mlip_step_host(mlip_ctx* ctx, const mlip_model* m, int L, const double* pos_
 /* Per-layer active sets inside sub-domains (see mlip_part_layer_info): on by default; enable = 0 makes every layer run
  * on the whole extended sub-graph (same results; kept for A/B measurement and as a test control). */
 int mlip_ctx_set_active_sets(mlip_ctx* ctx, int enable);
+/* Halo rule used by the NEXT mlip_partition* calls of this context: 1 (default) = K-hop breadth-first search inside the
+ * geometric box, 0 = the whole geometric box (see mlip_partition). */
+int mlip_ctx_set_khop_halo(mlip_ctx* ctx, int enable);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);

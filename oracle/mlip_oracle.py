@@ -421,6 +421,29 @@ def khop_distance(graph, owned_idx, n_atoms, max_hops):
     return hops
 
 
+def partition_grid_khop(pos, cell, grid, halo, r_cut, graph=None):
+    """Stage 2 as the paper states it: the extended set of a bin is the K-hop
+    neighbourhood of its root atoms, K = ceil(halo / r_cut), found by breadth-first search over the
+    radius graph -- searched inside the geometric box of partition_grid (which contains every atom
+    within K hops whenever halo >= K r_cut, so the restriction then changes nothing).
+    Returns a list of (owned_idx, ext_idx, hops) with hops aligned with ext_idx (0 for root atoms)."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    N = len(pos)
+    if graph is None:
+        graph = neighbor_list(pos, cell, r_cut)
+    recv, send, shift = graph
+    K = max(1, int(np.ceil(halo / r_cut - 1e-9)))
+    out = []
+    for owned, box in partition_grid(pos, cell, grid, halo):
+        inside = np.zeros(N, bool)
+        inside[box] = True
+        keep = inside[recv] & inside[send]
+        hops = khop_distance((recv[keep], send[keep], shift[keep]), owned, N, K)
+        ext = np.nonzero(inside & (hops <= K))[0]
+        out.append((owned, ext, hops[ext]))
+    return out
+
+
 def halo_depth_classes(pos, cell, grid, halo, r_cut):
     """Depth class of every atom of every extended set (same bins, same order as partition_grid):
     0 for root atoms, else ceil(D / r_cut) clipped to [1, ceil(halo / r_cut)], D = the largest per-axis

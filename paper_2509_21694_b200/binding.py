@@ -65,6 +65,7 @@ def load_library():
     lib.mlip_part_layer_info.argtypes = [vp, i32, i32, i32, P(i64), P(i64), P(i64)]
     lib.mlip_part_destroy.argtypes = [vp]; lib.mlip_part_destroy.restype = None
     lib.mlip_ctx_set_active_sets.argtypes = [vp, i32]
+    lib.mlip_ctx_set_khop_halo.argtypes = [vp, i32]
     lib.mlip_energy_forces.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
     lib.mlip_energy_forces_shard.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.mlip_step_host.argtypes = [vp, vp, i32, vp, vp, vp, i64, P(i32), dbl, i32, vp, vp]
@@ -117,6 +118,10 @@ class Context:
     def set_active_sets(self, enable: bool):
         """mlip_ctx_set_active_sets: per-layer active sets inside sub-domains (on by default)."""
         self.check(self.lib.mlip_ctx_set_active_sets(self.h, 1 if enable else 0))
+
+    def set_khop_halo(self, enable: bool):
+        """mlip_ctx_set_khop_halo: K-hop search (default) or whole geometric box for the next partitions."""
+        self.check(self.lib.mlip_ctx_set_khop_halo(self.h, 1 if enable else 0))
 
     def profile(self, enable: bool):
         """mlip_ctx_profile: start (clearing the counters) or stop per-kernel-group event timing."""

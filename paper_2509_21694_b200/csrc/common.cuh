@@ -43,6 +43,7 @@ struct mlip_ctx {
   std::string err;
   int64_t launches = 0;
   bool active_sets = true;  // per-layer active sets inside sub-domains (mlip_ctx_set_active_sets)
+  bool khop_halo = true;    // halo and depth classes by K-hop search instead of geometry (mlip_ctx_set_khop_halo)
   void set_error(const std::string& s) { err = s; }
   // ---- optional per-group timing ----
   struct ProfRec { int cat; int64_t launches; cudaEvent_t a, b; };
@@ -142,10 +143,11 @@ struct SubGraph {
   const int32_t* rev = nullptr;      // [E] index of the reverse edge
   const float4* rvec = nullptr;      // [E] (r_x, r_y, r_z, |r|), float32 rounded from float64
   // Depth classes (sub-domains only; n_cls == 0 means "no classes, every layer runs on all atoms"). Atoms are numbered
-  // by (class, cell order): class 0 = root atoms, class k >= 1 = halo atoms whose largest per-axis periodic distance to
-  // the bin lies in ((k-1) r_c, k r_c]. An edge is shorter than r_c, so an atom of class k only has neighbours of class
-  // >= k-1, and the root energies (and their gradient) need layer l only on receivers of class <= L-1-l with senders of
-  // class <= L-l (each root atom keeps its K-hop neighbourhood). Both sets are prefixes of the numbering.
+  // by (class, cell order): class 0 = root atoms, class k >= 1 = halo atoms k hops from the nearest root atom (K-hop
+  // search) or, geometric variant, whose largest per-axis periodic distance to the bin lies in ((k-1) r_c, k r_c]. Either
+  // way an atom of class k only has neighbours of class >= k-1, so the root energies (and their gradient) need layer l
+  // only on receivers of class <= L-1-l with senders of class <= L-l (each root atom keeps its K-hop
+  // neighbourhood). Both sets are prefixes of the numbering.
   int n_cls = 0;
   int64_t n_le[MLIP_MAX_CLS] = {};   // atoms of class <= c
   int64_t E_le[MLIP_MAX_CLS] = {};   // edges whose receiver has class <= c  (= rowptr[n_le[c]])
@@ -188,6 +190,7 @@ struct mlip_part {
   mlip_ctx* ctx;
   int grid[3];
   double halo = 0;
+  bool khop = false;  // classes are hop counts (K-hop search) rather than geometric shells
   int64_t N = 0;
   std::vector<PartSub> subs;
 };

@@ -95,6 +95,11 @@ extern "C" int mlip_ctx_profile_read(mlip_ctx* ctx, int group, double* ms_total,
 }
 extern "C" const char* mlip_last_error(const mlip_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
 extern "C" int64_t mlip_ctx_launch_count(const mlip_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" int mlip_ctx_set_khop_halo(mlip_ctx* ctx, int enable) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  ctx->khop_halo = enable != 0;
+  return MLIP_OK;
+}
 extern "C" int mlip_ctx_set_active_sets(mlip_ctx* ctx, int enable) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
   ctx->active_sets = enable != 0;

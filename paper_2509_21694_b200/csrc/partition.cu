@@ -13,11 +13,12 @@ struct BinGeom {
   double width_over_rc[3];  // perpendicular width / r_cut: fractional distance -> distance in units of r_c
 };
 
-// Depth class of every atom for one bin: 0 = root (owned), k >= 1 = halo atom whose largest per-axis periodic distance
-// to the bin lies in ((k-1) r_c, k r_c] (clamped to n_cls-1), -1 = outside the extended set. The flag is written into
-// the class-major array ext[class * N + i], so that ONE exclusive scan over n_cls * N entries numbers the extended atoms
-// by (class, cell order). The 1e-9 slack only ever moves an atom to a LOWER class (more work, never a missing term).
-__global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom b, int n_cls, int32_t* __restrict__ ext,
+// Depth class of every atom for one bin. Geometric rule: 0 = root (owned), k >= 1 = halo atom whose largest per-axis
+// periodic distance to the bin lies in ((k-1) r_c, k r_c] (clamped to n_cls-1), -1 = outside the extended box. The 1e-9
+// slack only ever moves an atom to a LOWER class (more work, never a missing term). With bfs != 0 the halo atoms are
+// only marked CLS_UNSET here and get their class from the breadth-first search below.
+constexpr int CLS_UNSET = 1 << 20;
+__global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom b, int n_cls, int bfs,
                              int32_t* __restrict__ cls) {
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
@@ -42,8 +43,28 @@ __global__ void k_part_flags(int64_t N, const double* __restrict__ frac, BinGeom
   }
   int c = -1;
   if (own) c = 0;
-  else if (in_ext) c = depth < 1 ? 1 : (depth > n_cls - 1 ? n_cls - 1 : depth);
+  else if (in_ext) c = bfs ? CLS_UNSET : (depth < 1 ? 1 : (depth > n_cls - 1 ? n_cls - 1 : depth));
   cls[i] = c;
+}
+
+// One level of the K-hop search of PAPER.md:165 (Stage 2), pull form: an unreached atom of the extended box takes
+// class k if one of its neighbours has class k-1. The radius graph is symmetric, so the senders of the in-edges of i
+// are its neighbours. Writes (k) never collide with the value tested (k-1): in place, no atomics, deterministic.
+__global__ void __launch_bounds__(256) k_part_bfs(int64_t N, int k, const int32_t* __restrict__ rowptr,
+                                                  const int32_t* __restrict__ send, int32_t* __restrict__ cls) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N || cls[i] != CLS_UNSET) return;
+  for (int e = rowptr[i]; e < rowptr[i + 1]; ++e)
+    if (cls[send[e]] == k - 1) { cls[i] = k; return; }
+}
+
+// flag of atom i in the class-major array ext[class * N + i], so that ONE exclusive scan over n_cls * N entries numbers
+// the extended atoms by (class, cell order); atoms the search did not reach within n_cls-1 hops leave the sub-domain
+__global__ void k_part_mark(int64_t N, int n_cls, int32_t* __restrict__ cls, int32_t* __restrict__ ext) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  int c = cls[i];
+  if (c >= n_cls) { c = -1; cls[i] = -1; }
   if (c >= 0) ext[(int64_t)c * N + i] = 1;
 }
 
@@ -150,6 +171,8 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
   int n_cls = 1 + (int)ceil(halo / G->r_cut - 1e-9);
   if (n_cls < 2) n_cls = 2;
   if (n_cls > MLIP_MAX_CLS) n_cls = MLIP_MAX_CLS;
+  const bool bfs = ctx->khop_halo;
+  P->khop = bfs;
   const int64_t CN = (int64_t)n_cls * N;
   if (CN >= (int64_t)1 << 31) { ctx->set_error("partition: n_cls * N >= 2^31"); return fail(MLIP_ERR_OVERFLOW); }
   int32_t *ext = nullptr, *cls = nullptr, *scan = nullptr, *lid = nullptr, *deg = nullptr, *geid = nullptr;
@@ -171,7 +194,13 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
         int32_t cls_start[MLIP_MAX_CLS + 1] = {0}, E_at[MLIP_MAX_CLS] = {0};
         cudaMemsetAsync(ext, 0, sizeof(int32_t) * (CN + 1), st);
         if (N > 0) {
-          k_part_flags<<<nblk(N, 256), 256, 0, st>>>(N, G->frac, b, n_cls, ext, cls);
+          k_part_flags<<<nblk(N, 256), 256, 0, st>>>(N, G->frac, b, n_cls, bfs ? 1 : 0, cls);
+          ctx->launches++;
+          for (int k = 1; bfs && k < n_cls; ++k) {
+            k_part_bfs<<<nblk(N, 256), 256, 0, st>>>(N, k, G->rowptr, G->send, cls);
+            ctx->launches++;
+          }
+          k_part_mark<<<nblk(N, 256), 256, 0, st>>>(N, n_cls, cls, ext);
           ctx->launches++;
         }
         P_TRY(mlip_exclusive_scan_i32(ctx, ext, scan, CN, nullptr));

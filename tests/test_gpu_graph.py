@@ -68,14 +68,25 @@ def test_partition_sizes_match_oracle():
     mlip, ctx = _ctx()
     s = small_system(10, 0.1, seed=4)  # 36 A box, 4000 atoms
     g = gpu_graph(mlip, ctx, s, 5.0)
+    graph = O.neighbor_list(s.pos, s.cell, 5.0)
+    # geometric halo (reading R2): the whole box of atoms within `halo` of the bin along every axis
+    ctx.set_khop_halo(False)
     for grid, halo in [((3, 1, 1), 5.0), ((2, 2, 1), 4.0), ((1, 1, 4), 2.0)]:
         part = mlip.Partition(ctx, g, halo, grid=grid)
         info = part.info()
         oparts = O.partition_grid(s.pos, s.cell, grid, halo)
-        graph = O.neighbor_list(s.pos, s.cell, 5.0)
         assert sum(i["n_owned"] for i in info) == len(s.pos)
         for i, (owned, ext) in zip(info, oparts):
             assert i["n_owned"] == len(owned) and i["n_ext"] == len(ext)
             assert i["n_edges"] == len(O.induced_subgraph(graph, ext, len(s.pos))[0])
     slab = mlip.Partition(ctx, g, 5.0, n_sub=3).info()
     assert [i["n_owned"] for i in slab] == [len(p[0]) for p in O.partition_slabs(s.pos, s.cell, 3, 5.0)]
+    # K-hop halo (the default): breadth-first search from the root atoms inside that box
+    ctx.set_khop_halo(True)
+    for grid, halo in [((3, 1, 1), 5.0), ((2, 2, 1), 4.0), ((1, 1, 4), 2.0), ((2, 1, 1), 10.0), ((1, 2, 1), 9.0)]:
+        info = mlip.Partition(ctx, g, halo, grid=grid).info()
+        oparts = O.partition_grid_khop(s.pos, s.cell, grid, halo, 5.0, graph)
+        assert sum(i["n_owned"] for i in info) == len(s.pos)
+        for i, (owned, ext, hops) in zip(info, oparts):
+            assert i["n_owned"] == len(owned) and i["n_ext"] == len(ext)
+            assert i["n_edges"] == len(O.induced_subgraph(graph, ext, len(s.pos))[0])

@@ -175,19 +175,23 @@ def test_bf16_rejects_d64():
 
 
 # ---------------------------------------------------------------- per-layer active sets
-def _run_part(spec, blob, system, L, precision, grid, halo, active=True, n_sub=None):
+def _run_part(spec, blob, system, L, precision, grid, halo, active=True, n_sub=None, khop=True):
     mlip, ctx, model = gpu_setup(spec, blob)
     ctx.set_active_sets(active)
+    ctx.set_khop_halo(khop)
     g = gpu_graph(mlip, ctx, system, spec.r_cut)
     part = mlip.Partition(ctx, g, halo, n_sub=n_sub) if n_sub else mlip.Partition(ctx, g, halo, grid=grid)
     return gpu_energy_forces(mlip, ctx, model, L, g, part, precision), part.layer_info(L), part.info()
 
 
-def test_active_set_sizes_match_oracle_classes():
-    """mlip_part_layer_info against the oracle's depth classes: layer l runs on receivers of class
-    <= L-1-l, senders of class <= L-l, and the induced edges whose receiver is in the first set."""
+@pytest.mark.parametrize("khop", [False, True])
+def test_active_set_sizes_match_oracle_classes(khop):
+    """mlip_part_layer_info against the oracle's depth classes (geometric shells or K-hop counts): layer l
+    runs on receivers of class <= L-1-l, senders of class <= L-l, and the induced edges whose receiver is
+    in the first set."""
     import paper_2509_21694_b200 as mlip
     ctx = mlip.Context(0)
+    ctx.set_khop_halo(khop)
     r_cut, L = 3.0, 3
     s = small_system(12, 0.08, seed=17)   # 43.2 A box
     g = gpu_graph(mlip, ctx, s, r_cut)
@@ -195,11 +199,15 @@ def test_active_set_sizes_match_oracle_classes():
     for grid, halo in [((4, 1, 1), 9.0), ((2, 2, 1), 9.0), ((1, 3, 1), 7.5), ((2, 1, 1), 12.0)]:
         part = mlip.Partition(ctx, g, halo, grid=grid)
         info = part.layer_info(L)
-        parts = O.partition_grid(s.pos, s.cell, grid, halo)
-        classes = O.halo_depth_classes(s.pos, s.cell, grid, halo, r_cut)
+        if khop:
+            both = O.partition_grid_khop(s.pos, s.cell, grid, halo, r_cut, graph)
+            parts, classes = [(o, e) for o, e, _ in both], [h for _, _, h in both]
+        else:
+            parts = O.partition_grid(s.pos, s.cell, grid, halo)
+            classes = O.halo_depth_classes(s.pos, s.cell, grid, halo, r_cut)
         for rows, (owned, ext), cls in zip(info, parts, classes):
             lr, ls, _ = O.induced_subgraph(graph, ext, len(s.pos))
-            top = cls.max()
+            top = max(1, int(np.ceil(halo / r_cut - 1e-9)))
             for l, row in enumerate(rows):
                 cr, cs = min(L - 1 - l, top), min(L - l, top)
                 assert row["n_recv"] == int((cls <= cr).sum())
@@ -227,9 +235,12 @@ def test_fp32_active_sets_equal_full_subgraphs_and_oracle(grid, n_sub, L, halo):
     E0, F0, Ei0 = _run(spec, blob, s, L)
     (E, F, Ei), layers, info = _run_part(spec, blob, s, L, 0, grid, halo, active=True, n_sub=n_sub)
     (Ef, Ff, Eif), layers_off, _ = _run_part(spec, blob, s, L, 0, grid, halo, active=False, n_sub=n_sub)
-    assert sum(r["n_edges"] for rows in layers for r in rows) < sum(r["n_edges"] for rows in layers_off for r in rows)
+    (Eg, Fg, Eig), layers_geo, _ = _run_part(spec, blob, s, L, 0, grid, halo, active=True, n_sub=n_sub, khop=False)
+    n_ev = lambda lay: sum(r["n_edges"] for rows in lay for r in rows)
+    assert n_ev(layers) <= n_ev(layers_geo) < n_ev(layers_off) or L == 1
     assert E == Ef and np.array_equal(Ei, Eif)
     assert np.abs(F - Ff).max() <= 1e-6 * rms(F0)
+    assert abs(Eg - E) <= 1e-6 * np.abs(Ei0).sum() and np.abs(Fg - F).max() <= 1e-5 * rms(F0)
     assert np.abs(F - F0).max() <= 1e-5 * rms(F0)
     assert abs(E - E0) <= 1e-5 * np.abs(Ei0).sum()
     err = errors(E, F, Ei, ref[0], ref[2], ref[1])

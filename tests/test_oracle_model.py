@@ -316,3 +316,27 @@ def test_outermost_shell_never_receives():
     keep2 = cls[ls] < L
     E2, _, F2 = O.energy_forces(m, L, s.pos[ext], s.cell, s.species[ext], (lr[keep2], ls[keep2], lsh[keep2]), om)
     assert np.abs(F2 - F0).max() > 1e-6 * rms(F0)
+
+
+@pytest.mark.parametrize("grid", [(3, 1, 1), (2, 2, 1)])
+def test_khop_partition_equals_unpartitioned(grid):
+    """PAPER.md:165 as stated: extending every bin by the K-hop neighbourhood of its root atoms (K = number
+    of layers kept) reproduces the unpartitioned energies and forces; K-1 hops do not. The K-hop set is
+    a subset of the geometric box and, on this lattice (a hop advances < r_cut along an axis), a proper one."""
+    spec, blob, m = make_model(r_cut=3.0, nbar=12.0)
+    L = 2
+    s = small_system(8, 0.08, seed=29)
+    g = O.neighbor_list(s.pos, s.cell, spec.r_cut)
+    E, E_i, F = O.energy_forces(m, L, s.pos, s.cell, s.species, g)
+    kh = O.partition_grid_khop(s.pos, s.cell, grid, L * spec.r_cut, spec.r_cut, g)
+    geo = O.partition_grid(s.pos, s.cell, grid, L * spec.r_cut)
+    assert all(np.all(np.isin(ext, gext)) for (_, ext, _), (_, gext) in zip(kh, geo))
+    assert sum(len(p[1]) for p in kh) < sum(len(p[1]) for p in geo)
+    assert all(h.max() == L and np.array_equal(h == 0, np.isin(ext, owned)) for owned, ext, h in kh)
+    Ep, Eip, Fp, _ = O.energy_forces_partitioned(m, L, s.pos, s.cell, s.species, [(o, e) for o, e, _ in kh], g)
+    assert abs(Ep - E) < 1e-12 * np.abs(E_i).sum()
+    assert np.allclose(Eip, E_i, rtol=0, atol=1e-12)
+    assert np.abs(Fp - F).max() < 1e-12 * rms(F)
+    bad = [(o, e[h <= L - 1]) for o, e, h in kh]
+    Eb, _, Fb, _ = O.energy_forces_partitioned(m, L, s.pos, s.cell, s.species, bad, g)
+    assert np.abs(Fb - F).max() > 1e-4 * rms(F)
