@@ -160,6 +160,17 @@ int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* m, int L, const ml
                              const mlip_part* part, int shard, int n_shards, int precision,
                              double* energy_dev, float* forces_dev, float* atom_energy_dev);
 
+/* Energy, forces and the stress tensor sigma = (1/V) dE/d(strain) (with energy-gradient forces the
+ * stress decomposes over sub-graphs like the forces do). Every edge vector follows a homogeneous strain as
+ * r_e -> (1 + eps) r_e, so sigma_ab = (1/V) sum over sub-domains and their directed edges of rbar_e r_a r_b / r_e with
+ * rbar_e the adjoint of the root-energy sum w.r.t. the edge length -- the same per-edge scalars the forces are
+ * assembled from. Arguments as mlip_energy_forces_shard (shard = 0, n_shards = 1 for the whole box), plus
+ *   stress_dev [3,3] float64, device, row-major, symmetric, eV/Angstrom^3 (this shard's partial sum). */
+int mlip_energy_forces_stress(mlip_ctx* ctx, const mlip_model* m, int L, const mlip_graph* g,
+                              const mlip_part* part, int shard, int n_shards, int precision,
+                              double* energy_dev, float* forces_dev, float* atom_energy_dev,
+                              double* stress_dev);
+
 /* Whole step from HOST buffers: copies positions/species to the device, builds the graph,
  * partitions (grid = {1,1,1} means one domain), evaluates, copies E and F back and
  * synchronises. This is the call bench.py times for its end-to-end figure. */
@@ -174,6 +185,22 @@ int mlip_ctx_set_active_sets(mlip_ctx* ctx, int enable);
 /* Halo rule used by the NEXT mlip_partition* calls of this context: 1 (default) = K-hop breadth-first search inside the
  * geometric box, 0 = the whole geometric box (see mlip_partition). */
 int mlip_ctx_set_khop_halo(mlip_ctx* ctx, int enable);
+
+/* On-device NVE molecular dynamics (the use the paper builds the partitioned evaluation for):
+ * n_steps of velocity-Verlet -- v += (dt/2) a; x += dt v; rebuild the graph (and the partition when grid != {1,1,1});
+ * E, F; v += (dt/2) a -- with a = 9.648533e-3 F / m. Every step runs on the GPU; the host only sequences launches.
+ *   pos_dev, vel_dev   [n_atoms,3] float64, device, IN/OUT (Angstrom, Angstrom/fs; positions are not wrapped)
+ *   mass_dev           [n_atoms] float64, device (amu);  species_dev [n_atoms] int32, device
+ *   cell_host          [3,3] float64, HOST (fixed cell)
+ *   grid, halo         partition as in mlip_partition_grid ({1,1,1}: one domain)
+ *   dt                 fs
+ *   total_energy_host  [n_steps+1] float64, HOST or NULL: potential + kinetic energy (eV) before every step and after
+ *                      the last one
+ * Synchronises the stream before returning. */
+int mlip_md_nve(mlip_ctx* ctx, const mlip_model* m, int L, double* pos_dev, double* vel_dev,
+                const double* mass_dev, const double* cell_host, const int32_t* species_dev,
+                int64_t n_atoms, const int grid[3], double halo, int precision, double dt, int n_steps,
+                double* total_energy_host);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);

@@ -326,6 +326,24 @@ def energy_forces(model, L, pos, cell, species, graph=None, omega=None, return_e
     return E, E_i, F
 
 
+def stress_from_rbar(cell, rvec, r, rbar):
+    """Stress sigma = (1/V) dE/d(strain) (PAPER.md:173 lists stress beside energy and forces as a model
+    output). Under a homogeneous strain x -> (1 + eps) x, C -> C (1 + eps)^T every edge vector transforms as
+    r_e -> (1 + eps) r_e, so d r_e / d eps_ab = r_a r_b / r and
+        sigma_ab = (1/V) sum_e rbar_e r_ea r_eb / r_e      (sum over DIRECTED edges, rbar_e = dE/dr_e;
+    edges with r = 0 contribute nothing, reading R13). Symmetric by construction; eV / A^3."""
+    V = abs(np.linalg.det(np.asarray(cell, np.float64)))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        w = np.where(r > 0.0, rbar / r, 0.0)
+    return np.einsum("e,ea,eb->ab", w, rvec, rvec) / V
+
+
+def energy_forces_stress(model, L, pos, cell, species, graph=None, omega=None):
+    """E, E_i, F and the stress tensor [3,3] of the unpartitioned model."""
+    E, E_i, F, ex = energy_forces(model, L, pos, cell, species, graph, omega, return_extra=True)
+    return E, E_i, F, stress_from_rbar(cell, ex["rvec"], ex["r"], ex["rbar"])
+
+
 # --------------------------------------------------------------------------------------
 # O6 partitioned evaluation (PAPER.md:157,165,169-171)
 # --------------------------------------------------------------------------------------
@@ -472,6 +490,22 @@ def halo_depth_classes(pos, cell, grid, halo, r_cut):
     return out
 
 
+def stress_partitioned(model, L, pos, cell, species, parts, graph=None):
+    """"a similar decomposition applies" -- the strain derivative is linear in the energy,
+    so sigma = sum_s (1/V) d( sum_{i in own(s)} E_i^(s) ) / d eps, each term over the edges of sub-graph s."""
+    pos = np.asarray(pos, np.float64); cell = np.asarray(cell, np.float64)
+    species = np.asarray(species)
+    N = len(pos)
+    if graph is None:
+        graph = neighbor_list(pos, cell, model.r_cut)
+    sigma = np.zeros((3, 3))
+    for owned, ext in parts:
+        lg = induced_subgraph(graph, ext, N)
+        omega = np.isin(ext, owned).astype(np.float64)
+        sigma += energy_forces_stress(model, L, pos[ext], cell, species[ext], lg, omega)[3]
+    return sigma
+
+
 def halo_growth_factor(parts):
     """H = (# atoms added by the halo) / (# root atoms), PAPER.md:289 (S1)."""
     return [(len(ext) - len(owned)) / max(len(owned), 1) for owned, ext in parts]
@@ -483,8 +517,9 @@ def halo_growth_factor(parts):
 ACC_UNIT = 9.648533e-3  # (eV/A)/amu -> A/fs^2
 
 
-def nve_velocity_verlet(model, L, pos, cell, species, masses, vel, dt, n_steps):
-    """Velocity-Verlet; returns total energy (potential + kinetic, eV) per step."""
+def nve_velocity_verlet(model, L, pos, cell, species, masses, vel, dt, n_steps, return_state=False):
+    """Velocity-Verlet; returns total energy (potential + kinetic, eV) per step
+    (and the final positions and velocities when return_state is set)."""
     pos = np.array(pos, np.float64); vel = np.array(vel, np.float64)
     E, _, F = energy_forces(model, L, pos, cell, species)
     out = []
@@ -497,4 +532,6 @@ def nve_velocity_verlet(model, L, pos, cell, species, masses, vel, dt, n_steps):
         vel += 0.5 * dt * ACC_UNIT * F / masses[:, None]
     kin = 0.5 * np.sum(masses[:, None] * vel * vel) / ACC_UNIT
     out.append(E + kin)
+    if return_state:
+        return np.array(out), pos, vel
     return np.array(out)

@@ -5,4 +5,4 @@ only, every step runs in the library's CUDA kernels. Importing this package does
 library; the first call does, and fails loudly if it is missing or no B200 is present.
 """
 from .binding import (MLIP_BF16, MLIP_FP32, Context, Graph, MlipError, Model, Partition, energy_forces, energy_forces_shard,  # noqa: F401
-                      lib_path, load_library, step_host)
+                      energy_forces_stress, lib_path, load_library, md_nve, step_host)

@@ -68,6 +68,8 @@ def load_library():
     lib.mlip_ctx_set_khop_halo.argtypes = [vp, i32]
     lib.mlip_energy_forces.argtypes = [vp, vp, i32, vp, vp, i32, vp, vp, vp]
     lib.mlip_energy_forces_shard.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp]
+    lib.mlip_energy_forces_stress.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp, vp]
+    lib.mlip_md_nve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i64, P(i32), dbl, i32, dbl, i32, vp]
     lib.mlip_step_host.argtypes = [vp, vp, i32, vp, vp, vp, i64, P(i32), dbl, i32, vp, vp]
     lib.mlip_ctx_launch_count.argtypes = [vp]; lib.mlip_ctx_launch_count.restype = i64
     lib.mlip_ctx_profile.argtypes = [vp, i32]
@@ -276,6 +278,39 @@ def energy_forces_shard(ctx: Context, model: Model, L: int, graph: Graph, part: 
                                                int(precision), C.c_void_p(E.data_ptr()), C.c_void_p(F.data_ptr()),
                                                C.c_void_p(Ei.data_ptr()) if Ei is not None else None))
     return E, F, Ei
+
+
+def energy_forces_stress(ctx: Context, model: Model, L: int, graph: Graph, part: Partition | None = None,
+                         precision: int = MLIP_FP32, shard: int = 0, n_shards: int = 1):
+    """mlip_energy_forces_stress -> (E float64[1], F float32[N,3], E_i float32[N], sigma float64[3,3]), CUDA tensors."""
+    torch = _torch()
+    dev = f"cuda:{ctx.device}"
+    E = torch.empty(1, dtype=torch.float64, device=dev)
+    F = torch.empty((graph.n_atoms, 3), dtype=torch.float32, device=dev)
+    Ei = torch.empty(graph.n_atoms, dtype=torch.float32, device=dev)
+    S = torch.empty((3, 3), dtype=torch.float64, device=dev)
+    ctx.check(ctx.lib.mlip_energy_forces_stress(ctx.h, model.h, int(L), graph.h, part.h if part is not None else None,
+                                                int(shard), int(n_shards), int(precision), C.c_void_p(E.data_ptr()),
+                                                C.c_void_p(F.data_ptr()), C.c_void_p(Ei.data_ptr()),
+                                                C.c_void_p(S.data_ptr())))
+    return E, F, Ei, S
+
+
+def md_nve(ctx: Context, model: Model, L: int, pos, vel, mass, cell: np.ndarray, species, dt: float, n_steps: int,
+           grid=(1, 1, 1), halo: float = 0.0, precision: int = MLIP_FP32):
+    """mlip_md_nve: pos/vel float64 CUDA tensors updated in place; returns total energy per step (numpy [n_steps+1])."""
+    torch = _torch()
+    assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous()
+    assert vel.is_cuda and vel.dtype == torch.float64 and vel.is_contiguous()
+    assert mass.is_cuda and mass.dtype == torch.float64 and species.dtype == torch.int32
+    cell = np.ascontiguousarray(cell, dtype=np.float64)
+    g = (C.c_int * 3)(*[int(x) for x in grid])
+    out = np.zeros(n_steps + 1, dtype=np.float64)
+    ctx.check(ctx.lib.mlip_md_nve(ctx.h, model.h, int(L), C.c_void_p(pos.data_ptr()), C.c_void_p(vel.data_ptr()),
+                                  C.c_void_p(mass.data_ptr()), cell.ctypes.data_as(C.c_void_p),
+                                  C.c_void_p(species.data_ptr()), int(pos.shape[0]), g, float(halo), int(precision),
+                                  float(dt), int(n_steps), out.ctypes.data_as(C.c_void_p)))
+    return out
 
 
 def step_host(ctx: Context, model: Model, L: int, pos: np.ndarray, cell: np.ndarray, species: np.ndarray,

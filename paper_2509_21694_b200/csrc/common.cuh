@@ -221,4 +221,5 @@ void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float s
 // energy_forces.cu
 int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* m, int L, const SubGraph& g, int precision,
                        double* energy_accum_dev, float* forces_internal /*[N,3]*/,
-                       float* atom_energy_internal /*[N] or null*/);
+                       float* atom_energy_internal /*[N] or null*/,
+                       double* virial_accum_dev /*[6] xx,yy,zz,yz,xz,xy or null*/);

@@ -105,6 +105,49 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
   }
 }
 
+// Virial of one sub-domain: W_ab += sum_e rbar_e r_a r_b / r over its directed edges (rbar is zero on the
+// edges no layer evaluated). float64 per-block partials in a fixed order, then one block: deterministic, no atomics.
+__global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const float4* __restrict__ rvec,
+                                                        const float* __restrict__ rbar, double* __restrict__ partial) {
+  __shared__ double sh[6][256];
+  double w[6] = {0, 0, 0, 0, 0, 0};
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < E; e += (int64_t)gridDim.x * blockDim.x) {
+    const float4 rv = rvec[e];
+    if (rv.w > 0.f) {
+      const double s = (double)rbar[e] / (double)rv.w, x = rv.x, y = rv.y, z = rv.z;
+      w[0] += s * x * x; w[1] += s * y * y; w[2] += s * z * z;
+      w[3] += s * y * z; w[4] += s * x * z; w[5] += s * x * y;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 6; ++k) sh[k][threadIdx.x] = w[k];
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) sh[k][threadIdx.x] += sh[k][threadIdx.x + s];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 6) partial[(size_t)blockIdx.x * 6 + threadIdx.x] = sh[threadIdx.x][0];
+}
+__global__ void k_virial_final(int n_partial, const double* __restrict__ partial, double* __restrict__ virial) {
+  const int k = threadIdx.x;
+  if (k >= 6) return;
+  double v = 0.0;
+  for (int i = 0; i < n_partial; ++i) v += partial[(size_t)i * 6 + k];
+  virial[k] += v;
+}
+// stress[3][3] = W / V from the accumulated (xx, yy, zz, yz, xz, xy)
+__global__ void k_stress_out(const double* __restrict__ virial, double inv_volume, double* __restrict__ stress) {
+  if (threadIdx.x != 0) return;
+  const double xx = virial[0] * inv_volume, yy = virial[1] * inv_volume, zz = virial[2] * inv_volume;
+  const double yz = virial[3] * inv_volume, xz = virial[4] * inv_volume, xy = virial[5] * inv_volume;
+  stress[0] = xx; stress[1] = xy; stress[2] = xz;
+  stress[3] = xy; stress[4] = yy; stress[5] = yz;
+  stress[6] = xz; stress[7] = yz; stress[8] = zz;
+}
+
 __global__ void k_unpermute(int64_t N, const int32_t* __restrict__ perm, const float* __restrict__ F_int,
                             const float* __restrict__ E_int, float* __restrict__ F_out, float* __restrict__ E_out) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -116,7 +159,7 @@ __global__ void k_unpermute(int64_t N, const int32_t* __restrict__ perm, const f
 }  // namespace
 
 int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph& g, int precision,
-                       double* energy_accum, float* F_int, float* Ei_int) {
+                       double* energy_accum, float* F_int, float* Ei_int, double* virial_accum) {
   const int64_t n = g.n, E = g.E;
   if (n == 0) return MLIP_OK;
   const int d = M->h.d;
@@ -273,6 +316,14 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
     k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, F_int);
     ctx->launches++;
+    if (virial_accum && E > 0) {
+      const int nb = (int)(E < 148 * 8 * 256 ? (E + 255) / 256 : 148 * 8);
+      double* vpart = nullptr;
+      W_ALLOC(vpart, double, (size_t)nb * 6);
+      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, vpart);
+      k_virial_final<<<1, 32, 0, st>>>(nb, vpart, virial_accum);
+      ctx->launches += 2;
+    }
   }
   release();
 #undef W_ALLOC
@@ -286,9 +337,27 @@ extern "C" int mlip_energy_forces(mlip_ctx* ctx, const mlip_model* M, int L, con
   return mlip_energy_forces_shard(ctx, M, L, G, part, 0, 1, precision, energy_dev, forces_dev, atom_energy_dev);
 }
 
+static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G, const mlip_part* part,
+                              int shard, int n_shards, int precision, double* energy_dev, float* forces_dev,
+                              float* atom_energy_dev, double* stress_dev);
+
 extern "C" int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G,
                                         const mlip_part* part, int shard, int n_shards, int precision,
                                         double* energy_dev, float* forces_dev, float* atom_energy_dev) {
+  return energy_forces_impl(ctx, M, L, G, part, shard, n_shards, precision, energy_dev, forces_dev, atom_energy_dev, nullptr);
+}
+
+extern "C" int mlip_energy_forces_stress(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G,
+                                         const mlip_part* part, int shard, int n_shards, int precision,
+                                         double* energy_dev, float* forces_dev, float* atom_energy_dev,
+                                         double* stress_dev) {
+  if (ctx && !stress_dev) { ctx->set_error("mlip_energy_forces_stress: null stress pointer"); return MLIP_ERR_INVALID_ARG; }
+  return energy_forces_impl(ctx, M, L, G, part, shard, n_shards, precision, energy_dev, forces_dev, atom_energy_dev, stress_dev);
+}
+
+static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const mlip_graph* G, const mlip_part* part,
+                              int shard, int n_shards, int precision, double* energy_dev, float* forces_dev,
+                              float* atom_energy_dev, double* stress_dev) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
   if (n_shards < 1 || shard < 0 || shard >= n_shards) { ctx->set_error("shard outside [0, n_shards)"); return MLIP_ERR_INVALID_ARG; }
   if (n_shards > 1 && !part) { ctx->set_error("sharded evaluation needs a partition"); return MLIP_ERR_INVALID_ARG; }
@@ -311,13 +380,18 @@ extern "C" int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* M, int 
   cudaMemsetAsync(F_int, 0, sizeof(float) * 3 * N, st);
   cudaMemsetAsync(E_int, 0, sizeof(float) * N, st);
   cudaMemsetAsync(energy_dev, 0, sizeof(double), st);
+  double* virial = nullptr;
+  if (stress_dev) {
+    MLIP_TRY(ctx->alloc(&virial, 6));
+    cudaMemsetAsync(virial, 0, 6 * sizeof(double), st);
+  }
   int status = MLIP_OK;
   if (!part) {
-    status = mlip_eval_subgraph(ctx, M, L, G->view(), precision, energy_dev, F_int, E_int);
+    status = mlip_eval_subgraph(ctx, M, L, G->view(), precision, energy_dev, F_int, E_int, virial);
   } else {
     for (size_t k = 0; k < part->subs.size(); ++k) {
       if ((int)(k % (size_t)n_shards) != shard) continue;  // sub-domain k belongs to shard k mod n_shards
-      status = mlip_eval_subgraph(ctx, M, L, part->subs[k].g, precision, energy_dev, F_int, E_int);
+      status = mlip_eval_subgraph(ctx, M, L, part->subs[k].g, precision, energy_dev, F_int, E_int, virial);
       if (status != MLIP_OK) break;
     }
   }
@@ -325,7 +399,13 @@ extern "C" int mlip_energy_forces_shard(mlip_ctx* ctx, const mlip_model* M, int 
     k_unpermute<<<nblk(N, 256), 256, 0, st>>>(N, G->perm, F_int, E_int, forces_dev, atom_energy_dev);
     ctx->launches++;
   }
-  ctx->free(F_int); ctx->free(E_int);
+  if (status == MLIP_OK && stress_dev) {
+    const double* c = G->cell;
+    const double vol = fabs(c[0] * (c[4] * c[8] - c[5] * c[7]) - c[1] * (c[3] * c[8] - c[5] * c[6]) + c[2] * (c[3] * c[7] - c[4] * c[6]));
+    k_stress_out<<<1, 32, 0, st>>>(virial, vol > 0.0 ? 1.0 / vol : 0.0, stress_dev);
+    ctx->launches++;
+  }
+  ctx->free(F_int); ctx->free(E_int); ctx->free(virial);
   if (status != MLIP_OK) return status;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;

@@ -259,3 +259,79 @@ def test_bf16_active_sets_match_oracle():
         assert err["rms_F"] <= BF16_RMS_F
         # same tiles of the same edge prefix, exact zeros skipped: the two evaluations agree far below bf16 accuracy
         assert rms(F - Ff) <= 1e-3 * rms(Ff)
+
+
+# ---------------------------------------------------------------- stress
+def _gpu_stress(spec, blob, system, L, precision=0, grid=None, halo=0.0, shards=1):
+    import torch
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, system, spec.r_cut)
+    part = mlip.Partition(ctx, g, halo, grid=grid) if grid is not None else None
+    tot = None
+    for k in range(shards):
+        E, F, Ei, S = mlip.energy_forces_stress(ctx, model, L, g, part, precision, shard=k, n_shards=shards)
+        torch.cuda.synchronize()
+        out = [float(E.item()), F.cpu().numpy().astype(np.float64), S.cpu().numpy()]
+        tot = out if tot is None else [a + b for a, b in zip(tot, out)]
+    return tot
+
+
+def test_fp32_stress_matches_oracle_unpartitioned_and_partitioned():
+    """sigma = (1/V) dE/d(strain) against the oracle (itself pinned by strain finite differences):
+    1e-4 of the largest component in fp32, identical decomposition over sub-domains and over shards."""
+    spec = ModelSpec(4, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 25)
+    s = small_system(8, 0.08, seed=51)
+    E_ref, Ei_ref, F_ref, sig_ref = O.energy_forces_stress(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    scale = np.abs(sig_ref).max()
+    E0, F0, S0 = _gpu_stress(spec, blob, s, 2)
+    assert np.abs(S0 - sig_ref).max() <= 1e-4 * scale and np.array_equal(S0, S0.T)
+    assert np.abs(F0 - F_ref).max() <= FP32_MAX_F * rms(F_ref)
+    for grid, shards in [((3, 1, 1), 1), ((2, 2, 1), 1), ((4, 1, 1), 2)]:
+        E, F, S = _gpu_stress(spec, blob, s, 2, grid=grid, halo=6.0, shards=shards)
+        assert np.abs(S - sig_ref).max() <= 1e-4 * scale
+        assert np.abs(S - S0).max() <= 1e-5 * scale
+        assert np.abs(F - F0).max() <= 1e-5 * rms(F0) and abs(E - E0) <= 1e-5 * np.abs(Ei_ref).sum()
+    cfg = make_config(1)
+    ref = O.energy_forces_stress(oracle_model(cfg.model, cfg.weights), cfg.L, cfg.system.pos, cfg.system.cell, cfg.system.species)
+    E, F, S = _gpu_stress(cfg.model, cfg.weights, cfg.system, cfg.L)
+    assert np.abs(S - ref[3]).max() <= 1e-4 * np.abs(ref[3]).max()
+
+
+def test_bf16_stress_matches_oracle():
+    spec = ModelSpec(4, 256, 16, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 26)
+    s = small_system(8, 0.08, seed=52)
+    sig_ref = O.energy_forces_stress(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)[3]
+    for grid in [None, (2, 1, 1)]:
+        E, F, S = _gpu_stress(spec, blob, s, 2, precision=1, grid=grid, halo=6.0)
+        assert np.abs(S - sig_ref).max() <= BF16_RMS_F * np.abs(sig_ref).max()
+
+
+# ---------------------------------------------------------------- on-device MD (PAPER.md:89, 131)
+@pytest.mark.parametrize("grid,halo", [((1, 1, 1), 0.0), ((2, 1, 1), 6.0)])
+def test_md_nve_matches_oracle_trajectory(grid, halo):
+    """mlip_md_nve against the oracle's velocity-Verlet (pinned by its second-order energy error) on the same
+    start: total energy per step, final positions and velocities. fp32 forces perturb a 20-step trajectory far
+    below the tolerances; atoms cross the periodic box unwrapped, which the graph builder supports."""
+    import torch
+    spec = ModelSpec(4, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 35)
+    s = small_system(6, 0.08, seed=61)   # 21.6 A box, 864 atoms
+    rng = np.random.default_rng(7)
+    masses = rng.uniform(10.0, 60.0, len(s.pos))
+    vel0 = rng.normal(0, 0.004, s.pos.shape); vel0 -= vel0.mean(0)
+    n_steps, dt = 20, 2.0
+    e_ref, pos_ref, vel_ref = O.nve_velocity_verlet(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses,
+                                                    vel0, dt, n_steps, return_state=True)
+    mlip, ctx, model = gpu_setup(spec, blob)
+    pos = torch.tensor(s.pos, dtype=torch.float64, device="cuda:0").contiguous()
+    vel = torch.tensor(vel0, dtype=torch.float64, device="cuda:0").contiguous()
+    mass = torch.tensor(masses, dtype=torch.float64, device="cuda:0")
+    species = torch.tensor(s.species, dtype=torch.int32, device="cuda:0")
+    e = mlip.md_nve(ctx, model, 2, pos, vel, mass, s.cell, species, dt, n_steps, grid=grid, halo=halo)
+    kin0 = 0.5 * np.sum(masses[:, None] * vel0 ** 2) / O.ACC_UNIT
+    assert np.abs(e - e_ref).max() <= 1e-4 * kin0
+    assert np.abs(pos.cpu().numpy() - pos_ref).max() <= 1e-5          # Angstrom, after 40 fs
+    assert np.abs(vel.cpu().numpy() - vel_ref).max() <= 1e-5 * np.abs(vel_ref).max() + 1e-8
+    assert np.abs(pos_ref - s.pos).max() > 0.05                       # the atoms did move

@@ -340,3 +340,57 @@ def test_khop_partition_equals_unpartitioned(grid):
     bad = [(o, e[h <= L - 1]) for o, e, h in kh]
     Eb, _, Fb, _ = O.energy_forces_partitioned(m, L, s.pos, s.cell, s.species, bad, g)
     assert np.abs(Fb - F).max() > 1e-4 * rms(F)
+
+
+# ---------------------------------------------------------------- stress
+def test_stress_equals_strain_finite_difference_and_is_symmetric():
+    """sigma_ab = (1/V) dE/d eps_ab, pinned by central differences of E under the homogeneous strain
+    x -> (1 + eps) x, C -> C (1 + eps)^T with the edge list (and its image shifts) held fixed."""
+    spec, blob, m = make_model(d=8, r_cut=4.0, nbar=20.0)
+    s = small_system(2, 0.15, seed=19)
+    g = O.neighbor_list(s.pos, s.cell, spec.r_cut)
+    E, E_i, F, sig = O.energy_forces_stress(m, 2, s.pos, s.cell, s.species, g)
+    assert np.allclose(sig, sig.T, rtol=0, atol=1e-14 * np.abs(sig).max())
+    V = abs(np.linalg.det(s.cell))
+    h = 1e-6
+    fd = np.zeros((3, 3))
+    for a in range(3):
+        for b in range(3):
+            eps = np.zeros((3, 3)); eps[a, b] = h
+            Ep = O.energy_forces(m, 2, s.pos @ (np.eye(3) + eps).T, s.cell @ (np.eye(3) + eps).T, s.species, g)[0]
+            Em = O.energy_forces(m, 2, s.pos @ (np.eye(3) - eps).T, s.cell @ (np.eye(3) - eps).T, s.species, g)[0]
+            fd[a, b] = (Ep - Em) / (2 * h) / V
+    assert np.abs(fd - sig).max() < 1e-6 * np.abs(sig).max()
+    # rigid rotation costs no energy: the antisymmetric part of dE/d eps vanishes
+    assert np.abs(fd - fd.T).max() < 1e-6 * np.abs(sig).max()
+
+
+def test_stress_dimer_closed_form_and_cubic_lattice_isotropy():
+    spec, blob, m = make_model(d=8, r_cut=4.0, nbar=20.0)
+    # dimer along x: two directed edges, sigma_xx = 2 rbar r / V, everything else zero
+    cell = np.diag([30.0, 30.0, 30.0])
+    pos = np.array([[5.0, 5.0, 5.0], [7.5, 5.0, 5.0]])
+    sp = np.array([0, 1], np.int32)
+    E, E_i, F, ex = O.energy_forces(m, 2, pos, cell, sp, return_extra=True)
+    sig = O.stress_from_rbar(cell, ex["rvec"], ex["r"], ex["rbar"])
+    assert len(ex["r"]) == 2
+    expect = np.zeros((3, 3)); expect[0, 0] = float(np.sum(ex["rbar"]) * 2.5 / 27000.0)
+    assert np.allclose(sig, expect, rtol=1e-12, atol=1e-18)
+    # virial theorem for a pair: sigma_xx V = -F_x(atom 1) * (x_1 - x_0)
+    assert np.isclose(sig[0, 0] * 27000.0, -F[1, 0] * 2.5, rtol=1e-10)
+    # perfect single-species fcc: cubic symmetry => isotropic stress
+    sites, cell = fcc_box(3, 3.6)
+    sig = O.energy_forces_stress(m, 2, sites, cell, np.zeros(len(sites), np.int32))[3]
+    assert np.abs(sig - np.eye(3) * sig[0, 0]).max() < 1e-12 * abs(sig[0, 0])
+
+
+def test_stress_partitioned_equals_unpartitioned():
+    spec, blob, m = make_model(r_cut=3.0, nbar=12.0)
+    L = 2
+    s = small_system(8, 0.08, seed=33)
+    g = O.neighbor_list(s.pos, s.cell, spec.r_cut)
+    sig = O.energy_forces_stress(m, L, s.pos, s.cell, s.species, g)[3]
+    for parts in (O.partition_grid(s.pos, s.cell, (3, 1, 1), L * spec.r_cut),
+                  [(o, e) for o, e, _ in O.partition_grid_khop(s.pos, s.cell, (2, 2, 1), L * spec.r_cut, spec.r_cut, g)]):
+        sp_ = O.stress_partitioned(m, L, s.pos, s.cell, s.species, parts, g)
+        assert np.abs(sp_ - sig).max() < 1e-12 * np.abs(sig).max()
