@@ -194,6 +194,7 @@ def run_ours(args):
     import torch.distributed as dist
 
     import paper_2509_21694_b200 as mlip
+    from paper_2509_21694_b200.dist import all_reduce_results
     from synth_inputs import make_config
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -230,8 +231,7 @@ def run_ours(args):
         part = mlip.Partition(ctx, g, cfg.halo, grid=cfg.grid) if partitioned else None
         if world > 1:
             E, F, _ = mlip.energy_forces_shard(ctx, model, cfg.L, g, part, rank, world, prec, out=out)
-            dist.all_reduce(E)
-            dist.all_reduce(F)
+            all_reduce_results(E, F)
         else:
             E, F, _ = mlip.energy_forces(ctx, model, cfg.L, g, part, prec, want_atom_energy=False, out=out)
         info["edges"] = g.num_edges
