@@ -182,6 +182,19 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------
 # the CUDA path
 # ------------------------------------------------------------------------------------------
+def ncu_traffic(config: int, group: str):
+    """DRAM bytes per launch of a kernel group from the committed ncu --set full capture (profiles/*_traffic.csv,
+    newest round last), or None when no capture of this config exists."""
+    import csv
+    import glob
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
+        for row in csv.DictReader(open(path)):
+            if int(row["config"]) == config and row["kernel_group"] == group:
+                best = float(row["dram_bytes_per_launch"])
+    return best
+
+
 def flops_edge_layer(d: int, n_rbf: int) -> float:
     """Algorithmic flop per edge per layer of one direction: the first edge
     linear factorises into per-node projections, so only the n_rbf x d term and the d x d second
@@ -311,7 +324,8 @@ def run_ours(args):
     else:
         bound, peak, peak_src = "alu", ALU_FP32_TFLOPS, "derived: 148 SM x 128 FMA x 2 x 1.965 GHz"
     roofline = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(args.config, dom), "traffic_unit": "dram bytes per launch (ncu)",
+                "peak_source": peak_src,
                 "algorithmic_flop_per_step": flop, "kernel_ms_per_step": per_step[dom],
                 "executed_over_algorithmic": 2.0 if dom == "edge_bwd" else 1.0}
 
