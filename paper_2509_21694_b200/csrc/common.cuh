@@ -204,6 +204,10 @@ int mlip_exclusive_scan_i32(mlip_ctx* ctx, const int32_t* in, int32_t* out, int6
 struct GemmArgs {
   const float* X1 = nullptr; int ld1 = 0; int K1 = 0;
   const float* X2 = nullptr; int ld2 = 0; int K2 = 0;
+  // tensor-core path only: a column block may be given as bf16 instead (same ld / K fields); it is then copied
+  // into the operand slab as it is -- the value the fp32 form would have been rounded to on load
+  const __nv_bfloat16* X1b = nullptr;
+  const __nv_bfloat16* X2b = nullptr;
   int act_in = 0;                 // 1: SiLU applied to X on load
   const void* B = nullptr;        // [N, K1+K2] row-major (fp32 path) / bf16 SW128 operand image (tensor path)
   const float* bias = nullptr;    // [N]

@@ -10,12 +10,17 @@ namespace {
 inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 __global__ void k_embed(int64_t n, int d, const int32_t* __restrict__ species, const float* __restrict__ T,
-                        float* __restrict__ h) {
+                        float* __restrict__ h, __nv_bfloat16* __restrict__ hb /*bf16 copy for the GEMM operands, or null*/) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n * (d / 4)) return;
   const int64_t i = idx / (d / 4);
   const int c = (int)(idx % (d / 4)) * 4;
-  *reinterpret_cast<float4*>(h + i * d + c) = *reinterpret_cast<const float4*>(T + (size_t)species[i] * d + c);
+  const float4 v = *reinterpret_cast<const float4*>(T + (size_t)species[i] * d + c);
+  *reinterpret_cast<float4*>(h + i * d + c) = v;
+  if (hb) {
+    __nv_bfloat162 lo = __floats2bfloat162_rn(v.x, v.y), hi = __floats2bfloat162_rn(v.z, v.w);
+    *reinterpret_cast<uint2*>(hb + i * d + c) = make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
+  }
 }
 
 // E_i = wo . SiLU(o_i) + b_E + E0[z_i];  obar_i = omega_i wo * SiLU'(o_i)   (O4, first line of O5)
@@ -191,7 +196,19 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   float *m = nullptr, *o = nullptr, *hbar = nullptr, *cbar = nullptr, *PQbar = nullptr, *head = nullptr, *tail = nullptr,
         *rbar = nullptr, *E_i = nullptr, *abar = nullptr;
   __half *abar_h = nullptr, *mbar_h = nullptr;
+  // tensor-core path: tensors that are only ever read as bf16 GEMM operands are STORED as bf16 -- the value the operand
+  // producer would round the fp32 form to, so results do not change while the HBM-bound node GEMMs move fewer bytes:
+  // hb = copy of the residual stream h^l (two buffers, alternating), cbar_b, Qbar_b
+  __nv_bfloat16 *hb[2] = {nullptr, nullptr}, *cbar_b = nullptr, *Qbar_b = nullptr;
   double* partial = nullptr;
+  if (bf) {
+    W_ALLOC(hb[0], __nv_bfloat16, n * d); W_ALLOC(hb[1], __nv_bfloat16, n * d);
+    W_ALLOC(cbar_b, __nv_bfloat16, n * d); W_ALLOC(Qbar_b, __nv_bfloat16, n * d);
+  }
+  auto from_h = [&](GemmArgs& a, int l) {  // X1 = h^l
+    if (bf) a.X1b = hb[l & 1]; else a.X1 = h[l];
+    a.ld1 = d; a.K1 = d;
+  };
   W_ALLOC(m, float, n * d); W_ALLOC(o, float, n * d); W_ALLOC(hbar, float, n * d); W_ALLOC(cbar, float, n * d);
   W_ALLOC(PQbar, float, n * 2 * d); W_ALLOC(head, float, (tiles + 1) * d); W_ALLOC(tail, float, (tiles + 1) * d);
   W_ALLOC(rbar, float, E + 1); W_ALLOC(E_i, float, n);
@@ -204,7 +221,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
 
   {
     ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
-    k_embed<<<nblk(n * (d / 4), 256), 256, 0, st>>>(n, d, g.species, M->T, h[0]);
+    k_embed<<<nblk(n * (d / 4), 256), 256, 0, st>>>(n, d, g.species, M->T, h[0], hb[0]);
     ctx->launches++;
   }
 
@@ -232,9 +249,9 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     const int64_t nr = n_recv(l), ns = n_send(l);
     GemmArgs a;
     if (bf) {
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = nr; a.N = d;
+      a = GemmArgs(); from_h(a, l); a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = nr; a.N = d;
       W_TRY(gemm(ctx, a));
-      a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = ns; a.N = d;
+      a = GemmArgs(); from_h(a, l); a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = ns; a.N = d;
       W_TRY(gemm(ctx, a));
     } else {
       a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.B = W.W1ab; a.bias = W.b1pad; a.Y = P[l]; a.ldy = 2 * d; a.n = ns; a.N = 2 * d;
@@ -247,17 +264,17 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
       W_TRY(bf ? mlip_edge_forward_tc(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
     }
-    a = GemmArgs(); a.X1 = h[l]; a.ld1 = d; a.K1 = d; a.X2 = m; a.ld2 = d; a.K2 = d;
+    a = GemmArgs(); from_h(a, l); a.X2 = m; a.ld2 = d; a.K2 = d;
     a.B = bf ? (const void*)W.V1_bf : (const void*)W.V1; a.bias = W.c1; a.Y = c[l]; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
     a = GemmArgs(); a.X1 = c[l]; a.ld1 = d; a.K1 = d; a.act_in = 1;
     a.B = bf ? (const void*)W.V2_bf : (const void*)W.V2; a.bias = W.c2; a.residual = h[l]; a.ldr = d;
-    a.Y = h[l + 1]; a.ldy = d; a.n = nr; a.N = d;
+    a.Y = h[l + 1]; a.Ybf = bf ? hb[(l + 1) & 1] : nullptr; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
   }
   {
     GemmArgs a;
-    a.X1 = h[L]; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->Wo_bf : (const void*)M->Wo; a.bias = M->bo;
+    from_h(a, L); a.B = bf ? (const void*)M->Wo_bf : (const void*)M->Wo; a.bias = M->bo;
     a.Y = o; a.ldy = d; a.n = n0; a.N = d;
     W_TRY(gemm(ctx, a));
   }
@@ -284,13 +301,15 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     const int64_t nr = n_recv(l), ns = n_send(l), Er = e_recv(l);
     GemmArgs a;
     a = GemmArgs(); a.X1 = hbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V2T_bf : (const void*)W.V2T;
-    a.mul_dsilu = c[l]; a.ldz = d; a.Y = cbar; a.ldy = d; a.n = nr; a.N = d;
+    a.mul_dsilu = c[l]; a.ldz = d; a.ldy = d; a.n = nr; a.N = d;
+    if (bf) a.Ybf = cbar_b; else a.Y = cbar;
     W_TRY(gemm(ctx, a));
-    a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1bT_bf : (const void*)W.V1bT;
+    auto from_cbar = [&](GemmArgs& x) { if (bf) x.X1b = cbar_b; else x.X1 = cbar; x.ld1 = d; x.K1 = d; };
+    a = GemmArgs(); from_cbar(a); a.B = bf ? (const void*)W.V1bT_bf : (const void*)W.V1bT;
     if (bf) a.Yh = mbar_h; else a.Y = mbar;
     a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
-    a = GemmArgs(); a.X1 = cbar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
+    a = GemmArgs(); from_cbar(a); a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
     a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
     cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
@@ -304,10 +323,11 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     {
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
       // Qbar_j over the senders of this layer, summing only the reverse edges that were evaluated (rev[e] < Er)
-      W_TRY(bf ? mlip_gather_rev_tc(ctx, ns, Er, d, g.rowptr, g.rev, abar_h, Qbar)
+      W_TRY(bf ? mlip_gather_rev_tc(ctx, ns, Er, d, g.rowptr, g.rev, abar_h, Qbar_b)
                : mlip_gather_rev_f32(ctx, ns, Er, d, g.rowptr, g.rev, abar, Qbar));
     }
-    a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.X2 = Qbar; a.ld2 = d; a.K2 = d;
+    a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.ld2 = d; a.K2 = d;
+    if (bf) a.X2b = Qbar_b; else a.X2 = Qbar;
     a.B = bf ? (const void*)W.W1abT_bf : (const void*)W.W1abT; a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d;
     a.n = ns; a.N = d;
     W_TRY(gemm(ctx, a));
