@@ -29,6 +29,10 @@ struct EdgeArgs {
   __half* abar_h = nullptr;                        // backward spill, f16 tile images [tiles,128,d]
   float* Pbar = nullptr;                           // backward out [n,d]
   float* rbar = nullptr;                           // [E] accumulated over layers
+  // backward only: false for the FIRST layer, whose node-side adjoints (Pbar, the spilled abar -> Qbar) would only feed
+  // the gradient w.r.t. the species embedding -- forces need nothing but rbar, so the spill, the segmented sum and the
+  // sender-side gather of that layer are skipped
+  bool node_adjoint = true;
 };
 
 int64_t mlip_edge_f32_tiles(int64_t E);

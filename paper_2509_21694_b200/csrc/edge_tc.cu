@@ -484,12 +484,13 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           }
         }
         tc::mbar_wait(bar(B_SEL_FULL), (uint32_t)(it & 1));
-        const bool seg_mma = *reinterpret_cast<volatile int*>(&seg[b].R) <= MAX_SEG;
+        const bool seg_mma = *reinterpret_cast<volatile int*>(&seg[b].R) <= MAX_SEG && (!BWD || a.node_adjoint);
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           wait_slab(s);
           if (BWD) {
-            tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
+            if (a.node_adjoint)
+              tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
             tc::bulk_commit();  // one bulk group per slab: a slab is released as soon as ITS copy has read it
             // G4: ebar/2 = abar . (W1c/2). B = the G1 image [channel][16] read MN-major (N = rbf index, K = channel),
             // no swizzle: N-direction core-matrix stride (SBO) 128 B, K-direction 8-channel group stride (LBO) 256 B
@@ -563,7 +564,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       const int R = G.R;
       tc::mbar_wait(bar(B_SEG_FULL), par);
       tc::fence_after_sync();
-      if (R <= MAX_SEG) {
+      if (BWD && !a.node_adjoint) {
+        // first layer: no node-side adjoint wanted, only E4 below
+      } else if (R <= MAX_SEG) {
         // Yseg: 16 columns (receiver slots) per 128 channels; warp group g reads 2 NCH of the 8 NCH columns
         constexpr int NR = 2 * NCH;
         const int h = (g * NR) >> 4, r0 = (g * NR) & 15;
@@ -864,9 +867,12 @@ int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   const unsigned grid = (unsigned)(tiles < ctx->num_sms ? tiles : ctx->num_sms);
   MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_tc<D, BWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   k_edge_tc<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
-  k_segment_fixup_tc<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
-                                                                             BWD ? a.Pbar : a.m);
-  ctx->launches += 2;
+  ctx->launches++;
+  if (!BWD || a.node_adjoint) {
+    k_segment_fixup_tc<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
+                                                                               BWD ? a.Pbar : a.m);
+    ctx->launches++;
+  }
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
 }

@@ -309,17 +309,24 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     if (bf) a.Yh = mbar_h; else a.Y = mbar;
     a.ldy = d; a.n = nr; a.N = d;
     W_TRY(gemm(ctx, a));
-    a = GemmArgs(); from_cbar(a); a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
-    a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = nr; a.N = d;
-    W_TRY(gemm(ctx, a));
-    cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
+    // The adjoint of h^0 (the species embedding) is a weight gradient: forces need only rbar. The first layer therefore
+    // skips everything that would only feed it: the h-path GEMM, the abar spill, the Pbar sums, the sender-side gather
+    // and the projection GEMM.
+    const bool node_adjoint = l > 0;
+    if (node_adjoint) {
+      a = GemmArgs(); from_cbar(a); a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
+      a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = nr; a.N = d;
+      W_TRY(gemm(ctx, a));
+      cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
+    }
     set_layer(l);
-    ea.E = Er; ea.n = nr;
+    ea.E = Er; ea.n = nr; ea.node_adjoint = bf ? node_adjoint : true;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
       W_TRY(bf ? mlip_edge_backward_tc(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
     }
+    if (!node_adjoint) continue;
     {
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
       // Qbar_j over the senders of this layer, summing only the reverse edges that were evaluated (rev[e] < Er)
