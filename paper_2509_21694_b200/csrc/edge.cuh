@@ -14,6 +14,9 @@ struct EdgeArgs {
   const __half* Ph = nullptr;                      // halved receiver pre-projection (tensor-core path, f16), ld = d
   const float* Q = nullptr; int ldq = 0;           // sender pre-projection W1b h_j (fp32 path)
   const __half* Qh = nullptr;                      // halved sender pre-projection (tensor-core path, f16), ld = d
+  // tensor-core path: when given, row a of Ph / Qh belongs to atom i with row_index[i] == a. The first layer passes the
+  // species here: h^0 is the species embedding, so P^0 and Q^0 are S-row tables and the per-edge gathers hit L1
+  const int32_t* row_index = nullptr;
   const float* W1c = nullptr;                      // [d,16] fp32
   const float* W2T = nullptr;                      // [in,out] fp32
   const float* W2 = nullptr;                       // [out,in] fp32

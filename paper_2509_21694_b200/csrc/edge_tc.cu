@@ -264,6 +264,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         rc[k] = -1; sd[k] = 0; rr[k] = 0.f;
         if (ge < a.E) { rc[k] = a.recv[ge]; sd[k] = a.send[ge]; rr[k] = a.rvec[ge].w; }
       }
+      if (a.row_index) {  // M.send carries the ROW of the Q table: the sender itself, or its species in the first layer
+#pragma unroll
+        for (int k = 0; k < EPL; ++k)
+          if (rc[k] >= 0) sd[k] = a.row_index[sd[k]];
+      }
       tc::mbar_wait(bar(B_META_EMPTY + b), (uint32_t)(((it >> 1) & 1) ^ 1));
       uint32_t pk[EPL][8];
 #pragma unroll
@@ -352,7 +357,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           uint4 pr[NSLOT];
 #pragma unroll
           for (int r = 0; r < NSLOT; ++r)
-            if (r < R) pr[r] = ldg_nc_v4(a.Ph + (size_t)G.rid[r] * D + lane * 8);
+            if (r < R) pr[r] = ldg_nc_v4(a.Ph + (size_t)(a.row_index ? a.row_index[G.rid[r]] : G.rid[r]) * D + lane * 8);
 #pragma unroll
           for (int r = 0; r < NSLOT; ++r)
             if (r < R) *reinterpret_cast<uint4*>(gen + SM::ptile + r * D * 2 + lane * 16) = pr[r];
@@ -636,7 +641,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       const bool fast = R <= NSLOT;
       const int myslot = G.slot[row];
       const unsigned char* prow = fast ? gen + SM::ptile + myslot * (D * 2) + 32 * g
-                                       : reinterpret_cast<const unsigned char*>(a.Ph + (size_t)(valid ? rc : 0) * D + 16 * g);
+                                       : reinterpret_cast<const unsigned char*>(
+                                             a.Ph + (size_t)(valid ? (a.row_index ? a.row_index[rc] : rc) : 0) * D + 16 * g);
 
       // ---- E1: a' = X + P'_i + Q'_j ; s = a' + a' tanh(a') ----
       tc::mbar_wait(bar(B_D1_FULL), par);

@@ -232,6 +232,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   auto set_layer = [&](int l) {
     const LayerWeights& W = M->layers[l];
     ea.P = P[l]; ea.ldp = 2 * d; ea.Q = Qf[l]; ea.ldq = 2 * d; ea.Ph = Ph[l]; ea.Qh = Qh[l];
+    ea.row_index = (bf && l == 0) ? g.species : nullptr;  // P^0, Q^0 are per-species tables (below)
     ea.W1c = W.W1c; ea.W2T = W.W2T; ea.W2 = W.W2; ea.b2 = W.b2;
     ea.W2img = W.W2img; ea.W1cimg = W.W1cimg;
   };
@@ -248,7 +249,14 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     const LayerWeights& W = M->layers[l];
     const int64_t nr = n_recv(l), ns = n_send(l);
     GemmArgs a;
-    if (bf) {
+    if (bf && l == 0) {
+      // h^0_i = T[z_i]: the pre-projections of the first layer are S-row tables, P^0 = W1a T + b1, Q^0 = W1b T, indexed
+      // by species inside the edge kernels (EdgeArgs::row_index)
+      a = GemmArgs(); a.X1 = M->T; a.ld1 = d; a.K1 = d; a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = M->h.n_species; a.N = d;
+      W_TRY(gemm(ctx, a));
+      a = GemmArgs(); a.X1 = M->T; a.ld1 = d; a.K1 = d; a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = M->h.n_species; a.N = d;
+      W_TRY(gemm(ctx, a));
+    } else if (bf) {
       a = GemmArgs(); from_h(a, l); a.B = W.W1a_bf; a.bias = W.b1h; a.Yh = Ph[l]; a.ldy = d; a.n = nr; a.N = d;
       W_TRY(gemm(ctx, a));
       a = GemmArgs(); from_h(a, l); a.B = W.W1b_bf; a.Yh = Qh[l]; a.ldy = d; a.n = ns; a.N = d;
