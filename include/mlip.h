@@ -38,7 +38,7 @@ extern "C" {
 typedef enum {
   MLIP_OK = 0,
   MLIP_ERR_INVALID_ARG = -1,
-  MLIP_ERR_UNSUPPORTED = -2,     /* singular / non-orthorhombic cell, d not in {64,128,256}, L > L_max ... */
+  MLIP_ERR_UNSUPPORTED = -2,     /* singular cell, d not in {64,128,256}, L > L_max ... */
   MLIP_ERR_HALO_TOO_SMALL = -3,  /* halo < L*r_cut: refused rather than silently wrong forces */
   MLIP_ERR_OUT_OF_MEMORY = -4,
   MLIP_ERR_OVERFLOW = -5,        /* number of edges >= 2^31 or image shift outside [-127,127] */
@@ -91,7 +91,7 @@ void mlip_model_destroy(mlip_model* m);
  * (strict, float64, fixed operation order, reading R10) and not (i == j and n == 0).
  *   pos_dev     [n_atoms,3] float64, device, unwrapped Cartesian positions (Angstrom)
  *   cell_host   [3,3] float64, HOST, rows are the lattice vectors a1,a2,a3; must be
- *               orthorhombic (diagonal) in this version, else MLIP_ERR_UNSUPPORTED (R12)
+ *               any non-singular (triclinic) cell; a singular one gives MLIP_ERR_UNSUPPORTED (R12)
  *   species_dev [n_atoms] int32, device, values in [0, n_species)
  * The graph keeps its own (cell-sorted) copy of what it needs. */
 int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const double* cell_host,

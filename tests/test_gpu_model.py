@@ -335,3 +335,30 @@ def test_md_nve_matches_oracle_trajectory(grid, halo):
     assert np.abs(pos.cpu().numpy() - pos_ref).max() <= 1e-5          # Angstrom, after 40 fs
     assert np.abs(vel.cpu().numpy() - vel_ref).max() <= 1e-5 * np.abs(vel_ref).max() + 1e-8
     assert np.abs(pos_ref - s.pos).max() > 0.05                       # the atoms did move
+
+
+# ---------------------------------------------------------------- triclinic cells (reading R12)
+def test_fp32_triclinic_cell_matches_oracle_and_partitions():
+    """General (non-orthorhombic) lattice, unwrapped positions: energies, forces and stress against the oracle, and a
+    partitioned evaluation (bins on the scaled coordinates, halo against the perpendicular widths) against both."""
+    from synth_inputs import System
+    rng = np.random.default_rng(11)
+    cell = np.array([[26.0, 0.0, 0.0], [5.0, 23.0, 0.0], [-4.0, 3.0, 21.0]])
+    n = 1400
+    pos = rng.uniform(0, 1, (n, 3)) @ cell
+    # keep atoms apart (random points can sit on top of each other): reject pairs closer than 1.6 A
+    g0 = O.neighbor_list(pos, cell, 1.6)
+    keep = np.ones(n, bool); keep[np.maximum(g0[0], g0[1])] = False
+    pos = pos[keep] + rng.integers(-1, 2, (int(keep.sum()), 3)).astype(float) @ cell
+    s = System(pos, cell, rng.integers(0, 4, len(pos)).astype(np.int32))
+    spec = ModelSpec(4, 64, 8, 2, 3.5, 1.0 / np.sqrt(14.0))
+    blob = make_weights(spec, 55)
+    E_ref, Ei_ref, F_ref, sig_ref = O.energy_forces_stress(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    E0, F0, S0 = _gpu_stress(spec, blob, s, 2)
+    assert abs(E0 - E_ref) <= FP32_EPS_E * np.abs(Ei_ref).sum()
+    assert np.abs(F0 - F_ref).max() <= FP32_MAX_F * rms(F_ref)
+    assert np.abs(S0 - sig_ref).max() <= 1e-4 * np.abs(sig_ref).max()
+    for grid in [(2, 1, 1), (1, 2, 1), (1, 1, 2)]:
+        E, F, S = _gpu_stress(spec, blob, s, 2, grid=grid, halo=7.0)
+        assert np.abs(F - F0).max() <= 1e-5 * rms(F0) and abs(E - E0) <= 1e-5 * np.abs(Ei_ref).sum()
+        assert np.abs(S - S0).max() <= 1e-5 * np.abs(sig_ref).max()
