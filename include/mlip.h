@@ -90,8 +90,8 @@ void mlip_model_destroy(mlip_model* m);
  * sort + prefix sum. Directed edge (i <- j, n) exists iff |x_j - x_i + n.C|^2 < r_cut^2
  * (strict, float64, fixed operation order, reading R10) and not (i == j and n == 0).
  *   pos_dev     [n_atoms,3] float64, device, unwrapped Cartesian positions (Angstrom)
- *   cell_host   [3,3] float64, HOST, rows are the lattice vectors a1,a2,a3; must be
- *               any non-singular (triclinic) cell; a singular one gives MLIP_ERR_UNSUPPORTED (R12)
+ *   cell_host   [3,3] float64, HOST, rows are the lattice vectors a1,a2,a3 of any non-singular
+ *               (triclinic) cell; a singular one gives MLIP_ERR_UNSUPPORTED (R12)
  *   species_dev [n_atoms] int32, device, values in [0, n_species)
  * The graph keeps its own (cell-sorted) copy of what it needs. */
 int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const double* cell_host,
