@@ -189,7 +189,10 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   std::vector<__half*> Ph(L, nullptr), Qh(L, nullptr);
   for (int l = 0; l <= L; ++l) W_ALLOC(h[l], float, n * d);
   for (int l = 0; l < L; ++l) {
-    if (bf) { W_ALLOC(Ph[l], __half, n * d); W_ALLOC(Qh[l], __half, n * d); }
+    if (bf) {  // layer 0 holds the S-row species tables (section 5b of DESIGN.md), the others one row per atom
+      const int64_t rows = l == 0 ? (int64_t)M->h.n_species : n;
+      W_ALLOC(Ph[l], __half, rows * d); W_ALLOC(Qh[l], __half, rows * d);
+    }
     else { W_ALLOC(P[l], float, n * 2 * d); Qf[l] = P[l] + d; }
     W_ALLOC(c[l], float, n * d);
   }

@@ -362,3 +362,50 @@ def test_fp32_triclinic_cell_matches_oracle_and_partitions():
         E, F, S = _gpu_stress(spec, blob, s, 2, grid=grid, halo=7.0)
         assert np.abs(F - F0).max() <= 1e-5 * rms(F0) and abs(E - E0) <= 1e-5 * np.abs(Ei_ref).sum()
         assert np.abs(S - S0).max() <= 1e-5 * np.abs(sig_ref).max()
+
+
+# ---------------------------------------------------------------- degenerate inputs
+@pytest.mark.parametrize("precision,d", [(0, 64), (1, 128)])
+def test_degenerate_systems(precision, d):
+    """Empty box, atoms without neighbours, a sub-domain without atoms, two coincident atoms (r = 0 edges, reading R13)
+    and a box smaller than r_cut (self images): finite results equal to the oracle's."""
+    import torch
+    from synth_inputs import System
+    spec = ModelSpec(4, d, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 65)
+    om = oracle_model(spec, blob)
+    tolF = FP32_MAX_F if precision == 0 else 5e-2
+    tolE = FP32_EPS_E if precision == 0 else 3e-3   # a handful of atoms: no averaging of the bf16 operand rounding
+    # empty system
+    mlip, ctx, model = gpu_setup(spec, blob)
+    s0 = System(np.zeros((0, 3)), np.eye(3) * 10.0, np.zeros(0, np.int32))
+    g = gpu_graph(mlip, ctx, s0, spec.r_cut)
+    E, F, Ei = gpu_energy_forces(mlip, ctx, model, 2, g, None, precision)
+    assert E == 0.0 and F.shape == (0, 3)
+    part = mlip.Partition(ctx, g, 6.0, grid=(2, 1, 1))
+    E, F, Ei = gpu_energy_forces(mlip, ctx, model, 2, g, part, precision)
+    assert E == 0.0
+    # three isolated atoms + one bonded pair, in a box cut so that some bins are empty
+    pos = np.array([[1.0, 1.0, 1.0], [12.0, 1.0, 1.0], [1.0, 14.0, 9.0], [20.0, 20.0, 20.0], [21.9, 20.3, 19.8]])
+    s1 = System(pos, np.eye(3) * 40.0, np.array([0, 1, 2, 3, 1], np.int32))
+    ref = O.energy_forces(om, 2, s1.pos, s1.cell, s1.species)
+    for grid in [None, (4, 1, 1), (2, 2, 2)]:
+        E, F, Ei = _run(spec, blob, s1, 2, precision, grid=grid, halo=6.0)
+        assert abs(E - ref[0]) <= tolE * np.abs(ref[1]).sum()
+        assert np.abs(F - ref[2]).max() <= tolF * max(rms(ref[2]), 1e-6) + 1e-6
+        assert np.all(F[:3] == 0.0)
+    # two coincident atoms: the r = 0 edges are kept, their direction is defined as zero
+    s2 = small_system(3, 0.05, seed=9)
+    pos2 = s2.pos.copy(); pos2[5] = pos2[17]
+    s2 = System(pos2, s2.cell, s2.species)
+    ref = O.energy_forces(om, 2, s2.pos, s2.cell, s2.species)
+    E, F, Ei = _run(spec, blob, s2, 2, precision)
+    assert np.all(np.isfinite(F)) and abs(E - ref[0]) <= tolE * np.abs(ref[1]).sum()
+    assert np.abs(F - ref[2]).max() <= tolF * rms(ref[2])
+    # box smaller than r_cut: an atom is its own neighbour through the periodic images
+    s3 = System(np.array([[0.3, 0.2, 0.1], [1.4, 1.2, 1.1]]), np.eye(3) * 2.6, np.array([0, 2], np.int32))
+    ref = O.energy_forces(om, 2, s3.pos, s3.cell, s3.species)
+    E, F, Ei = _run(spec, blob, s3, 2, precision)
+    assert abs(E - ref[0]) <= tolE * np.abs(ref[1]).sum()
+    # the net force is what is left of much larger image contributions that cancel: the bf16 path is held to an absolute bound
+    assert np.abs(F - ref[2]).max() <= tolF * max(rms(ref[2]), 1e-6) + (1e-6 if precision == 0 else 1e-4)
