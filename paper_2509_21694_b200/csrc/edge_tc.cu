@@ -439,6 +439,13 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int b = it & 1;
         const bool has_next = tile + gridDim.x < n_tiles;
+        // the spill copies of the previous tile have been in flight since its E3; by now (G1 of this tile is issued) they
+        // have read their slabs, so this wait does not hold up the MMA issue the way a wait inside the GS loop did
+        if (BWD && it > 0) {
+          tc::bulk_wait_read<0>();
+#pragma unroll
+          for (int s = 0; s < NCH; ++s) mbar_arrive(bar(B_SPILL_S + s));
+        }
         // G2, one K slab at a time
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
@@ -512,16 +519,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
                            tc::smem_desc(base + SM::ring + (s - 1) * SLOT_BYTES + j * 2048, SLOT_BYTES, 1024, tc::LAYOUT_SW128),
                            tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
           }
-          if (BWD && s > 0) {
-            tc::bulk_wait_read<1>();  // every spill copy but the newest has read its slab
-            mbar_arrive(bar(B_SPILL_S + s - 1));
-          }
         }
         tc::mma_commit(bar(B_SEG_FULL));
         if (BWD) {
           if (has_next) issue_g1(it + 1);  // backward: X (D3) is released by the last E3 read
-          tc::bulk_wait_read<0>();
-          mbar_arrive(bar(B_SPILL_S + NCH - 1));
         }
       }
       if (BWD) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -606,7 +607,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         for (int k = 0; k < 16; ++k)
           if (k < a.n_rbf) part = fmaf(__uint_as_float(eb[k]), gk[k] * fmaf(c1, r - (float)k * delta, du), part);
         const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
-        if (valid) a.rbar[e0 + row] += fmaf(ubar, du, 2.0f * part);
+        // one addition per edge and layer, layers are separate launches: a fire-and-forget reduction is deterministic
+        // and, unlike a read-modify-write, has no global-load latency inside E1 of the next tile
+        if (valid) atomicAdd(a.rbar + e0 + row, fmaf(ubar, du, 2.0f * part));
       }
       tc::fence_before_sync();
       __syncwarp();
