@@ -420,6 +420,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       constexpr uint32_t IDESC_NH_BT = tc::idesc_f16(128, D / 2, 0, 1);
       constexpr uint32_t IDESC_N16_BT = tc::idesc_f16(128, 16, 0, 1);
       constexpr uint32_t IDESC_SEG = tc::idesc_f16(128, 16, 1, 0);   // A read MN-major (M = channel, K = edge)
+      constexpr uint32_t IDESC_N64 = tc::idesc_f16(128, 64, 0, 0);   // G1 of the next tile, one 64-column slab at a time
       uint32_t srp = 0;  // bit s: parity of the next completion of S_READY[s]
       auto wait_slab = [&](int s) {
         tc::mbar_wait(bar(B_S_READY + s), (srp >> s) & 1u);
@@ -519,11 +520,17 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
                            tc::smem_desc(base + SM::ring + (s - 1) * SLOT_BYTES + j * 2048, SLOT_BYTES, 1024, tc::LAYOUT_SW128),
                            tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
           }
+          if (BWD && has_next) {
+            // G1 of the NEXT tile, slab by slab: E3 has just published slab s, i.e. read the last of the X columns of this
+            // slab, so they can take the next tile's e_hat . W1c^T now instead of after the whole of E3 (the backward
+            // kernel used to start every tile waiting ~1 k cycles for G1)
+            if (s == 0) { tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)((it + 1) & 1)); tc::fence_after_sync(); }
+            tc::mma_bf16(TX + (uint32_t)(64 * s), tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE),
+                         tc::smem_desc(base + SM::w1c + s * 2048, 128, 256, tc::LAYOUT_NONE), IDESC_N64, false);
+            if (s == NCH - 1) tc::mma_commit(bar(B_D1_FULL));
+          }
         }
         tc::mma_commit(bar(B_SEG_FULL));
-        if (BWD) {
-          if (has_next) issue_g1(it + 1);  // backward: X (D3) is released by the last E3 read
-        }
       }
       if (BWD) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
