@@ -501,6 +501,15 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           wait_slab(s);
+          if (BWD && has_next) {
+            // G1 of the NEXT tile, slab by slab and ahead of this slab's G4 / GS: E3 has just published slab s, i.e. read the
+            // last of the X columns of this slab, so they can take the next tile's e_hat . W1c^T now instead of after the whole of E3 (the backward
+            // kernel used to start every tile waiting ~1 k cycles for G1)
+            if (s == 0) { tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)((it + 1) & 1)); tc::fence_after_sync(); }
+            tc::mma_bf16(TX + (uint32_t)(64 * s), tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE),
+                         tc::smem_desc(base + SM::w1c + s * 2048, 128, 256, tc::LAYOUT_NONE), IDESC_N64, false);
+            if (s == NCH - 1) tc::mma_commit(bar(B_D1_FULL));
+          }
           if (BWD) {
             if (a.node_adjoint)
               tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
@@ -519,15 +528,6 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
               tc::mma_bf16(TY + 16 * (s >> 1),
                            tc::smem_desc(base + SM::ring + (s - 1) * SLOT_BYTES + j * 2048, SLOT_BYTES, 1024, tc::LAYOUT_SW128),
                            tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, j != 0);
-          }
-          if (BWD && has_next) {
-            // G1 of the NEXT tile, slab by slab: E3 has just published slab s, i.e. read the last of the X columns of this
-            // slab, so they can take the next tile's e_hat . W1c^T now instead of after the whole of E3 (the backward
-            // kernel used to start every tile waiting ~1 k cycles for G1)
-            if (s == 0) { tc::mbar_wait(bar(B_EHAT_FULL), (uint32_t)((it + 1) & 1)); tc::fence_after_sync(); }
-            tc::mma_bf16(TX + (uint32_t)(64 * s), tc::smem_desc(base + SM::ehat, 128, 256, tc::LAYOUT_NONE),
-                         tc::smem_desc(base + SM::w1c + s * 2048, 128, 256, tc::LAYOUT_NONE), IDESC_N64, false);
-            if (s == NCH - 1) tc::mma_commit(bar(B_D1_FULL));
           }
         }
         tc::mma_commit(bar(B_SEG_FULL));
