@@ -33,8 +33,13 @@
 //       more than 16 receivers take a shared-memory loop.
 //   G4  ebar[edge, k] = abar . (W1c/2)  (N = 16, the W1c image read MN-major)
 //   E4  rbar_e += ubar_e u' + sum_k 2 ebar_k (u' g_k + u g'_k)
-// Segments that straddle tiles go through per-tile head/tail rows and k_segment_fixup_tc: no
-// floating-point atomics anywhere, results are bitwise reproducible.
+// Segments that straddle tiles go through per-tile head/tail rows and k_segment_fixup_tc. The only
+// reduction instruction is the one addition per edge and layer into rbar (E4), whose order is fixed by the
+// launch order, so results are bitwise reproducible.
+// Backward scheduling notes (from in-kernel clock64 timelines, profiles/r1e): G1 of the next tile is issued
+// slab by slab as E3 publishes (X columns released), ahead of that slab's G4 / GS; the spill copies are only
+// waited for once per tile, after that G1; the first layer runs with node_adjoint = false (no spill, no
+// segmented sum) and with row_index = species (P, Q are S-row tables).
 #include <cuda_fp16.h>
 #include "common.cuh"
 #include "edge.cuh"
@@ -597,7 +602,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         if (tid < D) segmented_store_tc<D>(ring, M.recv, BWD ? nullptr : M.w, a.rowptr, e0, tile, out, a.head, a.tail, tid);
         named_bar_sync(1, N_EPI_WARPS * 32);
       }
-      if (BWD && g == 0) {
+      // (column group 1: with the usual 3-4 receivers per tile only groups 0 and 2 have segment sums to read out above,
+      // so E4 goes to a group that would otherwise idle here while the others wait for it at the next barrier)
+      if (BWD && g == 1) {
         // ---- E4: rbar_e += ubar u' + sum_k ebar_k (u' g_k + u g'_k); G4 used the halved W1c image ----
         uint32_t eb[16];
         tmem_ld16_nowait(TY + tlane + 32u, eb);
