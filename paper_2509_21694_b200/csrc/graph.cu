@@ -90,7 +90,10 @@ __device__ __forceinline__ uint32_t pack_shift(int nx, int ny, int nz) {
   return ((uint32_t)(nx + 128) << 16) | ((uint32_t)(ny + 128) << 8) | (uint32_t)(nz + 128);
 }
 
-template <bool FILL>
+// MODE 0: count. MODE 1: fill the CSR rows (base = rowptr[i]). MODE 2: count AND write the keys of atom i to the
+// fixed-capacity row [i * cap, (i + 1) * cap) of a scratch buffer, so that the 27-cell search runs once; a row that
+// would overflow raises err_flag = 4 and the caller falls back to MODE 0 + MODE 1.
+template <int MODE>
 __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
                                                    const double* __restrict__ pos_s,
                                                    const int32_t* __restrict__ wrap_s,
@@ -100,7 +103,8 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
                                                    const int32_t* __restrict__ rowptr,
                                                    unsigned long long* __restrict__ keys,
                                                    unsigned long long* __restrict__ total,
-                                                   int* __restrict__ err_flag) {
+                                                   int* __restrict__ err_flag, int cap) {
+  constexpr bool FILL = MODE != 0;
   const int lane = threadIdx.x & 31;
   const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (i >= N) return;
@@ -111,7 +115,7 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
   const int c1 = (id / g.nc[2]) % g.nc[1];
   const int c0 = id / (g.nc[2] * g.nc[1]);
   int count = 0;
-  int64_t base = FILL ? (int64_t)rowptr[i] : 0;
+  int64_t base = MODE == 1 ? (int64_t)rowptr[i] : (MODE == 2 ? i * (int64_t)cap : 0);
   for (int o0 = -g.R[0]; o0 <= g.R[0]; ++o0) {
     const int t0 = c0 + o0, s0 = floordiv(t0, g.nc[0]), cc0 = t0 - s0 * g.nc[0];
     for (int o1 = -g.R[1]; o1 <= g.R[1]; ++o1) {
@@ -144,7 +148,7 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
             const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(rx, rx), __dmul_rn(ry, ry)), __dmul_rn(rz, rz));
             ok = d2 < g.rc2 && !(j == i && nx == 0 && ny == 0 && nz == 0);
             if (ok && (nx < -127 || nx > 127 || ny < -127 || ny > 127 || nz < -127 || nz > 127)) {
-              *err_flag = 1;
+              atomicOr(err_flag, 1);
               ok = false;
             }
             ps = pack_shift(nx, ny, nz);
@@ -152,7 +156,7 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
           const unsigned m = __ballot_sync(0xffffffffu, ok);
           if (FILL && ok) {
             const int rank = __popc(m & ((1u << lane) - 1u));
-            keys[base + count + rank] = ((unsigned long long)(uint32_t)j << 24) | ps;
+            if (MODE == 1 || count + rank < cap) keys[base + count + rank] = ((unsigned long long)(uint32_t)j << 24) | ps;
           }
           count += __popc(m);
         }
@@ -160,10 +164,22 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
       }
     }
   }
-  if (!FILL && lane == 0) {
+  if (MODE != 1 && lane == 0) {
     deg[i] = count;
     atomicAdd(total, (unsigned long long)count);
+    if (MODE == 2 && count > cap) atomicOr(err_flag, 4);
   }
+}
+
+// scratch rows of MODE 2 -> CSR rows
+__global__ void __launch_bounds__(256) k_compact_keys(int64_t N, int cap, const int32_t* __restrict__ rowptr,
+                                                      const unsigned long long* __restrict__ scratch,
+                                                      unsigned long long* __restrict__ keys) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= N) return;
+  const int lo = rowptr[i], len = rowptr[i + 1] - lo;
+  for (int t = lane; t < len; t += 32) keys[lo + t] = scratch[i * (int64_t)cap + t];
 }
 
 // ---- per-row sort of 64-bit keys (one warp per row, bitonic in shared memory) ------------------
@@ -375,7 +391,8 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
   double *frac = nullptr, *pos_s = nullptr;
   int32_t *wrap = nullptr, *cellid = nullptr, *cell_count = nullptr, *cell_start = nullptr, *order = nullptr,
           *wrap_s = nullptr, *cellid_s = nullptr, *deg = nullptr;
-  unsigned long long *keys = nullptr, *total = nullptr;
+  unsigned long long *keys = nullptr, *total = nullptr, *scratch = nullptr;
+  int cap = 0;
   int* err_flag = nullptr;
 #define G_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
   G_TRY(ctx->alloc(&frac, 3 * N)); G_TRY(ctx->alloc(&wrap, 3 * N)); G_TRY(ctx->alloc(&cellid, N));
@@ -400,8 +417,18 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
     k_gather_sorted<<<nblk(N, 256), 256, 0, st>>>(order, N, pos_dev, frac, wrap, species_dev, cellid, pos_s,
                                                   G->frac, wrap_s, G->species, cellid_s);
     cudaMemcpyAsync(G->perm, order, sizeof(int32_t) * N, cudaMemcpyDeviceToDevice, st);
-    k_neighbors<false><<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, wrap_s, cellid_s, cell_start, deg, nullptr,
-                                                          nullptr, total, err_flag);
+    // one search pass when a capped scratch row per atom is affordable: cap = 1.5 x the mean degree + 32
+    const double nbar = 4.18879020478639 * r_cut * r_cut * r_cut * (double)N / vol;
+    cap = (int)(1.5 * nbar + 32.0);
+    cap = (cap + 7) & ~7;
+    if ((double)N * cap * 8.0 <= 2.0e9 && ctx->alloc(&scratch, (size_t)N * cap) == MLIP_OK) {
+      k_neighbors<2><<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, wrap_s, cellid_s, cell_start, deg, nullptr,
+                                                        scratch, total, err_flag, cap);
+    } else {
+      scratch = nullptr;
+      k_neighbors<0><<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, wrap_s, cellid_s, cell_start, deg, nullptr,
+                                                        nullptr, total, err_flag, 0);
+    }
     ctx->launches += 4;
   }
   unsigned long long total_h = 0;
@@ -412,7 +439,7 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
     ctx->set_error(std::string("graph build (count): ") + cudaGetErrorString(cudaGetLastError()));
     return fail(MLIP_ERR_CUDA);
   }
-  if (err_h == 1) { ctx->set_error("image shift outside [-127,127]"); return fail(MLIP_ERR_OVERFLOW); }
+  if (err_h & 1) { ctx->set_error("image shift outside [-127,127]"); return fail(MLIP_ERR_OVERFLOW); }
   if (total_h >= (1ull << 31)) { ctx->set_error("number of edges >= 2^31"); return fail(MLIP_ERR_OVERFLOW); }
   const int64_t E = (int64_t)total_h;
   G->E = E;
@@ -420,8 +447,11 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
   G_TRY(ctx->alloc(&keys, E)); G_TRY(ctx->alloc(&G->recv, E)); G_TRY(ctx->alloc(&G->send, E));
   G_TRY(ctx->alloc(&G->shift, E)); G_TRY(ctx->alloc(&G->rev, E)); G_TRY(ctx->alloc(&G->rvec, E));
   if (E > 0) {
-    k_neighbors<true><<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, wrap_s, cellid_s, cell_start, nullptr,
-                                                         G->rowptr, keys, nullptr, err_flag);
+    if (scratch && !(err_h & 4))
+      k_compact_keys<<<nblk(N * 32, 256), 256, 0, st>>>(N, cap, G->rowptr, scratch, keys);
+    else
+      k_neighbors<1><<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, wrap_s, cellid_s, cell_start, nullptr,
+                                                        G->rowptr, keys, nullptr, err_flag, 0);
     k_sort_rows<<<nblk(N, 4), 128, 0, st>>>(N, G->rowptr, keys);
     k_finalize_edges<<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, G->rowptr, keys, G->recv, G->send, G->shift,
                                                         G->rvec);
@@ -430,7 +460,7 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
   }
   ctx->free(frac); ctx->free(wrap); ctx->free(cellid); ctx->free(cell_count); ctx->free(cell_start);
   ctx->free(order); ctx->free(pos_s); ctx->free(wrap_s); ctx->free(cellid_s); ctx->free(deg);
-  ctx->free(total); ctx->free(keys);
+  ctx->free(total); ctx->free(keys); ctx->free(scratch);
   cudaError_t e = cudaGetLastError();
   ctx->free(err_flag);
   if (e != cudaSuccess) { ctx->set_error(std::string("graph build: ") + cudaGetErrorString(e)); return fail(MLIP_ERR_CUDA); }

@@ -90,3 +90,14 @@ def test_partition_sizes_match_oracle():
         for i, (owned, ext, hops) in zip(info, oparts):
             assert i["n_owned"] == len(owned) and i["n_ext"] == len(ext)
             assert i["n_edges"] == len(O.induced_subgraph(graph, ext, len(s.pos))[0])
+
+
+def test_edge_list_clustered_atoms_overflow_fallback():
+    """A dense cluster in a large, mostly empty box: the per-atom scratch rows of the one-pass neighbour search are sized
+    from the MEAN density and overflow here, so the builder must fall back to count + fill -- same bit-exact list."""
+    rng = np.random.default_rng(23)
+    pts = rng.normal(0.0, 2.5, (400, 3)) + 30.0
+    far = rng.uniform(0, 60.0, (50, 3))
+    s = System(np.concatenate([pts, far]), np.eye(3) * 60.0, rng.integers(0, 4, 450).astype(np.int32))
+    n = _compare(s, 5.0)
+    assert n > 450 * 60   # mean degree far above the scratch capacity of 1.5 * (4/3 pi r^3 N / V) + 32 ~ 33
