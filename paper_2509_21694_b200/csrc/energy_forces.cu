@@ -328,8 +328,9 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
       a = GemmArgs(); from_cbar(a); a.B = bf ? (const void*)W.V1aT_bf : (const void*)W.V1aT;
       a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d; a.n = nr; a.N = d;
       W_TRY(gemm(ctx, a));
-      cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
     }
+    // (the fp32 edge kernel always accumulates its Pbar sums, so its buffer is cleared for the first layer too)
+    if (node_adjoint || !bf) cudaMemsetAsync(Pbar, 0, sizeof(float) * ns * d, st);
     set_layer(l);
     ea.E = Er; ea.n = nr; ea.node_adjoint = bf ? node_adjoint : true;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
