@@ -829,20 +829,26 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
   if (warp == 0) tc::tmem_dealloc<SM::tmem_cols>(tmem);
 }
 
-// out[i] = tail[t] + head[t+1] + ... for the segment that starts in tile t and continues beyond it
-__global__ void k_segment_fixup_tc(int64_t E, int D, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ recv,
-                                   const float* __restrict__ head, const float* __restrict__ tail, float* __restrict__ out) {
-  const int64_t t = blockIdx.x;
+// out[i] = tail[t] + head[t+1] + ... for the segment that starts in tile t and continues beyond it.
+// D/4 threads per tile (one float4 of channels each), 1024/D tiles per 256-thread block.
+__global__ void __launch_bounds__(256) k_segment_fixup_tc(int64_t E, int D, int64_t n_tiles, const int32_t* __restrict__ rowptr,
+                                                          const int32_t* __restrict__ recv, const float* __restrict__ head,
+                                                          const float* __restrict__ tail, float* __restrict__ out) {
+  const int tpt = D >> 2;  // threads per tile
+  const int64_t t = (int64_t)blockIdx.x * (blockDim.x / tpt) + threadIdx.x / tpt;
+  const int c = (threadIdx.x % tpt) * 4;
+  if (t >= n_tiles) return;
   const int64_t e0 = t * TE, e1 = e0 + TE;
   if (e1 >= E) return;
   const int i = recv[e1 - 1];
   const int64_t s0 = rowptr[i], s1 = rowptr[i + 1];
   if (!(s1 > e1 && s0 >= e0)) return;
-  for (int c = threadIdx.x; c < D; c += blockDim.x) {
-    float sum = tail[(size_t)t * D + c];
-    for (int64_t t2 = t + 1; t2 * TE < s1; ++t2) sum += head[(size_t)t2 * D + c];
-    out[(size_t)i * D + c] = sum;
+  float4 sum = *reinterpret_cast<const float4*>(tail + (size_t)t * D + c);
+  for (int64_t t2 = t + 1; t2 * TE < s1; ++t2) {
+    const float4 h = *reinterpret_cast<const float4*>(head + (size_t)t2 * D + c);
+    sum.x += h.x; sum.y += h.y; sum.z += h.z; sum.w += h.w;
   }
+  *reinterpret_cast<float4*>(out + (size_t)i * D + c) = sum;
 }
 
 // Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled f16 tile images written by E3
@@ -892,8 +898,9 @@ int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   k_edge_tc<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
   ctx->launches++;
   if (!BWD || a.node_adjoint) {
-    k_segment_fixup_tc<<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
-                                                                               BWD ? a.Pbar : a.m);
+    const int64_t tiles_per_block = 256 / (D / 4);
+    k_segment_fixup_tc<<<(unsigned)((tiles + tiles_per_block - 1) / tiles_per_block), 256, 0, ctx->stream>>>(
+        a.E, D, tiles, a.rowptr, a.recv, a.head, a.tail, BWD ? a.Pbar : a.m);
     ctx->launches++;
   }
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
