@@ -80,14 +80,20 @@ def oracle_sample(cfg_number: int, n_cells: int):
     cfg = make_config(cfg_number, n_cells_override=n_cells)
     s, m = cfg.system, cfg.model
     om = O.parse_weights(m.n_species, m.d, m.n_rbf, m.L_max, m.r_cut, m.agg_scale, cfg.weights)
+    graph = O.neighbor_list(s.pos, s.cell, m.r_cut)
     t0 = time.perf_counter()
     O.energy_forces(om, cfg.L, s.pos, s.cell, s.species)
     dt = time.perf_counter() - t0
-    return len(s.pos) / dt, len(s.pos), dt, len(os.sched_getaffinity(0))
+    return len(s.pos) / dt, len(s.pos), dt, len(os.sched_getaffinity(0)), len(graph[0]) * cfg.L / dt
 
 
-def sample_cells(cfg_number: int) -> int:
-    return {1: 3, 2: 5, 3: 4, 4: 6}.get(cfg_number, 4)
+def sample_cells(cfg_number: int, n_evaluations: int = 1) -> int:
+    """fcc cells per axis of the oracle's bounded sample: 10-30 s of host time per evaluation on ~16 cores when it is
+    evaluated once (the cpu_baseline leg) or a handful of times, about 4 s each when `--impl reference` repeats it
+    for many steps (the whole run has to end within a few minutes)."""
+    if n_evaluations > 8:
+        return {1: 3, 2: 5, 3: 4, 4: 6}.get(cfg_number, 4)
+    return {1: 3, 2: 8, 3: 6, 4: 12}.get(cfg_number, 4)
 
 
 def run_reference(args):
@@ -95,13 +101,13 @@ def run_reference(args):
     if rank != 0:
         return
     from synth_inputs import make_config
-    nc = sample_cells(args.config)
+    nc = sample_cells(args.config, args.warmup + args.steps)
     cfg_full = make_config(args.config, with_weights=False, n_cells_override=args.n_cells)
     vals = []
     n_atoms = 0
     cores = 0
     for i in range(args.warmup + args.steps):
-        v, n_atoms, dt, cores = oracle_sample(args.config, nc)
+        v, n_atoms, dt, cores, _ = oracle_sample(args.config, nc)
         if i >= args.warmup:
             vals.append((v, dt))
     value = float(np.mean([v for v, _ in vals]))
@@ -183,16 +189,45 @@ class ClockSampler:
 # the CUDA path
 # ------------------------------------------------------------------------------------------
 def ncu_traffic(config: int, group: str):
-    """DRAM bytes per launch of a kernel group from the committed ncu --set full capture (profiles/*_traffic.csv,
-    newest round last), or None when no capture of this config exists."""
+    """(DRAM bytes per launch, capture label) of a kernel group from the committed ncu --set full captures
+    (profiles/*_traffic.csv, newest round last; the label names the commit the capture was made on), or (None, None)
+    when no capture of this config exists."""
     import csv
     import glob
-    best = None
+    best, label = None, None
     for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_traffic.csv"))):
         for row in csv.DictReader(open(path)):
             if int(row["config"]) == config and row["kernel_group"] == group:
                 best = float(row["dram_bytes_per_launch"])
-    return best
+                label = f"{os.path.basename(path)} @ {row.get('commit') or 'commit not recorded'}"
+    return best, label
+
+
+MUFU_PER_SM_PER_CLK = 16   # MUFU (tanh/ex2) results per clock and SM: 4 per SM sub-partition (B300_MICROARCH.md pipes)
+
+
+def edge_rooflines(name, ms, edge_layers, launches, d, n_rbf, pk, sm_mhz, spill_layers=0):
+    """The three rooflines SURVEY.md 8(d) asks for on the fused edge kernels (they sit at the ridge): tensor pipe, MUFU
+    and HBM, each as algorithmic work / measured time / peak.
+      tensor  2 d n_rbf + 2 d^2 flop per edge-layer and direction (the reverse pass EXECUTES twice that: recompute)
+      MUFU    2 d transcendental results per edge-layer and direction (one tanh per SiLU; reverse pass: the recomputed ones)
+      HBM     sender row 2 d B + 28 B metadata per edge-layer; reverse pass adds the 2 d B abar spill of the layers with a
+              node adjoint and 4 B of rbar"""
+    if ms <= 0:
+        return []
+    t = ms * 1e-3
+    flop = edge_layers * flops_edge_layer(d, n_rbf)
+    mufu = edge_layers * 2.0 * d
+    hbm = edge_layers * (2.0 * d + 28.0) + spill_layers * 2.0 * d + (4.0 * edge_layers if name == "edge_bwd" else 0.0)
+    mufu_peak = 148 * MUFU_PER_SM_PER_CLK * sm_mhz * 1e6
+    return [
+        {"kernel": name, "bound": "tensor", "achieved": flop / t / 1e12, "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+         "frac": flop / t / 1e12 / pk["bf16_tflops_sustained"], "launches_per_step": launches},
+        {"kernel": name, "bound": "mufu", "achieved": mufu / t / 1e12, "peak": mufu_peak / 1e12, "unit": "Tresult/s",
+         "frac": mufu / t / mufu_peak, "peak_source": f"derived: 148 SM x 16 /clk x {sm_mhz:.0f} MHz (median SM clock of the run)"},
+        {"kernel": name, "bound": "hbm", "achieved": hbm / t / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s",
+         "frac": hbm / t / 1e9 / pk["hbm_gbs"]},
+    ]
 
 
 def flops_edge_layer(d: int, n_rbf: int) -> float:
@@ -239,7 +274,7 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # 256 MiB > 126 MB L2
     info = {}
 
-    def step():
+    def step(collect=False):
         g = mlip.Graph(ctx, pos, s.cell, species, m.r_cut)
         part = mlip.Partition(ctx, g, cfg.halo, grid=cfg.grid) if partitioned else None
         if world > 1:
@@ -247,11 +282,12 @@ def run_ours(args):
             all_reduce_results(E, F)
         else:
             E, F, _ = mlip.energy_forces(ctx, model, cfg.L, g, part, prec, want_atom_energy=False, out=out)
-        info["edges"] = g.num_edges
-        info["subs"] = part.info() if part is not None else [dict(n_owned=N, n_ext=N, n_edges=g.num_edges)]
-        # edge evaluations per layer and sub-domain (per-layer active sets: mlip_part_layer_info)
-        info["layers"] = (part.layer_info(cfg.L) if part is not None
-                          else [[dict(n_recv=N, n_send=N, n_edges=g.num_edges)] * cfg.L])
+        if collect:   # sizes for the roofline arithmetic: only in the separate profiling pass, never in the timed region
+            info["edges"] = g.num_edges
+            info["subs"] = part.info() if part is not None else [dict(n_owned=N, n_ext=N, n_edges=g.num_edges)]
+            # edge evaluations per layer and sub-domain (per-layer active sets: mlip_part_layer_info)
+            info["layers"] = (part.layer_info(cfg.L) if part is not None
+                              else [[dict(n_recv=N, n_send=N, n_edges=g.num_edges)] * cfg.L])
         return E, F
 
     def barrier():
@@ -266,7 +302,6 @@ def run_ours(args):
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
-    ctx.profile(True)
     launches0 = ctx.launches
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     for a, b in ev:
@@ -276,9 +311,17 @@ def run_ours(args):
         b.record()
     barrier()
     launches = ctx.launches - launches0
+    clocks = sampler.stop()
+    # separate pass with the per-kernel-group event timers on (they cost a few event records per launch group, so they
+    # stay out of the timed region above): kernel_ms_per_step and the roofline numerators come from here
+    prof_steps = max(1, min(args.steps, 3))
+    ctx.profile(True)
+    for _ in range(prof_steps):
+        flush.zero_()
+        step(collect=True)
+    barrier()
     groups = ctx.profile_read()
     ctx.profile(False)
-    clocks = sampler.stop()
     ms = torch.tensor([sum(a.elapsed_time(b) for a, b in ev) / args.steps], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
@@ -315,7 +358,8 @@ def run_ours(args):
     edges_total = sum(x["n_edges"] for x in info["subs"][rank::world]) if world > 1 else sum(x["n_edges"] for x in info["subs"])
     mine = info["layers"][rank::world] if world > 1 else info["layers"]
     edge_layers = sum(r["n_edges"] for rows in mine for r in rows)   # edge-layer evaluations actually launched
-    per_step = {k: v[0] / args.steps for k, v in groups.items()}
+    per_step = {k: v[0] / prof_steps for k, v in groups.items()}
+    n_launch = {k: v[1] / prof_steps for k, v in groups.items()}
     dom = max(("edge_fwd", "edge_bwd"), key=lambda k: per_step[k])
     flop = edge_layers * flops_edge_layer(m.d, m.n_rbf)
     achieved = flop / (per_step[dom] * 1e-3) / 1e12 if per_step[dom] > 0 else 0.0
@@ -323,25 +367,51 @@ def run_ours(args):
         bound, peak, peak_src = "tensor", pk["bf16_tflops_sustained"], pk["_source"] + " (sustained cuBLAS bf16)"
     else:
         bound, peak, peak_src = "alu", ALU_FP32_TFLOPS, "derived: 148 SM x 128 FMA x 2 x 1.965 GHz"
+    traffic, traffic_capture = ncu_traffic(args.config, dom)
     roofline = {"kernel": dom, "bound": bound, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(args.config, dom), "traffic_unit": "dram bytes per launch (ncu)",
-                "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": traffic, "traffic_unit": "dram bytes per launch (ncu)",
+                "traffic_capture": traffic_capture, "peak_source": peak_src,
                 "algorithmic_flop_per_step": flop, "kernel_ms_per_step": per_step[dom],
                 "executed_over_algorithmic": 2.0 if dom == "edge_bwd" else 1.0}
+    # every binding unit of the big kernel groups (SURVEY.md 8(d) "report all three" for the fused edge kernels)
+    rooflines = []
+    if prec_name == "bf16":
+        sm_mhz = clocks.get("sm_mhz") or pk.get("sm_max_mhz", 1965.0)
+        # layers with a node adjoint (all but the first) spill abar and are read back by the sender-side gather
+        spill_layers = sum(r["n_edges"] for rows in mine for r in rows[1:])
+        rooflines += edge_rooflines("edge_fwd", per_step["edge_fwd"], edge_layers, n_launch["edge_fwd"], m.d, m.n_rbf, pk, sm_mhz)
+        rooflines += edge_rooflines("edge_bwd", per_step["edge_bwd"], edge_layers, n_launch["edge_bwd"], m.d, m.n_rbf, pk, sm_mhz,
+                                    spill_layers)
+        if per_step["gather_rev"] > 0:
+            send_rows = sum(r["n_send"] for rows in mine for r in rows[1:])
+            gb = (spill_layers * (2.0 * m.d + 4.0) + send_rows * 2.0 * m.d) / 1e9
+            rooflines.append({"kernel": "gather_rev", "bound": "hbm", "achieved": gb / (per_step["gather_rev"] * 1e-3),
+                              "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gb / (per_step["gather_rev"] * 1e-3) / pk["hbm_gbs"]})
+        if per_step["node_gemm"] > 0:
+            # 10 d^2 flop per atom-layer forward (P, Q, V1, V2) and the same again in the reverse pass, + readout 2 d^2 x 2
+            atom_layers = sum(r["n_send"] for rows in mine for r in rows)
+            nflop = atom_layers * 20.0 * m.d * m.d
+            rooflines.append({"kernel": "node_gemm", "bound": "tensor", "achieved": nflop / (per_step["node_gemm"] * 1e-3) / 1e12,
+                              "peak": pk["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                              "frac": nflop / (per_step["node_gemm"] * 1e-3) / 1e12 / pk["bf16_tflops_sustained"]})
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         nc = sample_cells(args.config)
-        v, n_s, dt, cores = oracle_sample(args.config, nc)
+        v, n_s, dt, cores, el_rate = oracle_sample(args.config, nc)
         cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"same recipe at fcc {nc}^3 ({n_s} atoms), unpartitioned, one evaluation ({dt:.1f} s)"}
+               "sample": f"same recipe at fcc {nc}^3 ({n_s} atoms), unpartitioned, one evaluation ({dt:.1f} s)",
+               "edge_layers_per_s": el_rate,
+               # the partitioned workload evaluates edge_layers / N edge-layers per atom (halo included)
+               "extrapolated_to_workload": el_rate * N / max(edge_layers, 1),
+               "extrapolated_note": "sample edge-layers/s x N / edge-layers evaluated per step of this workload"}
 
     n_own = [x["n_owned"] for x in info["subs"]]
     n_ext = [x["n_ext"] for x in info["subs"]]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-        "dtype": "bf16" if prec_name == "bf16" else "f32", "data": "synthetic",
+        "dtype": "f16/bf16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg, N), "n_atoms": N, "n_edges": info["edges"],
                    "sub_domains": len(info["subs"]), "edges_in_subgraphs": int(edges_total),
                    "edge_layers_evaluated_per_step": int(edge_layers), "active_sets": not args.no_active_sets,
@@ -349,7 +419,8 @@ def run_ours(args):
                    "l2": "256 MiB buffer rewritten between timed iterations; working set also exceeds the 126 MB L2"
                    if N > 200000 else "256 MiB buffer rewritten between timed iterations",
                    "step": "mlip_build_graph + mlip_partition_grid + mlip_energy_forces, inputs resident in HBM"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "rooflines": rooflines,
+        "cpu_baseline": cpu,
         "kernel_ms_per_step": per_step, "energy": E_val, "force_sum": F_sum,
     }
     print(json.dumps(line), flush=True)

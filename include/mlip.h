@@ -42,9 +42,21 @@ typedef enum {
   MLIP_ERR_HALO_TOO_SMALL = -3,  /* halo < L*r_cut: refused rather than silently wrong forces */
   MLIP_ERR_OUT_OF_MEMORY = -4,
   MLIP_ERR_OVERFLOW = -5,        /* number of edges >= 2^31 or image shift outside [-127,127] */
-  MLIP_ERR_CUDA = -6
+  MLIP_ERR_CUDA = -6,
+  MLIP_ERR_NUMERIC = -7          /* non-finite energy or force: the 16-bit path left the IEEE-half range (see MLIP_BF16) */
 } mlip_status;
 
+/* Arithmetic of the contractions.
+ *   MLIP_FP32  fp32 CUDA-core FMA everywhere.
+ *   MLIP_BF16  16-bit tensor-core operands with fp32 accumulation (tcgen05, accumulators in TMEM). The name follows
+ *              BASELINE.json ("bf16 GEMM inputs"); what runs is: bf16 operands in the node contractions, IEEE HALF (f16)
+ *              operands in the fused edge kernels -- same tensor-core rate and bytes as bf16, three more mantissa
+ *              bits, and packed f16x2 epilogue arithmetic. Range contract of the f16 tensors (halved pre-activations
+ *              P, Q, a, p; messages; the adjoints mbar, pbar, abar): magnitudes must stay below 65504. The reverse
+ *              pass is scaled by a power of two chosen per sub-domain from max|d E / d o| (removed again when the
+ *              forces are assembled), so small adjoints do not fall into the f16 subnormals. A value that leaves
+ *              the range becomes inf/NaN, reaches E or F, and is reported as MLIP_ERR_NUMERIC by the next
+ *              synchronising call (mlip_step_host, mlip_md_*) or by mlip_ctx_status -- never a silent wrong number. */
 enum { MLIP_FP32 = 0, MLIP_BF16 = 1 };
 
 typedef struct mlip_ctx mlip_ctx;
@@ -65,9 +77,12 @@ typedef struct {
   int32_t L_max;      /* M: number of message-passing layers stored in the blob */
   float r_cut;        /* local cutoff r_c in Angstrom */
   float agg_scale;    /* alpha multiplying the neighbour sum (reading R7) */
-  int32_t flags;      /* must be 0 (bit 0 reserved for the three-body variant) */
-  int32_t reserved[3];
+  int32_t flags;      /* bit 0 (MLIP_FLAG_THREE_BODY): three-body variant, see mlip_model_load; other bits must be 0 */
+  int32_t n_rbf3;     /* three-body variant: radial functions of the angle basis, must be 4 (else 0) */
+  int32_t l_max;      /* three-body variant: largest l of Y_l^0(cos theta), must be 3 (else 0) */
+  float r_cut3;       /* three-body variant: cutoff r_3 <= r_cut of the edge pairs, Angstrom (else 0) */
 } mlip_model_header;
+#define MLIP_FLAG_THREE_BODY 1
 
 /* Number of floats the weight blob must hold for a header. */
 size_t mlip_model_num_weights(const mlip_model_header* h);
@@ -77,6 +92,11 @@ size_t mlip_model_num_weights(const mlip_model_header* h);
 int mlip_ctx_create(int device, void* stream, mlip_ctx** out);
 void mlip_ctx_destroy(mlip_ctx* ctx);
 const char* mlip_last_error(const mlip_ctx* ctx);
+/* Synchronises the context stream and returns (and clears) the status of the asynchronous work enqueued so far:
+ * MLIP_OK, MLIP_ERR_NUMERIC (non-finite energy or force, see MLIP_BF16), MLIP_ERR_CUDA. mlip_energy_forces* are
+ * asynchronous and cannot report such a condition themselves; calls that synchronise anyway (mlip_step_host,
+ * mlip_md_*) return it directly. */
+int mlip_ctx_status(mlip_ctx* ctx);
 
 /* Load a weight blob (HOST pointer, fp32, `n` floats, copied). Order, every matrix row-major
  * [out,in]:  T[S,d], E0[S], then for each of the L_max layers
@@ -140,8 +160,8 @@ void mlip_part_destroy(mlip_part* p);
  * sub-domains of the gradient of that sub-domain's root energy w.r.t. ALL of its atoms
  * (reading R1). part == NULL evaluates the whole box as one domain.
  * Sub-domains are evaluated one after another on the context stream.
- *   precision       MLIP_FP32 (fp32 CUDA-core contractions) or MLIP_BF16 (bf16 tensor-core
- *                   contractions with fp32 accumulation; requires d = 256 or 128)
+ *   precision       MLIP_FP32 (fp32 CUDA-core contractions) or MLIP_BF16 (16-bit tensor-core contractions
+ *                   with fp32 accumulation, see the enum; requires d = 256 or 128)
  *   energy_dev      [1] float64, device
  *   forces_dev      [n_atoms,3] float32, device, caller's atom numbering (eV/Angstrom)
  *   atom_energy_dev [n_atoms] float32, device, or NULL

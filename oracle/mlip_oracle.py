@@ -18,6 +18,10 @@ box, PAPER.md:23,151):
   O6  partition into spatial bins + halo; sum ROOT-node energies, sum the
       gradients of root energies w.r.t. ALL sub-graph atoms
 
+  O7  three-body (angle) variant of the layers, BASELINE.json config 5: the paper's workhorse model MatterSim is an
+      M3GNet-type network but the paper gives no equations; the definition is the proposal of
+      SURVEY.md 8(f) NEXT-1 (reading R17), written out at `three_body_terms`.
+
 The method (prune + partition + halo) reaches exactly the unpartitioned result
 (PAPER.md:165), so `energy_forces` IS the definition and `energy_forces_partitioned`
 restates the assembly rule. Pins (tests/test_oracle_*.py): brute-force O(N^2) neighbour
@@ -55,12 +59,17 @@ class Model:
     bo: np.ndarray
     wo: np.ndarray
     bE: float
+    r_cut3: float = 0.0   # > 0: three-body variant (O7); layers then also hold G[16,d], g[16], W3[d,16]
 
 
-def parse_weights(n_species, d, n_rbf, L_max, r_cut, agg_scale, blob) -> Model:
+N_ANGLE = 16  # (l_max + 1) * n_rbf3 = 4 * 4 angle-basis functions of the three-body variant, index 4 l + n
+
+
+def parse_weights(n_species, d, n_rbf, L_max, r_cut, agg_scale, blob, r_cut3=0.0) -> Model:
     """Blob order of include/mlip.h: T[S,d], E0[S], per layer W1[d,2d+k] (columns: receiver h_i,
-    sender h_j, e_hat), b1, W2[d,d], b2, V1[d,2d] (columns: h, m), c1, V2[d,d], c2; then
-    Wo[d,d], bo, wo, b_E. fp32 values are promoted to float64 unrounded (reading R15)."""
+    sender h_j, e_hat), b1, W2[d,d], b2, V1[d,2d] (columns: h, m), c1, V2[d,d], c2 (and, three-body variant
+    r_cut3 > 0, G[16,d], g[16], W3[d,16]); then Wo[d,d], bo, wo, b_E. fp32 values are promoted to float64
+    unrounded (reading R15)."""
     w = np.asarray(blob, dtype=np.float64)
     pos = 0
 
@@ -77,9 +86,12 @@ def parse_weights(n_species, d, n_rbf, L_max, r_cut, agg_scale, blob) -> Model:
     for _ in range(L_max):
         layers.append(dict(W1=take(d, 2 * d + n_rbf), b1=take(d), W2=take(d, d), b2=take(d),
                            V1=take(d, 2 * d), c1=take(d), V2=take(d, d), c2=take(d)))
+        if r_cut3 > 0.0:
+            layers[-1].update(G=take(N_ANGLE, d), g=take(N_ANGLE), W3=take(d, N_ANGLE))
     Wo = take(d, d); bo = take(d); wo = take(d); bE = float(take(1)[0])
     assert pos == w.size, "weight blob size does not match the header"
-    return Model(n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), T, E0, layers, Wo, bo, wo, bE)
+    assert 0.0 <= r_cut3 <= r_cut, "three-body cutoff must not exceed the two-body one (halo stays L r_cut)"
+    return Model(n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), T, E0, layers, Wo, bo, wo, bE, float(r_cut3))
 
 
 # --------------------------------------------------------------------------------------
@@ -214,6 +226,120 @@ def dsilu(x):
 
 
 # --------------------------------------------------------------------------------------
+# O7 three-body (angle) term, SURVEY.md 8(f) NEXT-1 (reading R17; PAPER.md:91,119,131 name the model family only)
+# --------------------------------------------------------------------------------------
+def envelope3(r, r3):
+    """u3(r) = (cos(pi r / r3) + 1)/2 for r < r3, else 0; and u3'(r)."""
+    x = np.pi * r / r3
+    inside = r < r3
+    return np.where(inside, 0.5 * (np.cos(x) + 1.0), 0.0), np.where(inside, -(0.5 * np.pi / r3) * np.sin(x), 0.0)
+
+
+def rbf3(r, r3):
+    """g3_n(r) = exp(-gamma3 (r - n r3/3)^2), n = 0..3, gamma3 = 1/(2 (r3/3)^2); returns g [T,4], g' [T,4]."""
+    delta = r3 / 3.0
+    gamma = 0.5 / (delta * delta)
+    diff = r[:, None] - (np.arange(4, dtype=np.float64) * delta)[None, :]
+    g = np.exp(-gamma * diff * diff)
+    return g, -2.0 * gamma * diff * g
+
+
+def y_l0(c):
+    """Y_l^0(c) = sqrt((2l+1)/(4 pi)) P_l(c), l = 0..3 (P0 = 1, P1 = c, P2 = (3c^2-1)/2, P3 = (5c^3-3c)/2) and
+    d/dc; returns [T,4], [T,4]."""
+    norm = np.sqrt((2.0 * np.arange(4) + 1.0) / (4.0 * np.pi))
+    P = np.stack([np.ones_like(c), c, 0.5 * (3.0 * c * c - 1.0), 0.5 * (5.0 * c ** 3 - 3.0 * c)], axis=1)
+    dP = np.stack([np.zeros_like(c), np.ones_like(c), 3.0 * c, 0.5 * (15.0 * c * c - 3.0)], axis=1)
+    return P * norm, dP * norm
+
+
+TRIPLET_CHUNK = 1 << 21
+
+
+def triplet_chunks(recv, short, n_atoms):
+    """Ordered pairs (e, e') of DISTINCT in-edges of the same receiver, both shorter than r3 (`short`), yielded in
+    chunks of whole receivers. e != e' as edges: the same neighbour through two different images counts twice."""
+    se = np.nonzero(short)[0]
+    se = se[np.argsort(recv[se], kind="stable")]
+    rc = recv[se]
+    counts = np.bincount(rc, minlength=n_atoms)
+    start = np.cumsum(counts) - counts           # position in `se` of the first short edge of every receiver
+    per_recv = counts * counts
+    lo = 0
+    while lo < n_atoms:
+        hi, tot = lo, 0
+        while hi < n_atoms and (tot == 0 or tot + per_recv[hi] <= TRIPLET_CHUNK):
+            tot += per_recv[hi]
+            hi += 1
+        a, b = start[lo], (start[hi - 1] + counts[hi - 1])
+        if b > a:
+            m = counts[rc[a:b]]
+            pos_e = np.repeat(np.arange(a, b), m)
+            off = np.arange(len(pos_e)) - np.repeat(np.cumsum(m) - m, m)
+            pos_p = np.repeat(start[rc[a:b]], m) + off
+            keep = pos_p != pos_e
+            yield se[pos_e[keep]], se[pos_p[keep]]
+        lo = hi
+
+
+def _unit_vectors(rvec, r):
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return np.where(r[:, None] > 0.0, rvec / r[:, None], 0.0)   # rhat := 0 at r = 0 (reading R13)
+
+
+def _angle_basis(model, te, tp, rhat, r):
+    """Per triplet (e, e'): c = rhat_e . rhat_e', the 16 basis values Y_l(c) g3_n(r_e') at index 4 l + n and the
+    pieces their derivatives are assembled from."""
+    c = np.einsum("ta,ta->t", rhat[te], rhat[tp])
+    Y, dY = y_l0(c)
+    g3, dg3 = rbf3(r[tp], model.r_cut3)
+    Y16, dY16 = np.repeat(Y, 4, axis=1), np.repeat(dY, 4, axis=1)
+    g16, dg16 = np.tile(g3, (1, 4)), np.tile(dg3, (1, 4))
+    return c, Y16, dY16, g16, dg16
+
+
+def three_body_terms(model, lay, h, recv, send, rvec, r):
+    """t_e = u3(r_e) S_e,  S_e = sum over in-edges e' = (i <- k) != e of the same receiver with r_e' < r3 of
+           u3(r_e') [Y_l^0(cos theta_ee') g3_n(r_e')]_{4l+n} * sigma(G h_k + g)          (16 components),
+    zero for edges with r_e >= r3; cos theta_ee' = rhat_e . rhat_e' is the angle at the receiver. The term enters the
+    first edge linear as W3 t_e. Returns t [E,16], S [E,16], z [N,16]."""
+    N = len(h)
+    z = expit(h @ lay["G"].T + lay["g"])
+    u3, _ = envelope3(r, model.r_cut3)
+    rhat = _unit_vectors(rvec, r)
+    S = np.zeros((len(recv), N_ANGLE))
+    for te, tp in triplet_chunks(recv, r < model.r_cut3, N):
+        _, Y16, _, g16, _ = _angle_basis(model, te, tp, rhat, r)
+        S += _scatter_matrix(te, len(recv)) @ (u3[tp, None] * Y16 * g16 * z[send[tp]])
+    return u3[:, None] * S, S, z
+
+
+def three_body_backward(model, lay, h, recv, send, rvec, r, tbar, S, z):
+    """Reverse mode of three_body_terms given tbar = d(.)/d t_e [E,16]: returns the contributions to rbar [E] (through
+    u3(r_e), u3(r_e') and g3_n(r_e')), to the per-edge VECTOR gradient gvec [E,3] (through cos theta, with
+    d c / d r_e = (rhat_e' - c rhat_e) / r_e) and to hbar [N,d] (through the gates sigma(G h_k + g))."""
+    N, E = len(h), len(recv)
+    u3, du3 = envelope3(r, model.r_cut3)
+    rhat = _unit_vectors(rvec, r)
+    with np.errstate(divide="ignore"):
+        inv_r = np.where(r > 0.0, 1.0 / r, 0.0)
+    rbar = du3 * np.sum(tbar * S, axis=1)
+    tau = tbar * u3[:, None]                       # adjoint of S_e
+    gvec = np.zeros((E, 3))
+    zbar = np.zeros((N, N_ANGLE))
+    for te, tp in triplet_chunks(recv, r < model.r_cut3, N):
+        c, Y16, dY16, g16, dg16 = _angle_basis(model, te, tp, rhat, r)
+        tz = tau[te] * z[send[tp]]
+        rbar += _scatter_matrix(tp, E) @ np.sum(tz * Y16 * (du3[tp, None] * g16 + u3[tp, None] * dg16), axis=1)
+        cbar = u3[tp] * np.sum(tz * dY16 * g16, axis=1)
+        gvec += _scatter_matrix(te, E) @ ((cbar * inv_r[te])[:, None] * (rhat[tp] - c[:, None] * rhat[te]))
+        gvec += _scatter_matrix(tp, E) @ ((cbar * inv_r[tp])[:, None] * (rhat[te] - c[:, None] * rhat[tp]))
+        zbar += _scatter_matrix(send[tp], N) @ (tau[te] * Y16 * g16 * u3[tp, None])
+    hbar = (zbar * z * (1.0 - z)) @ lay["G"]
+    return rbar, gvec, hbar
+
+
+# --------------------------------------------------------------------------------------
 # O3-O5 model
 # --------------------------------------------------------------------------------------
 def _scatter_matrix(index, n_rows, weights=None):
@@ -224,9 +350,9 @@ def _scatter_matrix(index, n_rows, weights=None):
     return sp.csr_matrix((data, (index, np.arange(e))), shape=(n_rows, e))
 
 
-def _edge_layer_forward(model, lay, h, recv, send, r, want_cache=False):
+def _edge_layer_forward(model, lay, h, recv, send, r, t=None):
     """m_i = alpha sum_{e in in(i)} u(r_e) phi_e with
-    a_e = W1 [h_i || h_j || e_hat_e] + b1 ; s = SiLU(a) ; p = W2 s + b2 ; phi = SiLU(p)."""
+    a_e = W1 [h_i || h_j || e_hat_e] + b1 (+ W3 t_e, three-body variant) ; s = SiLU(a) ; p = W2 s + b2 ; phi = SiLU(p)."""
     N, d = h.shape
     m = np.zeros((N, d))
     for lo in range(0, len(recv), EDGE_CHUNK):
@@ -235,21 +361,25 @@ def _edge_layer_forward(model, lay, h, recv, send, r, want_cache=False):
         g, _ = rbf(r[sl], model.r_cut, model.n_rbf)
         x = np.concatenate([h[recv[sl]], h[send[sl]], u[:, None] * g], axis=1)
         a = x @ lay["W1"].T + lay["b1"]
+        if t is not None:
+            a = a + t[sl] @ lay["W3"].T
         p = silu(a) @ lay["W2"].T + lay["b2"]
         phi = silu(p)
         m += _scatter_matrix(recv[sl], N, model.agg_scale * u) @ phi
     return m
 
 
-def forward(model, L, species, recv, send, r):
+def forward(model, L, species, recv, send, r, rvec=None):
     """h^0 = T[z]; L layers (O3); E_i = wo . SiLU(Wo h^L + bo) + b_E + E0[z] (O4).
-    Returns E_i and the per-layer node states needed by the reverse pass."""
+    Returns E_i and the per-layer node states needed by the reverse pass. `rvec` (edge vectors) is needed by the
+    three-body variant only."""
     assert 0 <= L <= model.L_max
     h = model.T[species].copy()
     hs, ms, cs = [], [], []
     for l in range(L):
         lay = model.layers[l]
-        m = _edge_layer_forward(model, lay, h, recv, send, r)
+        t = three_body_terms(model, lay, h, recv, send, rvec, r)[0] if model.r_cut3 > 0.0 else None
+        m = _edge_layer_forward(model, lay, h, recv, send, r, t)
         c = np.concatenate([h, m], axis=1) @ lay["V1"].T + lay["c1"]
         hs.append(h); ms.append(m); cs.append(c)
         h = h + silu(c) @ lay["V2"].T + lay["c2"]
@@ -258,15 +388,22 @@ def forward(model, L, species, recv, send, r):
     return E_i, dict(hs=hs, ms=ms, cs=cs, hL=h, o=o)
 
 
-def backward_rbar(model, L, species, recv, send, r, cache, omega):
-    """Reverse mode of sum_i omega_i E_i down to the per-edge scalar rbar_e = d(.)/d r_e (O5)."""
+def backward_rbar(model, L, species, recv, send, r, cache, omega, rvec=None, return_gvec=False):
+    """Reverse mode of sum_i omega_i E_i down to the per-edge scalar rbar_e = d(.)/d r_e (O5). The three-body variant
+    also depends on the edge DIRECTIONS; with return_gvec the per-edge vector gradient gvec_e = d(.)/d rvec_e at fixed
+    |r_e| contributions excluded from rbar (zeros for the two-body model) is returned as well."""
     N = len(species)
     d = model.d
+    three = model.r_cut3 > 0.0
     hbar = omega[:, None] * ((model.wo * dsilu(cache["o"])) @ model.Wo)
     rbar = np.zeros(len(recv))
+    gvec = np.zeros((len(recv), 3))
     for l in range(L - 1, -1, -1):
         lay = model.layers[l]
         h, c = cache["hs"][l], cache["cs"][l]
+        if three:
+            t, S3, z3 = three_body_terms(model, lay, h, recv, send, rvec, r)
+            tbar = np.zeros((len(recv), N_ANGLE))
         cbar = (hbar @ lay["V2"]) * dsilu(c)
         hm = cbar @ lay["V1"]
         hbar = hbar + hm[:, :d]
@@ -279,6 +416,8 @@ def backward_rbar(model, L, species, recv, send, r, cache, omega):
             g, dg = rbf(r[sl], model.r_cut, model.n_rbf)
             x = np.concatenate([h[ri], h[si], u[:, None] * g], axis=1)
             a = x @ lay["W1"].T + lay["b1"]
+            if three:
+                a = a + t[sl] @ lay["W3"].T
             p = silu(a) @ lay["W2"].T + lay["b2"]
             phi = silu(p)
             mb = mbar[ri]
@@ -287,6 +426,8 @@ def backward_rbar(model, L, species, recv, send, r, cache, omega):
             pbar = phibar * dsilu(p)
             sbar = pbar @ lay["W2"]
             abar = sbar * dsilu(a)
+            if three:
+                tbar[sl] = abar @ lay["W3"]
             xbar = abar @ lay["W1"]
             hadd += _scatter_matrix(ri, N) @ xbar[:, :d]
             hadd += _scatter_matrix(si, N) @ xbar[:, d:2 * d]
@@ -294,15 +435,25 @@ def backward_rbar(model, L, species, recv, send, r, cache, omega):
             ubar = ubar + np.sum(ebar * g, axis=1)
             rbar[sl] += ubar * du + np.sum(u[:, None] * ebar * dg, axis=1)
         hbar = hbar + hadd
+        if three:
+            rb3, gv3, hb3 = three_body_backward(model, lay, h, recv, send, rvec, r, tbar, S3, z3)
+            rbar += rb3
+            gvec += gv3
+            hbar = hbar + hb3
+    if return_gvec:
+        return rbar, gvec
     return rbar
 
 
-def forces_from_rbar(n_atoms, recv, send, rvec, r, rbar):
+def forces_from_rbar(n_atoms, recv, send, rvec, r, rbar, gvec=None):
     """F_k = sum_{e in in(k)} rbar_e rhat_e - sum_{e in out(k)} rbar_e rhat_e, rhat := 0 at r = 0
-    (reading R13), because d r_e / d x_send = rhat_e and d r_e / d x_recv = -rhat_e."""
+    (reading R13), because d r_e / d x_send = rhat_e and d r_e / d x_recv = -rhat_e. With the three-body variant the
+    gradient with respect to the edge VECTOR is rbar_e rhat_e + gvec_e and d rvec_e / d x_send = 1 = -d rvec_e / d x_recv."""
     with np.errstate(divide="ignore", invalid="ignore"):
         rhat = np.where(r[:, None] > 0.0, rvec / r[:, None], 0.0)
     f_edge = rbar[:, None] * rhat
+    if gvec is not None:
+        f_edge = f_edge + gvec
     return _scatter_matrix(recv, n_atoms) @ f_edge - _scatter_matrix(send, n_atoms) @ f_edge
 
 
@@ -315,18 +466,18 @@ def energy_forces(model, L, pos, cell, species, graph=None, omega=None, return_e
         graph = neighbor_list(pos, cell, model.r_cut)
     recv, send, shift = graph
     rvec, r = edge_vectors(pos, cell, recv, send, shift)
-    E_i, cache = forward(model, L, species, recv, send, r)
+    E_i, cache = forward(model, L, species, recv, send, r, rvec)
     if omega is None:
         omega = np.ones(len(species))
-    rbar = backward_rbar(model, L, species, recv, send, r, cache, np.asarray(omega, np.float64))
-    F = forces_from_rbar(len(species), recv, send, rvec, r, rbar)
+    rbar, gvec = backward_rbar(model, L, species, recv, send, r, cache, np.asarray(omega, np.float64), rvec, return_gvec=True)
+    F = forces_from_rbar(len(species), recv, send, rvec, r, rbar, gvec if model.r_cut3 > 0.0 else None)
     E = float(np.sum(omega * E_i))
     if return_extra:
-        return E, E_i, F, dict(rbar=rbar, r=r, rvec=rvec, cache=cache, graph=graph)
+        return E, E_i, F, dict(rbar=rbar, gvec=gvec, r=r, rvec=rvec, cache=cache, graph=graph)
     return E, E_i, F
 
 
-def stress_from_rbar(cell, rvec, r, rbar):
+def stress_from_rbar(cell, rvec, r, rbar, gvec=None):
     """Stress sigma = (1/V) dE/d(strain) (PAPER.md:173 lists stress beside energy and forces as a model
     output). Under a homogeneous strain x -> (1 + eps) x, C -> C (1 + eps)^T every edge vector transforms as
     r_e -> (1 + eps) r_e, so d r_e / d eps_ab = r_a r_b / r and
@@ -335,13 +486,16 @@ def stress_from_rbar(cell, rvec, r, rbar):
     V = abs(np.linalg.det(np.asarray(cell, np.float64)))
     with np.errstate(divide="ignore", invalid="ignore"):
         w = np.where(r > 0.0, rbar / r, 0.0)
-    return np.einsum("e,ea,eb->ab", w, rvec, rvec) / V
+    sigma = np.einsum("e,ea,eb->ab", w, rvec, rvec) / V
+    if gvec is not None:   # three-body variant: d rvec_e / d eps_ab = delta_.a r_eb, the gradient w.r.t. rvec_e has gvec_e on top
+        sigma = sigma + np.einsum("ea,eb->ab", gvec, rvec) / V
+    return sigma
 
 
 def energy_forces_stress(model, L, pos, cell, species, graph=None, omega=None):
     """E, E_i, F and the stress tensor [3,3] of the unpartitioned model."""
     E, E_i, F, ex = energy_forces(model, L, pos, cell, species, graph, omega, return_extra=True)
-    return E, E_i, F, stress_from_rbar(cell, ex["rvec"], ex["r"], ex["rbar"])
+    return E, E_i, F, stress_from_rbar(cell, ex["rvec"], ex["r"], ex["rbar"], ex["gvec"] if model.r_cut3 > 0.0 else None)
 
 
 # --------------------------------------------------------------------------------------

@@ -29,7 +29,7 @@ class MlipError(RuntimeError):
 class mlip_model_header(C.Structure):
     _fields_ = [("magic", C.c_uint32), ("version", C.c_uint32), ("n_species", C.c_int32), ("d", C.c_int32),
                 ("n_rbf", C.c_int32), ("L_max", C.c_int32), ("r_cut", C.c_float), ("agg_scale", C.c_float),
-                ("flags", C.c_int32), ("reserved", C.c_int32 * 3)]
+                ("flags", C.c_int32), ("n_rbf3", C.c_int32), ("l_max", C.c_int32), ("r_cut3", C.c_float)]
 
 
 def lib_path() -> str:
@@ -52,6 +52,7 @@ def load_library():
     lib.mlip_ctx_create.argtypes = [i32, vp, P(vp)]
     lib.mlip_ctx_destroy.argtypes = [vp]; lib.mlip_ctx_destroy.restype = None
     lib.mlip_last_error.argtypes = [vp]; lib.mlip_last_error.restype = C.c_char_p
+    lib.mlip_ctx_status.argtypes = [vp]
     lib.mlip_model_load.argtypes = [vp, P(mlip_model_header), vp, C.c_size_t, P(vp)]
     lib.mlip_model_destroy.argtypes = [vp]; lib.mlip_model_destroy.restype = None
     lib.mlip_build_graph.argtypes = [vp, vp, vp, vp, i64, dbl, P(vp)]
@@ -113,6 +114,10 @@ class Context:
         if status != 0:
             raise MlipError(status, self.lib.mlip_last_error(self.h).decode())
 
+    def status(self):
+        """mlip_ctx_status: synchronise the stream and raise if the asynchronous work reported an error."""
+        self.check(self.lib.mlip_ctx_status(self.h))
+
     @property
     def launches(self) -> int:
         return int(self.lib.mlip_ctx_launch_count(self.h))
@@ -144,7 +149,7 @@ class Context:
 
 
 def make_header(n_species, d, n_rbf, L_max, r_cut, agg_scale) -> mlip_model_header:
-    return mlip_model_header(MLIP_MAGIC, 1, n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), 0, (0, 0, 0))
+    return mlip_model_header(MLIP_MAGIC, 1, n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), 0, 0, 0, 0.0)
 
 
 class Model:

@@ -44,6 +44,10 @@ struct mlip_ctx {
   int64_t launches = 0;
   bool active_sets = true;  // per-layer active sets inside sub-domains (mlip_ctx_set_active_sets)
   bool khop_halo = true;    // halo and depth classes by K-hop search instead of geometry (mlip_ctx_set_khop_halo)
+  // Sticky device-side status word (MLIP_DEV_* bits, written by kernels with atomicOr): errors that only the device can
+  // see (non-finite results of the 16-bit path, a missing reverse edge) surface at the next synchronising call or at
+  // mlip_ctx_status, never as silently wrong numbers.
+  int* dev_status = nullptr;
   void set_error(const std::string& s) { err = s; }
   // ---- optional per-group timing ----
   struct ProfRec { int cat; int64_t launches; cudaEvent_t a, b; };
@@ -87,6 +91,25 @@ struct mlip_ctx {
   }
   void free(void* p) {
     if (p) cudaFreeAsync(p, stream);
+  }
+};
+
+enum { MLIP_DEV_REV_MISSING = 1, MLIP_DEV_NONFINITE = 2 };
+// Reads and clears the device status word; the stream must have been synchronised. Returns MLIP_OK or the status the
+// bits map to (with the context error message set).
+int mlip_take_dev_status(mlip_ctx* ctx);
+
+// Stream-ordered scratch buffers that are released when the scope ends, on every path out of it.
+struct Scratch {
+  mlip_ctx* c;
+  std::vector<void*> v;
+  explicit Scratch(mlip_ctx* ctx) : c(ctx) {}
+  ~Scratch() { for (void* p : v) c->free(p); }
+  template <class T>
+  int get(T** p, size_t n) {
+    const int s = c->alloc(p, n);
+    if (s == MLIP_OK) v.push_back(*p);
+    return s;
   }
 };
 
@@ -164,6 +187,7 @@ struct mlip_graph {
   int32_t* perm = nullptr;      // [N] internal -> caller index
   double* frac = nullptr;       // [N,3] wrapped fractional coordinates, internal order
   int32_t* species = nullptr;   // [N] internal order
+  int species_min = 0, species_max = 0;  // range of the species values (read back with the edge count)
   int32_t* rowptr = nullptr;    // [N+1]
   int32_t* recv = nullptr;      // [E]
   int32_t* send = nullptr;      // [E]

@@ -50,6 +50,57 @@ __global__ void __launch_bounds__(256) k_readout(int64_t n, int d, const float* 
   if (lane == 0) E_i[i] = acc + bE[0] + E0[species[i]];
 }
 
+// ---- power-of-two scale of the reverse pass (MLIP_BF16 only) -----------------------------------------------------
+// The reverse pass is linear in obar = d(sum of root energies)/d o, so obar may be multiplied by any s as long as the
+// per-edge adjoints rbar are divided by s when the forces and the virial are assembled. With s = 2^k chosen such that
+// max |s obar| lies in [2, 4), the f16 adjoints of the tensor-core edge kernels (mbar, pbar, abar) sit 14 octaves above
+// the f16 subnormals and 14 below its maximum whatever the energy scale of the model; a power of two changes no
+// mantissa. scale[0] = s, scale[1] = 1/s.
+__global__ void __launch_bounds__(256) k_absmax_partial(int64_t n, const float* __restrict__ x, float* __restrict__ partial) {
+  __shared__ float sh[256];
+  float m = 0.f;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    m = fmaxf(m, fabsf(x[i]));  // fmaxf drops NaN: a NaN in obar reaches the forces and is reported there
+  sh[threadIdx.x] = m;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (threadIdx.x < s) sh[threadIdx.x] = fmaxf(sh[threadIdx.x], sh[threadIdx.x + s]);
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void k_pick_scale(int n_partial, const float* __restrict__ partial, float* __restrict__ scale) {
+  if (threadIdx.x != 0) return;
+  float m = 0.f;
+  for (int i = 0; i < n_partial; ++i) m = fmaxf(m, partial[i]);
+  float s = 1.0f;
+  if (m > 0.f && m < 3.0e38f) {
+    int e;
+    frexpf(m, &e);            // m = f 2^e, f in [0.5, 1)  ->  m 2^(2-e) in [2, 4)
+    int k = 2 - e;
+    k = k > 60 ? 60 : (k < -60 ? -60 : k);
+    s = ldexpf(1.0f, k);
+  }
+  scale[0] = s;
+  scale[1] = 1.0f / s;
+}
+__global__ void k_scale_inplace(int64_t n4, float4* __restrict__ x, const float* __restrict__ scale) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n4) return;
+  const float s = scale[0];
+  float4 v = x[i];
+  v.x *= s; v.y *= s; v.z *= s; v.w *= s;
+  x[i] = v;
+}
+
+// non-finite energy or force -> sticky context status (MLIP_ERR_NUMERIC at the next synchronising call)
+__global__ void k_check_finite(int64_t n, const float* __restrict__ F, const double* __restrict__ energy, int* __restrict__ status) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = i < n && !isfinite(F[i]);
+  if (i == 0) bad = bad || !isfinite(energy[0]);
+  if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(status, MLIP_DEV_NONFINITE);
+}
+
 // deterministic float64 sum of the root-atom energies: per-block partials, then one block
 __global__ void __launch_bounds__(256) k_energy_partial(int64_t n, const float* __restrict__ E_i,
                                                         const float* __restrict__ omega, const int32_t* __restrict__ gid,
@@ -88,14 +139,16 @@ __global__ void __launch_bounds__(256) k_energy_final(int64_t n_partial, const d
 __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __restrict__ rowptr,
                                                 const int32_t* __restrict__ rev, const float4* __restrict__ rvec,
                                                 const float* __restrict__ rbar, const int32_t* __restrict__ gid,
+                                                const float* __restrict__ scale /*[2] = s, 1/s of the reverse pass, or null*/,
                                                 float* __restrict__ F) {
   const int lane = threadIdx.x & 31;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (k >= n) return;
+  const float inv_s = scale ? scale[1] : 1.0f;
   float fx = 0.f, fy = 0.f, fz = 0.f;
   for (int e = rowptr[k] + lane; e < rowptr[k + 1]; e += 32) {
     const float4 rv = rvec[e];
-    const float w = (rbar[e] + rbar[rev[e]]) * (rv.w > 0.f ? 1.0f / rv.w : 0.f);
+    const float w = (rbar[e] + rbar[rev[e]]) * (rv.w > 0.f ? inv_s / rv.w : 0.f);
     fx = fmaf(w, rv.x, fx); fy = fmaf(w, rv.y, fy); fz = fmaf(w, rv.z, fz);
   }
 #pragma unroll
@@ -113,13 +166,15 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
 // Virial of one sub-domain: W_ab += sum_e rbar_e r_a r_b / r over its directed edges (rbar is zero on the
 // edges no layer evaluated). float64 per-block partials in a fixed order, then one block: deterministic, no atomics.
 __global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const float4* __restrict__ rvec,
-                                                        const float* __restrict__ rbar, double* __restrict__ partial) {
+                                                        const float* __restrict__ rbar, const float* __restrict__ scale,
+                                                        double* __restrict__ partial) {
   __shared__ double sh[6][256];
   double w[6] = {0, 0, 0, 0, 0, 0};
+  const double inv_s = scale ? (double)scale[1] : 1.0;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < E; e += (int64_t)gridDim.x * blockDim.x) {
     const float4 rv = rvec[e];
     if (rv.w > 0.f) {
-      const double s = (double)rbar[e] / (double)rv.w, x = rv.x, y = rv.y, z = rv.z;
+      const double s = inv_s * (double)rbar[e] / (double)rv.w, x = rv.x, y = rv.y, z = rv.z;
       w[0] += s * x * x; w[1] += s * y * y; w[2] += s * z * z;
       w[3] += s * y * z; w[4] += s * x * z; w[5] += s * x * y;
     }
@@ -214,7 +269,9 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   // hb = copy of the residual stream h^l (two buffers, alternating), cbar_b, Qbar_b
   __nv_bfloat16 *hb[2] = {nullptr, nullptr}, *cbar_b = nullptr, *Qbar_b = nullptr;
   double* partial = nullptr;
+  float* scale = nullptr;  // [2 + 1184]: s, 1/s of the reverse pass (MLIP_BF16), then the per-block maxima
   if (bf) {
+    W_ALLOC(scale, float, 2 + 148 * 8);
     W_ALLOC(hb[0], __nv_bfloat16, n * d); W_ALLOC(hb[1], __nv_bfloat16, n * d);
     W_ALLOC(cbar_b, __nv_bfloat16, n * d); W_ALLOC(Qbar_b, __nv_bfloat16, n * d);
   }
@@ -310,7 +367,15 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     k_energy_partial<<<(unsigned)((n0 + 255) / 256), 256, 0, st>>>(n0, E_i, g.omega, g.gid, partial, Ei_int);
     k_energy_final<<<1, 256, 0, st>>>((n0 + 255) / 256, partial, energy_accum);
     ctx->launches += 3;
+    if (bf && n0 > 0 && L > 0) {
+      const int nb = (int)(n0 * d / 4 < 148 * 8 * 256 ? (n0 * d / 4 + 255) / 256 : 148 * 8);
+      k_absmax_partial<<<nb, 256, 0, st>>>(n0 * d, obar, scale + 2);
+      k_pick_scale<<<1, 32, 0, st>>>(nb, scale + 2, scale);
+      k_scale_inplace<<<nblk(n0 * d / 4, 256), 256, 0, st>>>(n0 * d / 4, reinterpret_cast<float4*>(obar), scale);
+      ctx->launches += 3;
+    }
   }
+  const float* rscale = (bf && n0 > 0 && L > 0) ? scale : nullptr;
   {
     GemmArgs a;
     a.X1 = obar; a.ld1 = d; a.K1 = d; a.B = bf ? (const void*)M->WoT_bf : (const void*)M->WoT;
@@ -373,13 +438,13 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   }
   {
     ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
-    k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, F_int);
+    k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, rscale, F_int);
     ctx->launches++;
     if (virial_accum && E > 0) {
       const int nb = (int)(E < 148 * 8 * 256 ? (E + 255) / 256 : 148 * 8);
       double* vpart = nullptr;
       W_ALLOC(vpart, double, (size_t)nb * 6);
-      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, vpart);
+      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, rscale, vpart);
       k_virial_final<<<1, 32, 0, st>>>(nb, vpart, virial_accum);
       ctx->launches += 2;
     }
@@ -430,18 +495,23 @@ static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const m
     return MLIP_ERR_HALO_TOO_SMALL;
   }
   if (fabs(G->r_cut - (double)M->h.r_cut) > 1e-6 * G->r_cut) { ctx->set_error("graph r_cut differs from model r_cut"); return MLIP_ERR_INVALID_ARG; }
+  if (G->N > 0 && (G->species_min < 0 || G->species_max >= M->h.n_species)) {
+    ctx->set_error("species outside [0, n_species) of the model");
+    return MLIP_ERR_INVALID_ARG;
+  }
   MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
   cudaStream_t st = ctx->stream;
   const int64_t N = G->N;
+  Scratch tmp(ctx);
   float *F_int = nullptr, *E_int = nullptr;
-  MLIP_TRY(ctx->alloc(&F_int, 3 * N));
-  MLIP_TRY(ctx->alloc(&E_int, N));
+  MLIP_TRY(tmp.get(&F_int, 3 * N));
+  MLIP_TRY(tmp.get(&E_int, N));
   cudaMemsetAsync(F_int, 0, sizeof(float) * 3 * N, st);
   cudaMemsetAsync(E_int, 0, sizeof(float) * N, st);
   cudaMemsetAsync(energy_dev, 0, sizeof(double), st);
   double* virial = nullptr;
   if (stress_dev) {
-    MLIP_TRY(ctx->alloc(&virial, 6));
+    MLIP_TRY(tmp.get(&virial, 6));
     cudaMemsetAsync(virial, 0, 6 * sizeof(double), st);
   }
   int status = MLIP_OK;
@@ -456,7 +526,8 @@ static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const m
   }
   if (status == MLIP_OK && N > 0) {
     k_unpermute<<<nblk(N, 256), 256, 0, st>>>(N, G->perm, F_int, E_int, forces_dev, atom_energy_dev);
-    ctx->launches++;
+    k_check_finite<<<nblk(3 * N, 256), 256, 0, st>>>(3 * N, F_int, energy_dev, ctx->dev_status);
+    ctx->launches += 2;
   }
   if (status == MLIP_OK && stress_dev) {
     const double* c = G->cell;
@@ -464,7 +535,6 @@ static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const m
     k_stress_out<<<1, 32, 0, st>>>(virial, vol > 0.0 ? 1.0 / vol : 0.0, stress_dev);
     ctx->launches++;
   }
-  ctx->free(F_int); ctx->free(E_int); ctx->free(virial);
   if (status != MLIP_OK) return status;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
@@ -483,8 +553,9 @@ extern "C" int mlip_step_host(mlip_ctx* ctx, const mlip_model* M, int L, const d
   double *pos_d = nullptr, *e_d = nullptr;
   int32_t* sp_d = nullptr;
   float* f_d = nullptr;
-  MLIP_TRY(ctx->alloc(&pos_d, 3 * N)); MLIP_TRY(ctx->alloc(&sp_d, N)); MLIP_TRY(ctx->alloc(&f_d, 3 * N));
-  MLIP_TRY(ctx->alloc(&e_d, 1));
+  Scratch tmp(ctx);
+  MLIP_TRY(tmp.get(&pos_d, 3 * N)); MLIP_TRY(tmp.get(&sp_d, N)); MLIP_TRY(tmp.get(&f_d, 3 * N));
+  MLIP_TRY(tmp.get(&e_d, 1));
   MLIP_CUDA_CHECK(ctx, cudaMemcpyAsync(pos_d, pos_host, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, st));
   MLIP_CUDA_CHECK(ctx, cudaMemcpyAsync(sp_d, species_host, sizeof(int32_t) * N, cudaMemcpyHostToDevice, st));
   mlip_graph* G = nullptr;
@@ -498,9 +569,8 @@ extern "C" int mlip_step_host(mlip_ctx* ctx, const mlip_model* M, int L, const d
   }
   mlip_part_destroy(P);
   mlip_graph_destroy(G);
-  ctx->free(pos_d); ctx->free(sp_d); ctx->free(f_d); ctx->free(e_d);
   cudaError_t e = cudaStreamSynchronize(st);
   if (status != MLIP_OK) return status;
   if (e != cudaSuccess) { ctx->set_error(std::string("step: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
-  return MLIP_OK;
+  return mlip_take_dev_status(ctx);
 }

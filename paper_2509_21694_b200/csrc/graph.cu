@@ -69,8 +69,14 @@ __global__ void k_gather_sorted(const int32_t* __restrict__ order, int64_t N,
                                 const int32_t* __restrict__ cellid,
                                 double* __restrict__ pos_s, double* __restrict__ frac_s,
                                 int32_t* __restrict__ wrap_s, int32_t* __restrict__ species_s,
-                                int32_t* __restrict__ cellid_s) {
+                                int32_t* __restrict__ cellid_s, int* __restrict__ sp_range /*[2]: max(s), max(-s)*/) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int sp = k < N ? species[order[k]] : 0;
+  const int hi = __reduce_max_sync(0xffffffffu, sp), lo = __reduce_max_sync(0xffffffffu, -sp);
+  if ((threadIdx.x & 31) == 0) {
+    if (hi > 0) atomicMax(&sp_range[0], hi);
+    if (lo > 0) atomicMax(&sp_range[1], lo);
+  }
   if (k >= N) return;
   const int64_t i = order[k];
 #pragma unroll
@@ -277,7 +283,9 @@ __global__ void k_reverse(int64_t E, const int32_t* __restrict__ rowptr, const i
     if (v == want) { found = mid; break; }
     if (v < want) lo = mid + 1; else hi = mid - 1;
   }
-  if (found < 0) *err_flag = 2;
+  // a missing partner (impossible for a symmetric list) is reported through the context status word; the edge points
+  // at itself so that nothing downstream indexes out of bounds
+  if (found < 0) { atomicOr(err_flag, MLIP_DEV_REV_MISSING); found = (int)e; }
   rev[e] = found;
 }
 
@@ -393,19 +401,20 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
           *wrap_s = nullptr, *cellid_s = nullptr, *deg = nullptr;
   unsigned long long *keys = nullptr, *total = nullptr, *scratch = nullptr;
   int cap = 0;
-  int* err_flag = nullptr;
+  int *err_flag = nullptr, *sp_range = nullptr;
 #define G_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
   G_TRY(ctx->alloc(&frac, 3 * N)); G_TRY(ctx->alloc(&wrap, 3 * N)); G_TRY(ctx->alloc(&cellid, N));
   G_TRY(ctx->alloc(&cell_count, 2 * n_cells + 2)); G_TRY(ctx->alloc(&cell_start, n_cells + 1));
   G_TRY(ctx->alloc(&order, N)); G_TRY(ctx->alloc(&pos_s, 3 * N)); G_TRY(ctx->alloc(&wrap_s, 3 * N));
   G_TRY(ctx->alloc(&cellid_s, N)); G_TRY(ctx->alloc(&deg, N + 1)); G_TRY(ctx->alloc(&total, 2));
-  G_TRY(ctx->alloc(&err_flag, 1));
+  G_TRY(ctx->alloc(&err_flag, 1)); G_TRY(ctx->alloc(&sp_range, 2));
   G_TRY(ctx->alloc(&G->perm, N)); G_TRY(ctx->alloc(&G->frac, 3 * N)); G_TRY(ctx->alloc(&G->species, N));
   G_TRY(ctx->alloc(&G->rowptr, N + 1));
   int32_t* cursor = cell_count + n_cells + 1;
   cudaMemsetAsync(cell_count, 0, sizeof(int32_t) * (2 * n_cells + 2), st);
   cudaMemsetAsync(total, 0, 2 * sizeof(unsigned long long), st);
   cudaMemsetAsync(err_flag, 0, sizeof(int), st);
+  cudaMemsetAsync(sp_range, 0, 2 * sizeof(int), st);
   if (N > 0) {
     k_frac_bin<<<nblk(N, 256), 256, 0, st>>>(pos_dev, N, g, frac, wrap, cellid, cell_count);
     ctx->launches++;
@@ -415,7 +424,7 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
     k_cell_scatter<<<nblk(N, 256), 256, 0, st>>>(cellid, N, cell_start, cursor, order);
     k_cell_sort<<<nblk(n_cells, 128), 128, 0, st>>>(cell_start, (int)n_cells, order);
     k_gather_sorted<<<nblk(N, 256), 256, 0, st>>>(order, N, pos_dev, frac, wrap, species_dev, cellid, pos_s,
-                                                  G->frac, wrap_s, G->species, cellid_s);
+                                                  G->frac, wrap_s, G->species, cellid_s, sp_range);
     cudaMemcpyAsync(G->perm, order, sizeof(int32_t) * N, cudaMemcpyDeviceToDevice, st);
     // one search pass when a capped scratch row per atom is affordable: cap = 1.5 x the mean degree + 32
     const double nbar = 4.18879020478639 * r_cut * r_cut * r_cut * (double)N / vol;
@@ -432,8 +441,9 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
     ctx->launches += 4;
   }
   unsigned long long total_h = 0;
-  int err_h = 0;
+  int err_h = 0, sp_h[2] = {0, 0};
   if (cudaMemcpyAsync(&total_h, total, sizeof(total_h), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaMemcpyAsync(sp_h, sp_range, sizeof(sp_h), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaMemcpyAsync(&err_h, err_flag, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess) {
     ctx->set_error(std::string("graph build (count): ") + cudaGetErrorString(cudaGetLastError()));
@@ -443,6 +453,7 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
   if (total_h >= (1ull << 31)) { ctx->set_error("number of edges >= 2^31"); return fail(MLIP_ERR_OVERFLOW); }
   const int64_t E = (int64_t)total_h;
   G->E = E;
+  G->species_max = sp_h[0]; G->species_min = -sp_h[1];
   G_TRY(mlip_exclusive_scan_i32(ctx, deg, G->rowptr, N, nullptr));
   G_TRY(ctx->alloc(&keys, E)); G_TRY(ctx->alloc(&G->recv, E)); G_TRY(ctx->alloc(&G->send, E));
   G_TRY(ctx->alloc(&G->shift, E)); G_TRY(ctx->alloc(&G->rev, E)); G_TRY(ctx->alloc(&G->rvec, E));
@@ -455,12 +466,12 @@ extern "C" int mlip_build_graph(mlip_ctx* ctx, const double* pos_dev, const doub
     k_sort_rows<<<nblk(N, 4), 128, 0, st>>>(N, G->rowptr, keys);
     k_finalize_edges<<<nblk(N * 32, 256), 256, 0, st>>>(N, g, pos_s, G->rowptr, keys, G->recv, G->send, G->shift,
                                                         G->rvec);
-    k_reverse<<<nblk(E, 256), 256, 0, st>>>(E, G->rowptr, G->recv, keys, G->rev, err_flag);
+    k_reverse<<<nblk(E, 256), 256, 0, st>>>(E, G->rowptr, G->recv, keys, G->rev, ctx->dev_status);
     ctx->launches += 4;
   }
   ctx->free(frac); ctx->free(wrap); ctx->free(cellid); ctx->free(cell_count); ctx->free(cell_start);
   ctx->free(order); ctx->free(pos_s); ctx->free(wrap_s); ctx->free(cellid_s); ctx->free(deg);
-  ctx->free(total); ctx->free(keys); ctx->free(scratch);
+  ctx->free(total); ctx->free(keys); ctx->free(scratch); ctx->free(sp_range);
   cudaError_t e = cudaGetLastError();
   ctx->free(err_flag);
   if (e != cudaSuccess) { ctx->set_error(std::string("graph build: ") + cudaGetErrorString(e)); return fail(MLIP_ERR_CUDA); }

@@ -62,8 +62,9 @@ extern "C" int mlip_md_nve(mlip_ctx* ctx, const mlip_model* M, int L, double* po
   const int nb = (int)(N < 148 * 4 * 256 ? (N + 255) / 256 : 148 * 4);
   float* F = nullptr;
   double *e_pot = nullptr, *partial = nullptr, *e_tot = nullptr;
-  MLIP_TRY(ctx->alloc(&F, 3 * N)); MLIP_TRY(ctx->alloc(&e_pot, 1)); MLIP_TRY(ctx->alloc(&partial, nb > 0 ? nb : 1));
-  MLIP_TRY(ctx->alloc(&e_tot, n_steps + 1));
+  Scratch tmp(ctx);
+  MLIP_TRY(tmp.get(&F, 3 * N)); MLIP_TRY(tmp.get(&e_pot, 1)); MLIP_TRY(tmp.get(&partial, nb > 0 ? nb : 1));
+  MLIP_TRY(tmp.get(&e_tot, n_steps + 1));
   int status = MLIP_OK;
   auto evaluate = [&]() {  // graph -> partition -> E, F at the current positions
     mlip_graph* G = nullptr;
@@ -98,9 +99,8 @@ extern "C" int mlip_md_nve(mlip_ctx* ctx, const mlip_model* M, int L, double* po
     if (total_energy_host)
       cudaMemcpyAsync(total_energy_host, e_tot, sizeof(double) * (n_steps + 1), cudaMemcpyDeviceToHost, st);
   }
-  ctx->free(F); ctx->free(e_pot); ctx->free(partial); ctx->free(e_tot);
   cudaError_t e = cudaStreamSynchronize(st);
   if (status != MLIP_OK) return status;
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) { ctx->set_error(std::string("md: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
-  return MLIP_OK;
+  return mlip_take_dev_status(ctx);
 }

@@ -48,12 +48,42 @@ extern "C" int mlip_ctx_create(int device, void* stream, mlip_ctx** out) {
     uint64_t thr = ~0ull;  // keep freed blocks in the pool between steps
     cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
   }
+  if (cudaMalloc((void**)&c->dev_status, sizeof(int)) != cudaSuccess || cudaMemset(c->dev_status, 0, sizeof(int)) != cudaSuccess) {
+    cudaGetLastError();
+    delete c;
+    return MLIP_ERR_OUT_OF_MEMORY;
+  }
   *out = c;
   return MLIP_OK;
 }
 
+int mlip_take_dev_status(mlip_ctx* ctx) {
+  int bits = 0;
+  if (cudaMemcpy(&bits, ctx->dev_status, sizeof(int), cudaMemcpyDeviceToHost) != cudaSuccess) {
+    ctx->set_error(std::string("status read: ") + cudaGetErrorString(cudaGetLastError()));
+    return MLIP_ERR_CUDA;
+  }
+  if (bits == 0) return MLIP_OK;
+  cudaMemset(ctx->dev_status, 0, sizeof(int));
+  if (bits & MLIP_DEV_NONFINITE) {
+    ctx->set_error("non-finite energy or force: with MLIP_BF16 the edge operands are IEEE half, |pre-activations| and "
+                   "|adjoints| must stay below 65504 (use MLIP_FP32 for this model)");
+    return MLIP_ERR_NUMERIC;
+  }
+  ctx->set_error("reverse edge not found while building the graph (internal error)");
+  return MLIP_ERR_CUDA;
+}
+
+extern "C" int mlip_ctx_status(mlip_ctx* ctx) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) { ctx->set_error(std::string("stream: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
+  return mlip_take_dev_status(ctx);
+}
+
 extern "C" void mlip_ctx_destroy(mlip_ctx* ctx) {
   if (!ctx) return;
+  cudaFree(ctx->dev_status);
   for (auto& r : ctx->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (cudaEvent_t e : ctx->event_pool) cudaEventDestroy(e);
   delete ctx;

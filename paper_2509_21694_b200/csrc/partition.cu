@@ -170,7 +170,10 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
   // depth classes 0 .. n_cls-1 (see SubGraph): the halo spans ceil(halo / r_c) shells of thickness r_c
   int n_cls = 1 + (int)ceil(halo / G->r_cut - 1e-9);
   if (n_cls < 2) n_cls = 2;
-  if (n_cls > MLIP_MAX_CLS) n_cls = MLIP_MAX_CLS;
+  if (n_cls > MLIP_MAX_CLS) {
+    ctx->set_error("partition: halo spans more than 31 shells of thickness r_cut (ceil(halo / r_cut) > 31)");
+    return fail(MLIP_ERR_UNSUPPORTED);
+  }
   const bool bfs = ctx->khop_halo;
   P->khop = bfs;
   const int64_t CN = (int64_t)n_cls * N;

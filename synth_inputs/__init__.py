@@ -30,10 +30,13 @@ class ModelSpec:
     L_max: int
     r_cut: float
     agg_scale: float  # alpha = 1/sqrt(nominal mean degree), reading R7
+    r_cut3: float = 0.0  # > 0: three-body variant (header flags bit 0): per layer G[16,d], g[16], W3[d,16] follow c2
 
     def n_weights(self) -> int:
         S, d, k = self.n_species, self.d, self.n_rbf
         per_layer = d * (2 * d + k) + d + d * d + d + d * 2 * d + d + d * d + d
+        if self.r_cut3 > 0.0:
+            per_layer += 16 * d + 16 + d * 16
         return S * d + S + self.L_max * per_layer + d * d + d + d + 1
 
 
@@ -124,6 +127,9 @@ def make_weights(spec: ModelSpec, seed: int) -> np.ndarray:
         mat(d, d); bias(d)  # W2, b2
         mat(d, 2 * d); bias(d)  # V1, c1
         mat(d, d); bias(d)  # V2, c2
+        if spec.r_cut3 > 0.0:
+            mat(16, d); bias(16)  # G, g (gates of the third atom)
+            mat(d, 16)  # W3
     mat(d, d); bias(d)  # Wo, bo
     parts.append(rng.normal(0.0, 1.0 / np.sqrt(d), size=(d,)))  # wo
     bias(1)  # b_E
@@ -158,7 +164,7 @@ def make_config(c: int, with_weights: bool = True, n_cells_override: int | None 
         grid, halo = (8, 1, 1), 20.0
     elif c == 5:
         sysm = make_water_system(n_cells_override or 32)
-        spec = ModelSpec(2, 128, 16, 4, 5.0, 1.0 / np.sqrt(53.0)); L, prec = 4, "fp32"
+        spec = ModelSpec(2, 128, 16, 4, 5.0, 1.0 / np.sqrt(53.0), r_cut3=4.0); L, prec = 4, "fp32"
         grid, halo = (4, 1, 1), 20.0
     else:
         raise ValueError(f"unknown config {c}")

@@ -72,15 +72,49 @@ def test_full_size_sampled_atom_energies_match_oracle(full):
         assert abs(Ei[i] - E_ref) <= 2e-2 * spread, (i, Ei[i], E_ref, spread)
 
 
-def test_full_size_sampled_atom_force_matches_oracle(full):
-    """F_i of one sampled atom next to a slab face: gradient of the energies of the atoms within L r_c of it, each
-    evaluated on its own complete neighbourhood, i.e. the oracle on the 2 L r_c ball with omega = 1 inside L r_c."""
-    cfg, F = full["cfg"], full["F"]
-    s, m = cfg.system, cfg.model
-    om = oracle_model(m, cfg.weights)
-    x = s.pos[:, 0] % 230.4
-    i = int(np.argmin(np.abs(x - 57.6) + 1e-3 * np.abs(s.pos[:, 1] - 60.0)))
-    pos, cell, sp, k, r = _ball(s, i, 2 * cfg.L * m.r_cut + 0.5)
-    omega = (r <= cfg.L * m.r_cut + 0.25).astype(np.float64)
-    F_ref = O.energy_forces(om, cfg.L, pos, cell, sp, omega=omega)[2][k]
-    assert np.abs(F[i] - F_ref).max() <= 5e-2 * rms(F), (F[i], F_ref, rms(F))
+def test_full_size_sampled_forces_and_energies_match_oracle(full):
+    """More than 200 forces and 700 per-atom energies around three sample points -- on a slab face, at the periodic corner
+    of the box (slab 7 | slab 0 through the wrap), in the middle of a slab -- against the float64 oracle evaluated on the
+    balls of radius 2 L r_c + R around the points (exact for the atoms within R: the K-hop neighbourhood).
+    The oracle needs minutes per ball, so its values are stored by tests/golden/make_full_size_refs.py."""
+    import os
+    cfg, F, Ei = full["cfg"], full["F"], full["Ei"]
+    ref = np.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config4_sampled_oracle.npz"))
+    fi = np.concatenate([ref[f"{n}_force_idx"] for n in ref["names"]])
+    F_ref = np.concatenate([ref[f"{n}_F"] for n in ref["names"]])
+    ei = np.concatenate([ref[f"{n}_energy_idx"] for n in ref["names"]])
+    E_ref = np.concatenate([ref[f"{n}_E_i"] for n in ref["names"]])
+    assert len(fi) >= 200 and len(ei) >= 200
+    # the samples straddle the partition: both sides of the face x = 57.6 and of the wrap x = 0 = 230.4
+    x = cfg.system.pos[:, 0] % 230.4
+    xs = x[ref["slab_face_force_idx"]]
+    assert (xs < 57.6).any() and (xs > 57.6).any()
+    xc = x[ref["box_corner_force_idx"]]
+    assert (xc < 20.0).any() and (xc > 210.0).any()
+    for n in ref["names"]:   # every sample point on its own, then all together
+        k, Fr = ref[f"{n}_force_idx"], ref[f"{n}_F"]
+        assert rms(F[k] - Fr) <= 2e-2 * rms(Fr), n
+    err_rms = rms(F[fi] - F_ref) / rms(F_ref)
+    err_max = np.abs(F[fi] - F_ref).max() / rms(F_ref)
+    print(f"config 4 sampled forces: n={len(fi)} rms={err_rms:.3e} max={err_max:.3e}")
+    assert err_rms <= 2e-2                                   # north_star bound of the bf16-GEMM path
+    assert err_max <= 1e-1                                   # reported; a loose guard against single-atom outliers
+    dE = np.abs(Ei[ei] - E_ref)
+    print(f"config 4 sampled energies: n={len(ei)} max={dE.max():.3e} spread={rms(E_ref - E_ref.mean()):.3e}")
+    assert dE.max() <= 2e-2 * rms(E_ref - E_ref.mean())
+
+
+def test_full_size_edge_list_matches_oracle_hash(full):
+    """Bit-exact edge list at 1,048,576 atoms / 47,189,556 edges: per-atom in-degree and an order-dependent 64-bit hash of
+    (i, j, n) per block of 256 receivers, against the values tests/golden/make_full_size_refs.py computed from the
+    oracle's k-d tree neighbour list."""
+    import os
+    from tests.golden.make_full_size_refs import edge_hash
+    ref = np.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "config4_edge_hash.npz"))
+    g = full["g"]
+    assert g.num_edges == int(ref["n_edges"]) == 47189556
+    recv, send, shift = [t.cpu().numpy() for t in g.export_edges()]
+    assert np.all(np.diff(recv) >= 0)
+    deg, blocks = edge_hash(recv, send, shift, len(full["cfg"].system.pos))
+    assert np.array_equal(deg, ref["degree"].astype(np.int64))
+    assert np.array_equal(blocks, ref["block_hash"])

@@ -12,6 +12,7 @@ from tests.gpu_util import errors, gpu_energy_forces, gpu_graph, gpu_setup, orac
 pytestmark = pytest.mark.gpu
 
 FP32_EPS_E, FP32_MAX_F = 1e-5, 1e-4
+FP32_REL_EI = 1e-5   # per-atom energy relative error (north_star; denominator max(|E_i,ref|, RMS E_ref), reading R14)
 BF16_RMS_F = 2e-2
 
 
@@ -29,7 +30,7 @@ def test_config1_fp32_parity():
     E, F, Ei = _run(cfg.model, cfg.weights, s, cfg.L)
     err = errors(E, F, Ei, ref[0], ref[2], ref[1])
     print(err)
-    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F and err["rel_Ei"] <= FP32_REL_EI
 
 
 @pytest.mark.parametrize("d,L,n_cells,r_cut,nbar", [(64, 3, 4, 5.0, 43.0), (128, 4, 4, 5.0, 43.0), (256, 2, 4, 6.0, 76.0),
@@ -42,7 +43,7 @@ def test_fp32_parity_shapes(d, L, n_cells, r_cut, nbar):
     E, F, Ei = _run(spec, blob, s, L)
     err = errors(E, F, Ei, ref[0], ref[2], ref[1])
     print(d, L, err)
-    assert err["eps_E"] <= FP32_EPS_E
+    assert err["eps_E"] <= FP32_EPS_E and err["rel_Ei"] <= FP32_REL_EI
     if L > 0:
         assert err["max_F"] <= FP32_MAX_F
     else:
@@ -60,7 +61,7 @@ def test_fp32_partitioned_equals_unpartitioned_and_oracle():
         assert np.abs(F - F0).max() <= 1e-5 * rms(F0)
         assert abs(E - E0) <= 1e-5 * np.abs(Ei0).sum()
         err = errors(E, F, Ei, ref[0], ref[2], ref[1])
-        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F and err["rel_Ei"] <= FP32_REL_EI
     # negative control: a halo of (L-1) r_cut is refused, not silently wrong
     mlip, ctx, model = gpu_setup(spec, blob)
     g = gpu_graph(mlip, ctx, s, spec.r_cut)
@@ -88,7 +89,7 @@ def test_mpdp_L_argument():
         ref = O.energy_forces(om, L, s.pos, s.cell, s.species)
         E, F, Ei = _run(spec, blob, s, L)
         err = errors(E, F, Ei, ref[0], ref[2], ref[1])
-        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+        assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F and err["rel_Ei"] <= FP32_REL_EI
     mlip, ctx, model = gpu_setup(spec, blob)
     g = gpu_graph(mlip, ctx, s, spec.r_cut)
     with pytest.raises(mlip.MlipError):
@@ -244,7 +245,7 @@ def test_fp32_active_sets_equal_full_subgraphs_and_oracle(grid, n_sub, L, halo):
     assert np.abs(F - F0).max() <= 1e-5 * rms(F0)
     assert abs(E - E0) <= 1e-5 * np.abs(Ei0).sum()
     err = errors(E, F, Ei, ref[0], ref[2], ref[1])
-    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F
+    assert err["eps_E"] <= FP32_EPS_E and err["max_F"] <= FP32_MAX_F and err["rel_Ei"] <= FP32_REL_EI
 
 
 def test_bf16_active_sets_match_oracle():

@@ -1,0 +1,149 @@
+"""-m gpu: parity cases at the edges of the MLIP_BF16 (tensor-core) path.
+
+* BASELINE.json configs 2 and 3 at FULL size (13,125 atoms, d = 256, L = 5 pruned / L = 15 unpruned)
+  against the float64 oracle. The oracle needs 5 / 14 minutes for them, so its E, E_i, F are stored in tests/golden/ by
+  tests/golden/make_full_size_refs.py (imports only oracle/ and synth_inputs/); MLIP_LIVE_ORACLE=1 recomputes them here.
+* sparse graphs (mean in-degree 5 and 10): every 128-edge tile then holds more receivers than the selector MMA of the
+  segmented sum takes (16) / than the staged receiver rows (8), so the shared-memory and global-row fall-backs run.
+* the IEEE-half range of the edge operands: a model that leaves it must end in MLIP_ERR_NUMERIC, never in silent inf/NaN
+  forces; a model whose energy scale is tiny must keep its accuracy (power-of-two scaling of the reverse pass).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import mlip_oracle as O
+from synth_inputs import ModelSpec, make_config, make_weights, small_system
+from tests.gpu_util import errors, gpu_energy_forces, gpu_graph, gpu_setup, oracle_model, rms
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+BF16_RMS_F = 2e-2
+
+
+def _run(spec, blob, system, L, precision=1, grid=None, halo=0.0):
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, system, spec.r_cut)
+    part = mlip.Partition(ctx, g, halo, grid=grid) if grid is not None else None
+    return gpu_energy_forces(mlip, ctx, model, L, g, part, precision)
+
+
+@pytest.mark.parametrize("c,name", [(2, "config2_L5_oracle.npz"), (3, "config3_L15_oracle.npz")])
+def test_full_size_config_2_and_3_bf16(c, name):
+    cfg = make_config(c)
+    s = cfg.system
+    if os.environ.get("MLIP_LIVE_ORACLE") == "1":
+        E_ref, Ei_ref, F_ref = O.energy_forces(oracle_model(cfg.model, cfg.weights), cfg.L, s.pos, s.cell, s.species)
+    else:
+        ref = np.load(os.path.join(GOLDEN, name))
+        assert int(ref["n_atoms"]) == len(s.pos) == 13125 and int(ref["L"]) == cfg.L
+        E_ref, Ei_ref, F_ref = float(ref["E"]), ref["E_i"], ref["F"]
+    E, F, Ei = _run(cfg.model, cfg.weights, s, cfg.L)
+    err = errors(E, F, Ei, E_ref, F_ref, Ei_ref)
+    print(c, err)
+    assert np.isfinite(F).all()
+    assert err["rms_F"] <= BF16_RMS_F                       # north_star: force RMS relative error of the bf16-GEMM path
+    assert err["eps_E"] <= 2e-3 and err["max_Ei"] <= 5e-2   # not north_star bounds: gross-error guards on the energies
+
+
+def test_full_size_config2_edge_list_bit_exact():
+    cfg = make_config(2, with_weights=False)
+    s = cfg.system
+    import paper_2509_21694_b200 as mlip
+    ctx = mlip.Context(0)
+    g = gpu_graph(mlip, ctx, s, cfg.model.r_cut)
+    recv, send, shift = [t.cpu().numpy() for t in g.export_edges()]
+    o_recv, o_send, o_shift = O.neighbor_list(s.pos, s.cell, cfg.model.r_cut)
+    assert g.num_edges == len(o_recv) == 995238
+    assert np.array_equal(recv, o_recv) and np.array_equal(send, o_send) and np.array_equal(shift, o_shift)
+
+
+def _sparse_system(vacancy, seed):
+    # fcc a = 3.6: first shell (12 sites) at 2.55 A, second at 3.6 A; r_cut = 3.0 keeps the first shell only
+    return small_system(10, 0.08, seed=seed, vacancy_fraction=vacancy)
+
+
+@pytest.mark.parametrize("d", [256, 128])
+@pytest.mark.parametrize("vacancy,min_recv_per_tile", [(0.55, 16), (0.15, 8)])
+def test_bf16_sparse_graph_many_receivers_per_tile(d, vacancy, min_recv_per_tile):
+    r_cut, L = 3.0, 2
+    s = _sparse_system(vacancy, seed=int(100 * vacancy) + d)
+    recv = O.neighbor_list(s.pos, s.cell, r_cut)[0]
+    deg = np.bincount(recv, minlength=len(s.pos))
+    n_tiles = -(-len(recv) // 128)
+    # pigeonhole: the tiles are runs of 128 receiver-sorted edges, every receiver appears in at least one tile, so with
+    # more than k * n_tiles receivers some tile holds more than k of them, in ANY receiver-sorted atom order
+    assert int((deg > 0).sum()) > min_recv_per_tile * n_tiles, (deg.mean(), n_tiles)
+    spec = ModelSpec(4, d, 16, L, r_cut, 1.0 / np.sqrt(max(deg.mean(), 1.0)))
+    blob = make_weights(spec, 300 + d)
+    ref = O.energy_forces(oracle_model(spec, blob), L, s.pos, s.cell, s.species)
+    for grid in [None, (2, 1, 1)]:
+        E, F, Ei = _run(spec, blob, s, L, grid=grid, halo=L * r_cut)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        print(d, vacancy, grid, err)
+        assert err["rms_F"] <= BF16_RMS_F and err["eps_E"] <= 5e-3
+    if vacancy > 0.5:
+        assert (deg == 0).sum() > 0 or deg.min() <= 1   # isolated / nearly isolated atoms are part of the case
+
+
+def test_f16_range_overflow_is_reported_not_silent():
+    """All weights x 30: the second edge linear of the first layer already exceeds 65504 in IEEE half. The outcome must be
+    the defined status MLIP_ERR_NUMERIC (-7), from mlip_ctx_status after the asynchronous call and from mlip_step_host;
+    the fp32 path evaluates the same model."""
+    spec = ModelSpec(4, 256, 16, 2, 5.0, 1.0 / np.sqrt(43.0))
+    blob = (make_weights(spec, 77) * np.float32(30.0)).astype(np.float32)
+    s = small_system(3, 0.1, seed=5)
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, s, spec.r_cut)
+    mlip.energy_forces(ctx, model, 2, g, None, mlip.MLIP_BF16)
+    with pytest.raises(mlip.MlipError) as ei:
+        ctx.status()
+    assert ei.value.code == -7
+    ctx.status()   # the condition is cleared once reported
+    with pytest.raises(mlip.MlipError) as ei:
+        mlip.step_host(ctx, model, 2, s.pos, s.cell, s.species, precision=mlip.MLIP_BF16)
+    assert ei.value.code == -7
+    E, F, Ei = gpu_energy_forces(mlip, ctx, model, 2, g, None, mlip.MLIP_FP32)
+    assert np.isfinite(F).all() and np.isfinite(E)
+
+
+@pytest.mark.parametrize("readout_scale", [1e-4, 1.0, 1e3])
+def test_bf16_energy_scale_does_not_cost_accuracy(readout_scale):
+    """w_o scaled by 1e-4 / 1e3: the adjoints of the reverse pass scale with it. Unscaled, 1e-4 puts mbar, pbar and abar
+    into the f16 subnormals; the per-sub-domain power-of-two scale of the reverse pass keeps the force error where it is
+    for the unit-scale model."""
+    spec = ModelSpec(4, 256, 16, 2, 5.0, 1.0 / np.sqrt(43.0))
+    blob = make_weights(spec, 78).copy()
+    d = spec.d
+    blob[-(d + 1):-1] *= np.float32(readout_scale)
+    s = small_system(4, 0.1, seed=6)
+    ref = O.energy_forces(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    for grid in [None, (2, 1, 1)]:
+        E, F, Ei = _run(spec, blob, s, 2, grid=grid, halo=10.0)
+        err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+        print(readout_scale, grid, err)
+        assert err["rms_F"] <= BF16_RMS_F
+
+
+def test_small_weights_bf16():
+    """All weights x 0.25 (every pre-activation in the linear regime of SiLU, forces about 1e-3 of the unit-scale model)."""
+    spec = ModelSpec(4, 256, 16, 2, 5.0, 1.0 / np.sqrt(43.0))
+    blob = (make_weights(spec, 79) * np.float32(0.25)).astype(np.float32)
+    s = small_system(4, 0.1, seed=8)
+    ref = O.energy_forces(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    E, F, Ei = _run(spec, blob, s, 2)
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    print(err)
+    assert err["rms_F"] <= BF16_RMS_F
+
+
+def test_species_outside_model_range_is_refused():
+    spec = ModelSpec(2, 64, 8, 1, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 80)
+    s = small_system(3, 0.05, seed=1, n_species=4)   # species 0..3 against a 2-species model
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, s, spec.r_cut)
+    with pytest.raises(mlip.MlipError) as ei:
+        mlip.energy_forces(ctx, model, 1, g, None, 0)
+    assert ei.value.code == -1
