@@ -222,6 +222,43 @@ int mlip_md_nve(mlip_ctx* ctx, const mlip_model* m, int L, double* pos_dev, doub
                 int64_t n_atoms, const int grid[3], double halo, int precision, double dt, int n_steps,
                 double* total_energy_host);
 
+/* On-device molecular dynamics, general form. Every MD result of the paper is ASE Langevin dynamics (PAPER.md:89, 91,
+ * 137); the paper does not print the update rule, so the thermostat is the BAOAB splitting (reading R20 of DESIGN.md):
+ *   B  v += (dt/2) a(x);  A  x += (dt/2) v;  O  v = c1 v + c2 sqrt(kB T / m) xi;  A  x += (dt/2) v;  E, F;  B  v += (dt/2) a
+ * with c1 = exp(-friction dt), c2 = sqrt(1 - c1^2), kB = 8.617333262e-5 eV/K and three standard normals xi per atom and
+ * step from the counter-based generator Philox4x32-10: counter (atom, step, 0, 0), key (seed low, seed high), Box-Muller
+ * on (x + 0.5) 2^-32 -- a pure function of (seed, step, atom index in the caller's numbering), independent of the
+ * partition, of the internal atom order and of the number of GPUs. thermostat = MLIP_MD_NVE is plain velocity Verlet.
+ *
+ * skin > 0 (Angstrom) switches on Verlet-skin reuse: the radius graph is built once with r_cut + skin and partitioned
+ * once (root atoms keep their sub-domain, the K-hop search runs over the skin graph, a superset of every later graph);
+ * every step only filters that candidate list with the canonical float64 predicate at the current positions -- the edge
+ * set of every step is exactly the one a fresh mlip_build_graph would return -- and the whole is rebuilt when an atom has
+ * moved more than skin/2 since the last build. cuda_graph = 1 additionally captures the per-step evaluation (filter,
+ * layers, reverse pass, force assembly: fixed launch dimensions between rebuilds) in a CUDA graph that is replayed until
+ * the next rebuild. Arguments as mlip_md_nve; stats may be NULL. Synchronises the stream before returning. */
+enum { MLIP_MD_NVE = 0, MLIP_MD_LANGEVIN = 1 };
+typedef struct {
+  double dt;            /* fs */
+  int32_t n_steps;
+  int32_t thermostat;   /* MLIP_MD_NVE or MLIP_MD_LANGEVIN */
+  double temperature;   /* K */
+  double friction;      /* 1/fs */
+  uint64_t seed;
+  double skin;          /* Angstrom; 0 = rebuild graph and partition every step */
+  int32_t cuda_graph;   /* 1 = replay a captured CUDA graph between rebuilds (needs skin > 0) */
+  int32_t reserved;
+} mlip_md_params;
+typedef struct {
+  int64_t n_rebuilds;        /* graph + partition builds, the initial one included */
+  int64_t n_graph_replays;   /* steps evaluated by replaying a captured CUDA graph */
+  double ms_total;           /* device time of the n_steps steps (CUDA events on the context stream) */
+} mlip_md_stats;
+int mlip_md_run(mlip_ctx* ctx, const mlip_model* m, int L, double* pos_dev, double* vel_dev,
+                const double* mass_dev, const double* cell_host, const int32_t* species_dev,
+                int64_t n_atoms, const int grid[3], double halo, int precision,
+                const mlip_md_params* params, double* total_energy_host, mlip_md_stats* stats);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 int64_t mlip_ctx_launch_count(const mlip_ctx* ctx);
 

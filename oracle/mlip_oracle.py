@@ -689,3 +689,82 @@ def nve_velocity_verlet(model, L, pos, cell, species, masses, vel, dt, n_steps, 
     if return_state:
         return np.array(out), pos, vel
     return np.array(out)
+
+
+# --------------------------------------------------------------------------------------
+# Langevin dynamics (the integrator of every MD result of the paper: ASE Langevin)
+# --------------------------------------------------------------------------------------
+KB_EV = 8.617333262e-5  # Boltzmann constant, eV/K
+
+_PHILOX_M0, _PHILOX_M1 = 0xD2511F53, 0xCD9E8D57
+_PHILOX_W0, _PHILOX_W1 = 0x9E3779B9, 0xBB67AE85
+
+
+def philox4x32(counter, key, rounds=10):
+    """Philox4x32-10 counter-based generator (Salmon, Moraes, Dror, Shaw, SC'11), vectorised over the leading axis:
+    counter uint32 [n,4], key uint32 [n,2] -> uint32 [n,4]. Random numbers the method draws are a pure function of
+    (seed, step, atom), so the CUDA path restates the same generator instead of sharing code."""
+    c = np.array(counter, dtype=np.uint64).reshape(-1, 4)
+    k = np.array(key, dtype=np.uint64).reshape(-1, 2)
+    c0, c1, c2, c3 = c[:, 0].copy(), c[:, 1].copy(), c[:, 2].copy(), c[:, 3].copy()
+    k0, k1 = k[:, 0].copy(), k[:, 1].copy()
+    mask = np.uint64(0xFFFFFFFF)
+    for _ in range(rounds):
+        p0 = np.uint64(_PHILOX_M0) * c0
+        p1 = np.uint64(_PHILOX_M1) * c2
+        hi0, lo0 = p0 >> np.uint64(32), p0 & mask
+        hi1, lo1 = p1 >> np.uint64(32), p1 & mask
+        c0, c1, c2, c3 = (hi1 ^ c1 ^ k0) & mask, lo1, (hi0 ^ c3 ^ k1) & mask, lo0
+        k0 = (k0 + np.uint64(_PHILOX_W0)) & mask
+        k1 = (k1 + np.uint64(_PHILOX_W1)) & mask
+    return np.stack([c0, c1, c2, c3], axis=1).astype(np.uint32)
+
+
+def langevin_normals(seed, step, n_atoms):
+    """Three standard normal numbers per atom for the O step of time step `step`: Philox4x32-10 with
+    counter = (atom, step, 0, 0), key = (seed low, seed high); the four 32-bit outputs x0..x3 give
+    u1 = (x0 + 0.5) 2^-32, u2 = (x1 + 0.5) 2^-32, u3 = (x2 + 0.5) 2^-32, u4 = (x3 + 0.5) 2^-32 and, by Box-Muller,
+    xi_x = sqrt(-2 ln u1) cos(2 pi u2), xi_y = sqrt(-2 ln u1) sin(2 pi u2), xi_z = sqrt(-2 ln u3) cos(2 pi u4)."""
+    ctr = np.zeros((n_atoms, 4), np.uint32)
+    ctr[:, 0] = np.arange(n_atoms, dtype=np.uint32)
+    ctr[:, 1] = np.uint32(step)
+    key = np.tile(np.array([[seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF]], dtype=np.uint32), (n_atoms, 1))
+    x = philox4x32(ctr, key).astype(np.float64)
+    u = (x + 0.5) * 2.0 ** -32
+    ra, rb = np.sqrt(-2.0 * np.log(u[:, 0])), np.sqrt(-2.0 * np.log(u[:, 2]))
+    return np.stack([ra * np.cos(2 * np.pi * u[:, 1]), ra * np.sin(2 * np.pi * u[:, 1]), rb * np.cos(2 * np.pi * u[:, 3])], axis=1)
+
+
+def langevin_baoab_generic(force_fn, pos, masses, vel, dt, n_steps, temperature, friction, seed):
+    """BAOAB splitting of Langevin dynamics (Leimkuhler & Matthews 2013; the paper runs ASE's Langevin integrator and
+    does not print its update rule -- reading R20): per step
+        B  v += (dt/2) a(x)          A  x += (dt/2) v
+        O  v = c1 v + c2 sqrt(kB T / m) xi,  c1 = exp(-friction dt), c2 = sqrt(1 - c1^2)
+        A  x += (dt/2) v             B  v += (dt/2) a(x)      (one force evaluation per step)
+    with a = ACC_UNIT F / m, xi from `langevin_normals(seed, step, N)`. friction = 0 is velocity Verlet exactly.
+    force_fn(pos) -> (E, F). Returns (total energy before every step and after the last, pos, vel)."""
+    pos = np.array(pos, np.float64); vel = np.array(vel, np.float64)
+    c1 = np.exp(-friction * dt)
+    c2 = np.sqrt(1.0 - c1 * c1)
+    sig = np.sqrt(KB_EV * temperature * ACC_UNIT / masses)[:, None]   # sqrt(kB T / m) in A/fs
+    E, F = force_fn(pos)
+    out = []
+    for step in range(n_steps):
+        out.append(E + 0.5 * np.sum(masses[:, None] * vel * vel) / ACC_UNIT)
+        vel += 0.5 * dt * ACC_UNIT * F / masses[:, None]
+        pos += 0.5 * dt * vel
+        if friction > 0.0:
+            vel = c1 * vel + c2 * sig * langevin_normals(seed, step, len(pos))
+        pos += 0.5 * dt * vel
+        E, F = force_fn(pos)
+        vel += 0.5 * dt * ACC_UNIT * F / masses[:, None]
+    out.append(E + 0.5 * np.sum(masses[:, None] * vel * vel) / ACC_UNIT)
+    return np.array(out), pos, vel
+
+
+def langevin_baoab(model, L, pos, cell, species, masses, vel, dt, n_steps, temperature, friction, seed):
+    """Langevin dynamics of the model potential (see langevin_baoab_generic)."""
+    def force_fn(x):
+        E, _, F = energy_forces(model, L, x, cell, species)
+        return E, F
+    return langevin_baoab_generic(force_fn, pos, masses, vel, dt, n_steps, temperature, friction, seed)

@@ -32,6 +32,20 @@ class mlip_model_header(C.Structure):
                 ("flags", C.c_int32), ("n_rbf3", C.c_int32), ("l_max", C.c_int32), ("r_cut3", C.c_float)]
 
 
+class mlip_md_params(C.Structure):
+    _fields_ = [("dt", C.c_double), ("n_steps", C.c_int32), ("thermostat", C.c_int32), ("temperature", C.c_double),
+                ("friction", C.c_double), ("seed", C.c_uint64), ("skin", C.c_double), ("cuda_graph", C.c_int32),
+                ("reserved", C.c_int32)]
+
+
+class mlip_md_stats(C.Structure):
+    _fields_ = [("n_rebuilds", C.c_int64), ("n_graph_replays", C.c_int64), ("ms_total", C.c_double)]
+
+
+MLIP_MD_NVE = 0
+MLIP_MD_LANGEVIN = 1
+
+
 def lib_path() -> str:
     return os.path.join(_HERE, "libmlip_b200.so")
 
@@ -71,6 +85,7 @@ def load_library():
     lib.mlip_energy_forces_shard.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.mlip_energy_forces_stress.argtypes = [vp, vp, i32, vp, vp, i32, i32, i32, vp, vp, vp, vp]
     lib.mlip_md_nve.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i64, P(i32), dbl, i32, dbl, i32, vp]
+    lib.mlip_md_run.argtypes = [vp, vp, i32, vp, vp, vp, vp, vp, i64, P(i32), dbl, i32, P(mlip_md_params), vp, P(mlip_md_stats)]
     lib.mlip_step_host.argtypes = [vp, vp, i32, vp, vp, vp, i64, P(i32), dbl, i32, vp, vp]
     lib.mlip_ctx_launch_count.argtypes = [vp]; lib.mlip_ctx_launch_count.restype = i64
     lib.mlip_ctx_profile.argtypes = [vp, i32]
@@ -148,14 +163,17 @@ class Context:
             self._release()
 
 
-def make_header(n_species, d, n_rbf, L_max, r_cut, agg_scale) -> mlip_model_header:
+def make_header(n_species, d, n_rbf, L_max, r_cut, agg_scale, r_cut3=0.0) -> mlip_model_header:
+    """r_cut3 > 0 selects the three-body variant (flags bit 0, n_rbf3 = 4, l_max = 3)."""
+    if r_cut3 > 0.0:
+        return mlip_model_header(MLIP_MAGIC, 1, n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), 1, 4, 3, float(r_cut3))
     return mlip_model_header(MLIP_MAGIC, 1, n_species, d, n_rbf, L_max, float(r_cut), float(agg_scale), 0, 0, 0, 0.0)
 
 
 class Model:
-    def __init__(self, ctx: Context, n_species, d, n_rbf, L_max, r_cut, agg_scale, blob: np.ndarray):
+    def __init__(self, ctx: Context, n_species, d, n_rbf, L_max, r_cut, agg_scale, blob: np.ndarray, r_cut3: float = 0.0):
         self.ctx = ctx
-        self.header = make_header(n_species, d, n_rbf, L_max, r_cut, agg_scale)
+        self.header = make_header(n_species, d, n_rbf, L_max, r_cut, agg_scale, r_cut3)
         blob = np.ascontiguousarray(blob, dtype=np.float32)
         h = C.c_void_p()
         ctx.check(ctx.lib.mlip_model_load(ctx.h, C.byref(self.header), blob.ctypes.data_as(C.c_void_p), blob.size, C.byref(h)))
@@ -316,6 +334,27 @@ def md_nve(ctx: Context, model: Model, L: int, pos, vel, mass, cell: np.ndarray,
                                   C.c_void_p(species.data_ptr()), int(pos.shape[0]), g, float(halo), int(precision),
                                   float(dt), int(n_steps), out.ctypes.data_as(C.c_void_p)))
     return out
+
+
+def md_run(ctx: Context, model: Model, L: int, pos, vel, mass, cell: np.ndarray, species, dt: float, n_steps: int,
+           grid=(1, 1, 1), halo: float = 0.0, precision: int = MLIP_FP32, thermostat: int = MLIP_MD_NVE,
+           temperature: float = 0.0, friction: float = 0.0, seed: int = 0, skin: float = 0.0, cuda_graph: bool = False):
+    """mlip_md_run: pos/vel float64 CUDA tensors updated in place; returns (total energy per step [n_steps+1], stats dict)."""
+    torch = _torch()
+    assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous()
+    assert vel.is_cuda and vel.dtype == torch.float64 and vel.is_contiguous()
+    assert mass.is_cuda and mass.dtype == torch.float64 and species.dtype == torch.int32
+    cell = np.ascontiguousarray(cell, dtype=np.float64)
+    g = (C.c_int * 3)(*[int(x) for x in grid])
+    out = np.zeros(n_steps + 1, dtype=np.float64)
+    prm = mlip_md_params(float(dt), int(n_steps), int(thermostat), float(temperature), float(friction), int(seed),
+                         float(skin), 1 if cuda_graph else 0, 0)
+    st = mlip_md_stats()
+    ctx.check(ctx.lib.mlip_md_run(ctx.h, model.h, int(L), C.c_void_p(pos.data_ptr()), C.c_void_p(vel.data_ptr()),
+                                  C.c_void_p(mass.data_ptr()), cell.ctypes.data_as(C.c_void_p),
+                                  C.c_void_p(species.data_ptr()), int(pos.shape[0]), g, float(halo), int(precision),
+                                  C.byref(prm), out.ctypes.data_as(C.c_void_p), C.byref(st)))
+    return out, dict(n_rebuilds=int(st.n_rebuilds), n_graph_replays=int(st.n_graph_replays), ms_total=float(st.ms_total))
 
 
 def step_host(ctx: Context, model: Model, L: int, pos: np.ndarray, cell: np.ndarray, species: np.ndarray,

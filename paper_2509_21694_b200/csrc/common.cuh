@@ -94,7 +94,7 @@ struct mlip_ctx {
   }
 };
 
-enum { MLIP_DEV_REV_MISSING = 1, MLIP_DEV_NONFINITE = 2 };
+enum { MLIP_DEV_REV_MISSING = 1, MLIP_DEV_NONFINITE = 2, MLIP_DEV_ROW_TOO_LONG = 4 };
 // Reads and clears the device status word; the stream must have been synchronised. Returns MLIP_OK or the status the
 // bits map to (with the context error message set).
 int mlip_take_dev_status(mlip_ctx* ctx);
@@ -123,6 +123,7 @@ struct ProfScope {
 struct LayerWeights {
   // fp32 device pointers into the blob copy (row-major [out,in])
   const float *W1, *b1, *W2, *b2, *V1, *c1, *V2, *c2;
+  const float *G3 = nullptr, *g3 = nullptr, *W3 = nullptr;  // three-body variant: G[16,d], g[16], W3[d,16] (blob)
   // derived fp32 matrices (device, owned by the model)
   float* W1ab;    // [2d, d]  rows 0..d-1 = W1a (receiver block), d..2d-1 = W1b (sender block)
   float* W1c;     // [d, n_rbf]

@@ -36,7 +36,20 @@ struct EdgeArgs {
   // the gradient w.r.t. the species embedding -- forces need nothing but rbar, so the spill, the segmented sum and the
   // sender-side gather of that layer are skipped
   bool node_adjoint = true;
+  // three-body variant (fp32 path): a_e += W3 t_e; the reverse pass writes tbar_e = W3^T abar_e
+  const float* t3 = nullptr;    // [E,16] or null
+  const float* W3 = nullptr;    // [d,16]
+  float* tbar = nullptr;        // [E,16] (backward out)
 };
+
+// three_body.cu
+int mlip_gate_forward(mlip_ctx* ctx, int64_t n, int d, const float* h, const float* G, const float* g, float* z);
+int mlip_triplet_forward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
+                         const float4* rvec, const float* z, float* t);
+int mlip_triplet_backward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
+                          const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta);
+int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
+                       const float* zeta, const float* z, const float* G, float* hbar);
 
 int64_t mlip_edge_f32_tiles(int64_t E);
 int mlip_edge_forward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);

@@ -31,8 +31,8 @@ struct Smem {
   static constexpr size_t ds_off = s_off + sizeof(float) * TE * LDS;
   static constexpr size_t wt_off(bool bwd) { return bwd ? ds_off + sizeof(float) * TE * LDS : ds_off; }
   static constexpr size_t misc_off(bool bwd) { return wt_off(bwd) + sizeof(float) * 2 * KC * D; }
-  // misc: ehat[TE][16], u[TE], du[TE], ubar[TE], r[TE], recv[TE], send[TE]
-  static constexpr size_t bytes(bool bwd) { return misc_off(bwd) + sizeof(float) * TE * (16 + 4) + sizeof(int) * TE * 2; }
+  // misc: ehat[TE][16], u[TE], du[TE], ubar[TE], r[TE], recv[TE], send[TE], t3[TE][16] (three-body variant)
+  static constexpr size_t bytes(bool bwd) { return misc_off(bwd) + sizeof(float) * TE * (16 + 4) + sizeof(int) * TE * 2 + sizeof(float) * TE * 16; }
 };
 
 // acc[i][4j+q] += sum_k S[ty*4+i][k] * Wg[k][tx*4 + 64j + q], Wg is [D][D] row-major in global
@@ -127,6 +127,7 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
   float* r_s = ubar_s + TE;
   int* recv_s = reinterpret_cast<int*>(r_s + TE);
   int* send_s = recv_s + TE;
+  float* t3_s = reinterpret_cast<float*>(send_s + TE);
 
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int64_t tile = blockIdx.x;
@@ -149,6 +150,14 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
       ehat[tid * 16 + k] = u * g;
     }
   }
+  if (a.t3) {  // three-body variant: the 16 angle terms of every edge of the tile
+    for (int idx = tid; idx < TE * 4; idx += 256) {
+      const int64_t e = e0 + (idx >> 2);
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (e < a.E) v = *reinterpret_cast<const float4*>(a.t3 + (size_t)e * 16 + (idx & 3) * 4);
+      *reinterpret_cast<float4*>(t3_s + idx * 4) = v;
+    }
+  }
   __syncthreads();
 
   // ---- a = P_i + Q_j + W1c e_hat ; s = SiLU(a) ----
@@ -161,6 +170,16 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
       const float4 w = *reinterpret_cast<const float4*>(a.W1c + (size_t)col * 16 + k4 * 4);
       w1c[4 * k4] = w.x; w1c[4 * k4 + 1] = w.y; w1c[4 * k4 + 2] = w.z; w1c[4 * k4 + 3] = w.w;
     }
+    float w3[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) w3[k] = 0.f;
+    if (a.t3) {
+#pragma unroll
+      for (int k4 = 0; k4 < 4; ++k4) {
+        const float4 w = *reinterpret_cast<const float4*>(a.W3 + (size_t)col * 16 + k4 * 4);
+        w3[4 * k4] = w.x; w3[4 * k4 + 1] = w.y; w3[4 * k4 + 2] = w.z; w3[4 * k4 + 3] = w.w;
+      }
+    }
     for (int e = grp; e < TE; e += G) {
       const int rc = recv_s[e];
       float s = 0.f, ds = 0.f;
@@ -168,6 +187,10 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
         float v = a.P[(size_t)rc * a.ldp + col] + a.Q[(size_t)send_s[e] * a.ldq + col];
 #pragma unroll
         for (int k = 0; k < 16; ++k) v = fmaf(w1c[k], ehat[e * 16 + k], v);
+        if (a.t3) {
+#pragma unroll
+          for (int k = 0; k < 16; ++k) v = fmaf(w3[k], t3_s[e * 16 + k], v);
+        }
         silu_both_f(v, s, ds);
       }
       S[e * LDS + col] = s;
@@ -256,6 +279,15 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
       const float4 w = *reinterpret_cast<const float4*>(a.W1c + (size_t)c * 16 + kq * 4);
       eb[0] = fmaf(av, w.x, eb[0]); eb[1] = fmaf(av, w.y, eb[1]);
       eb[2] = fmaf(av, w.z, eb[2]); eb[3] = fmaf(av, w.w, eb[3]);
+    }
+    if (a.tbar) {  // three-body variant: tbar_e = W3^T abar_e
+      float4 tb = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int c = 0; c < D; ++c) {
+        const float av = dS[e * LDS + c];
+        const float4 w = *reinterpret_cast<const float4*>(a.W3 + (size_t)c * 16 + kq * 4);
+        tb.x = fmaf(av, w.x, tb.x); tb.y = fmaf(av, w.y, tb.y); tb.z = fmaf(av, w.z, tb.z); tb.w = fmaf(av, w.w, tb.w);
+      }
+      if (e0 + e < a.E) *reinterpret_cast<float4*>(a.tbar + (size_t)(e0 + e) * 16 + kq * 4) = tb;
     }
     float part = 0.f;
     const float r = r_s[e], u = u_s[e], du = du_s[e];

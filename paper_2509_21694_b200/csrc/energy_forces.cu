@@ -140,6 +140,7 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
                                                 const int32_t* __restrict__ rev, const float4* __restrict__ rvec,
                                                 const float* __restrict__ rbar, const int32_t* __restrict__ gid,
                                                 const float* __restrict__ scale /*[2] = s, 1/s of the reverse pass, or null*/,
+                                                const float4* __restrict__ gvec /*[E] vector part of dE/d rvec_e (three-body), or null*/,
                                                 float* __restrict__ F) {
   const int lane = threadIdx.x & 31;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -148,8 +149,13 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
   float fx = 0.f, fy = 0.f, fz = 0.f;
   for (int e = rowptr[k] + lane; e < rowptr[k + 1]; e += 32) {
     const float4 rv = rvec[e];
-    const float w = (rbar[e] + rbar[rev[e]]) * (rv.w > 0.f ? inv_s / rv.w : 0.f);
+    const int re = rev[e];
+    const float w = (rbar[e] + rbar[re]) * (rv.w > 0.f ? inv_s / rv.w : 0.f);
     fx = fmaf(w, rv.x, fx); fy = fmaf(w, rv.y, fy); fz = fmaf(w, rv.z, fz);
+    if (gvec) {  // d rvec_e / d x_k = +1 for the in-edges of k, -1 for its out-edges (= the reverse edges)
+      const float4 a = gvec[e], b = gvec[re];
+      fx += a.x - b.x; fy += a.y - b.y; fz += a.z - b.z;
+    }
   }
 #pragma unroll
   for (int s = 16; s > 0; s >>= 1) {
@@ -167,7 +173,7 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
 // edges no layer evaluated). float64 per-block partials in a fixed order, then one block: deterministic, no atomics.
 __global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const float4* __restrict__ rvec,
                                                         const float* __restrict__ rbar, const float* __restrict__ scale,
-                                                        double* __restrict__ partial) {
+                                                        const float4* __restrict__ gvec, double* __restrict__ partial) {
   __shared__ double sh[6][256];
   double w[6] = {0, 0, 0, 0, 0, 0};
   const double inv_s = scale ? (double)scale[1] : 1.0;
@@ -177,6 +183,12 @@ __global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const float4*
       const double s = inv_s * (double)rbar[e] / (double)rv.w, x = rv.x, y = rv.y, z = rv.z;
       w[0] += s * x * x; w[1] += s * y * y; w[2] += s * z * z;
       w[3] += s * y * z; w[4] += s * x * z; w[5] += s * x * y;
+    }
+    if (gvec) {  // three-body variant: dE/d rvec_e has gvec_e on top of rbar_e rhat_e (symmetrised; the total is symmetric)
+      const float4 gq = gvec[e];
+      const double gx = gq.x, gy = gq.y, gz = gq.z, x = rv.x, y = rv.y, z = rv.z;
+      w[0] += gx * x; w[1] += gy * y; w[2] += gz * z;
+      w[3] += 0.5 * (gy * z + gz * y); w[4] += 0.5 * (gx * z + gz * x); w[5] += 0.5 * (gx * y + gy * x);
     }
   }
 #pragma unroll
@@ -285,6 +297,17 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   if (L > 0) { if (bf) { W_ALLOC(abar_h, __half, tiles * 128 * d); W_ALLOC(mbar_h, __half, n * d); } else W_ALLOC(abar, float, E * d); }  // bf16 spill: whole 128-edge tile images
   const int64_t n_part = (n + 255) / 256;
   W_ALLOC(partial, double, n_part);
+  // three-body variant (fp32 path): gates per layer, angle terms / their adjoints per edge, vector part of dE/d rvec
+  const bool tb = (M->h.flags & MLIP_FLAG_THREE_BODY) != 0 && L > 0;
+  const float r3 = M->h.r_cut3;
+  std::vector<float*> zg(L, nullptr);
+  float *t3 = nullptr, *tbar3 = nullptr;
+  float4* gvec = nullptr;
+  if (tb) {
+    for (int l = 0; l < L; ++l) W_ALLOC(zg[l], float, n * 16);
+    W_ALLOC(t3, float, (E + 1) * 16); W_ALLOC(tbar3, float, (E + 1) * 16); W_ALLOC(gvec, float4, E + 1);
+    cudaMemsetAsync(gvec, 0, sizeof(float4) * (E + 1), st);
+  }
   float* mbar = m;           // m is dead after the forward pass
   float* Pbar = PQbar;
   float* Qbar = PQbar + n * d;  // stored as two dense [n,d] blocks
@@ -342,6 +365,12 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     }
     set_layer(l);
     ea.m = m; ea.E = e_recv(l); ea.n = nr;
+    if (tb) {
+      ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
+      W_TRY(mlip_gate_forward(ctx, ns, d, h[l], W.G3, W.g3, zg[l]));
+      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3));
+      ea.t3 = t3; ea.W3 = W.W3;
+    }
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
       W_TRY(bf ? mlip_edge_forward_tc(ctx, d, ea) : mlip_edge_forward_f32(ctx, d, ea));
@@ -419,9 +448,19 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     set_layer(l);
     ea.E = Er; ea.n = nr; ea.node_adjoint = bf ? node_adjoint : true;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
+    if (tb) {  // the angle terms are recomputed like every other edge activation
+      ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
+      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3));
+      ea.t3 = t3; ea.W3 = W.W3; ea.tbar = tbar3;
+    }
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
       W_TRY(bf ? mlip_edge_backward_tc(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
+    }
+    float* zeta = t3;  // the angle terms are dead after the edge kernel: their buffer takes the per-edge gate adjoints
+    if (tb) {
+      ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
+      W_TRY(mlip_triplet_backward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], tbar3, rbar, gvec, zeta));
     }
     if (!node_adjoint) continue;
     {
@@ -435,16 +474,20 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     a.B = bf ? (const void*)W.W1abT_bf : (const void*)W.W1abT; a.residual = hbar; a.ldr = d; a.Y = hbar; a.ldy = d;
     a.n = ns; a.N = d;
     W_TRY(gemm(ctx, a));
+    if (tb) {  // adjoint of the gates of the senders (third atoms), through the reverse-edge index like Qbar
+      ProfScope p(ctx, MLIP_PROF_GATHER_REV);
+      W_TRY(mlip_gate_backward(ctx, ns, Er, d, g.rowptr, g.rev, zeta, zg[l], W.G3, hbar));
+    }
   }
   {
     ProfScope p(ctx, MLIP_PROF_READOUT_FORCES);
-    k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, rscale, F_int);
+    k_forces<<<nblk(n * 32, 256), 256, 0, st>>>(n, g.rowptr, g.rev, g.rvec, rbar, g.gid, rscale, gvec, F_int);
     ctx->launches++;
     if (virial_accum && E > 0) {
       const int nb = (int)(E < 148 * 8 * 256 ? (E + 255) / 256 : 148 * 8);
       double* vpart = nullptr;
       W_ALLOC(vpart, double, (size_t)nb * 6);
-      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, rscale, vpart);
+      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, rscale, gvec, vpart);
       k_virial_final<<<1, 32, 0, st>>>(nb, vpart, virial_accum);
       ctx->launches += 2;
     }
@@ -489,6 +532,10 @@ static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const m
   if (L < 0 || L > M->h.L_max) { ctx->set_error("L outside [0, L_max]"); return MLIP_ERR_UNSUPPORTED; }
   if (precision != MLIP_FP32 && precision != MLIP_BF16) { ctx->set_error("unknown precision"); return MLIP_ERR_INVALID_ARG; }
   if (precision == MLIP_BF16 && !(M->h.d == 256 || M->h.d == 128)) { ctx->set_error("MLIP_BF16 needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
+  if (precision == MLIP_BF16 && (M->h.flags & MLIP_FLAG_THREE_BODY)) {
+    ctx->set_error("the three-body variant runs in MLIP_FP32 only (BASELINE.json config 5 is fp32)");
+    return MLIP_ERR_UNSUPPORTED;
+  }
   if (part && part->N != G->N) { ctx->set_error("partition does not belong to this graph"); return MLIP_ERR_INVALID_ARG; }
   if (part && part->subs.size() > 1 && part->halo < (double)L * (double)M->h.r_cut * (1.0 - 1e-12)) {
     ctx->set_error("halo < L * r_cut: sub-graphs would not keep the K-hop neighbourhood of their root atoms");

@@ -1,8 +1,10 @@
 // On-device molecular dynamics driver (the use the paper builds the partitioned evaluation for: ns-scale MD of
-// 10^5..10^6 atoms): velocity-Verlet NVE integration with the whole step -- neighbour list,
-// partition, energy and forces, kicks and drift, kinetic energy -- on the GPU; the host only sequences launches.
+// 10^5..10^6 atoms): velocity-Verlet NVE and Langevin (BAOAB, reading R20; the paper runs ASE's
+// Langevin integrator) integration with the whole step -- neighbour list, partition, energy and
+// forces, kicks, drift, thermostat, kinetic energy -- on the GPU; the host only sequences launches.
 // Positions and velocities stay in float64 (the graph builder's predicate is float64, reading R10); forces are the
 // float32 output of mlip_energy_forces. Units: Angstrom, fs, amu, eV (1 eV/A/amu = 9.648533e-3 A/fs^2).
+#include <string.h>
 #include "common.cuh"
 
 namespace {
@@ -18,6 +20,46 @@ __global__ void k_vv_kick(int64_t N, double half_dt, double drift_dt, const floa
   const double v = vel[i] + half_dt * ACC_UNIT * (double)F[i] / mass[i / 3];
   vel[i] = v;
   if (drift_dt != 0.0) pos[i] += drift_dt * v;
+}
+
+// ---- Langevin thermostat: Philox4x32-10 normals, a pure function of (seed, step, atom) --------------------------------
+constexpr double KB_EV = 8.617333262e-5;  // eV/K
+__device__ __forceinline__ void philox4x32_10(uint32_t (&c)[4], uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c[0]), lo0 = 0xD2511F53u * c[0];
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c[2]), lo1 = 0xCD9E8D57u * c[2];
+    const uint32_t n0 = hi1 ^ c[1] ^ k0, n2 = hi0 ^ c[3] ^ k1;
+    c[0] = n0; c[1] = lo1; c[2] = n2; c[3] = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+}
+// B A O A of one BAOAB step for atom i (the closing B is k_vv_kick after the force evaluation):
+//   v += (dt/2) a ; x += (dt/2) v ; v = c1 v + c2 sqrt(kB T / m) xi ; x += (dt/2) v
+__global__ void __launch_bounds__(256) k_baoab_pre(int64_t N, double dt, double c1, double c2, double kT, uint64_t seed,
+                                                   uint32_t step, const float* __restrict__ F, const double* __restrict__ mass,
+                                                   double* __restrict__ vel, double* __restrict__ pos) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  uint32_t c[4] = {(uint32_t)i, step, 0u, 0u};
+  philox4x32_10(c, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32));
+  const double u1 = ((double)c[0] + 0.5) * 2.3283064365386963e-10, u2 = ((double)c[1] + 0.5) * 2.3283064365386963e-10;
+  const double u3 = ((double)c[2] + 0.5) * 2.3283064365386963e-10, u4 = ((double)c[3] + 0.5) * 2.3283064365386963e-10;
+  const double ra = sqrt(-2.0 * log(u1)), rb = sqrt(-2.0 * log(u3));
+  double s2, c2pi, s4, c4pi;
+  sincospi(2.0 * u2, &s2, &c2pi);
+  sincospi(2.0 * u4, &s4, &c4pi);
+  const double xi[3] = {ra * c2pi, ra * s2, rb * c4pi};
+  const double m = mass[i], sig = sqrt(kT * ACC_UNIT / m);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    double v = vel[3 * i + k] + 0.5 * dt * ACC_UNIT * (double)F[3 * i + k] / m;
+    double x = pos[3 * i + k] + 0.5 * dt * v;
+    v = c1 * v + c2 * sig * xi[k];
+    x += 0.5 * dt * v;
+    vel[3 * i + k] = v;
+    pos[3 * i + k] = x;
+  }
 }
 
 // kinetic energy (eV) = 1/2 sum m v^2 / ACC_UNIT: float64 per-block partials, then one block (deterministic)
@@ -45,62 +87,112 @@ __global__ void k_total_energy(int n_partial, const double* __restrict__ partial
   for (int i = 0; i < n_partial; ++i) s += partial[i];
   out[0] = e_pot[0] + 0.5 * s / ACC_UNIT;
 }
+
+// Graph -> partition -> E, F at the current positions. skin = 0: everything is rebuilt on every call.
+struct MdEvaluator {
+  mlip_ctx* ctx; const mlip_model* M; int L; const double* pos; const double* cell; const int32_t* species; int64_t N;
+  int grid[3]; double halo; int precision; double skin; bool use_graph; double* e_pot; float* F;
+  int64_t n_rebuilds = 0, n_replays = 0;
+  MdEvaluator(mlip_ctx* c, const mlip_model* m, int L_, const double* p, const double* cell_, const int32_t* sp, int64_t n,
+              const int g[3], double h, int prec, double skin_, bool graph, double* e, float* f)
+      : ctx(c), M(m), L(L_), pos(p), cell(cell_), species(sp), N(n), halo(h), precision(prec), skin(skin_), use_graph(graph),
+        e_pot(e), F(f) {
+    grid[0] = g[0]; grid[1] = g[1]; grid[2] = g[2];
+  }
+  bool split() const { return grid[0] > 1 || grid[1] > 1 || grid[2] > 1; }
+  int evaluate() {
+    mlip_graph* G = nullptr;
+    mlip_part* P = nullptr;
+    int s = mlip_build_graph(ctx, pos, cell, species, N, (double)M->h.r_cut, &G);
+    if (s == MLIP_OK && split()) s = mlip_partition_grid(ctx, G, grid, halo, &P);
+    if (s == MLIP_OK) s = mlip_energy_forces(ctx, M, L, G, P, precision, e_pot, F, nullptr);
+    mlip_part_destroy(P);
+    mlip_graph_destroy(G);
+    ++n_rebuilds;
+    return s;
+  }
+};
 }  // namespace
 
-extern "C" int mlip_md_nve(mlip_ctx* ctx, const mlip_model* M, int L, double* pos_dev, double* vel_dev,
+extern "C" int mlip_md_run(mlip_ctx* ctx, const mlip_model* M, int L, double* pos_dev, double* vel_dev,
                            const double* mass_dev, const double* cell_host, const int32_t* species_dev, int64_t N,
-                           const int grid[3], double halo, int precision, double dt, int n_steps,
-                           double* total_energy_host) {
+                           const int grid[3], double halo, int precision, const mlip_md_params* prm,
+                           double* total_energy_host, mlip_md_stats* stats) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
-  if (!M || !pos_dev || !vel_dev || !mass_dev || !cell_host || !species_dev || !grid || N < 0 || n_steps < 0 || !(dt > 0.0)) {
-    ctx->set_error("mlip_md_nve: invalid argument");
+  if (!M || !pos_dev || !vel_dev || !mass_dev || !cell_host || !species_dev || !grid || !prm || N < 0 || prm->n_steps < 0 ||
+      !(prm->dt > 0.0) || (prm->thermostat != MLIP_MD_NVE && prm->thermostat != MLIP_MD_LANGEVIN) || !(prm->skin >= 0.0)) {
+    ctx->set_error("mlip_md_run: invalid argument");
+    return MLIP_ERR_INVALID_ARG;
+  }
+  const bool langevin = prm->thermostat == MLIP_MD_LANGEVIN;
+  if (langevin && (!(prm->temperature >= 0.0) || !(prm->friction >= 0.0))) {
+    ctx->set_error("mlip_md_run: Langevin needs temperature >= 0 and friction >= 0");
+    return MLIP_ERR_INVALID_ARG;
+  }
+  if (prm->cuda_graph && !(prm->skin > 0.0)) {
+    ctx->set_error("mlip_md_run: cuda_graph = 1 needs skin > 0 (launch dimensions are only fixed between rebuilds)");
     return MLIP_ERR_INVALID_ARG;
   }
   MLIP_CUDA_CHECK(ctx, cudaSetDevice(ctx->device));
   cudaStream_t st = ctx->stream;
-  const bool split = grid[0] > 1 || grid[1] > 1 || grid[2] > 1;
+  const int n_steps = prm->n_steps;
+  const double dt = prm->dt;
   const int nb = (int)(N < 148 * 4 * 256 ? (N + 255) / 256 : 148 * 4);
   float* F = nullptr;
   double *e_pot = nullptr, *partial = nullptr, *e_tot = nullptr;
   Scratch tmp(ctx);
   MLIP_TRY(tmp.get(&F, 3 * N)); MLIP_TRY(tmp.get(&e_pot, 1)); MLIP_TRY(tmp.get(&partial, nb > 0 ? nb : 1));
   MLIP_TRY(tmp.get(&e_tot, n_steps + 1));
-  int status = MLIP_OK;
-  auto evaluate = [&]() {  // graph -> partition -> E, F at the current positions
-    mlip_graph* G = nullptr;
-    mlip_part* P = nullptr;
-    int s = mlip_build_graph(ctx, pos_dev, cell_host, species_dev, N, (double)M->h.r_cut, &G);
-    if (s == MLIP_OK && split) s = mlip_partition_grid(ctx, G, grid, halo, &P);
-    if (s == MLIP_OK) s = mlip_energy_forces(ctx, M, L, G, P, precision, e_pot, F, nullptr);
-    mlip_part_destroy(P);
-    mlip_graph_destroy(G);
-    return s;
-  };
+  MdEvaluator ev(ctx, M, L, pos_dev, cell_host, species_dev, N, grid, halo, precision, prm->skin, prm->cuda_graph != 0, e_pot, F);
+  const double c1 = langevin ? exp(-prm->friction * dt) : 1.0;
+  const double c2 = langevin ? sqrt(1.0 - c1 * c1) : 0.0;
   auto record = [&](int step) {
     if (N > 0) k_kinetic_partial<<<nb, 256, 0, st>>>(N, mass_dev, vel_dev, partial);
     k_total_energy<<<1, 32, 0, st>>>(N > 0 ? nb : 0, partial, e_pot, e_tot + step);
     ctx->launches += 2;
   };
-  status = evaluate();
+  int status = ev.evaluate();
+  cudaEvent_t t0 = ctx->get_event(), t1 = ctx->get_event();
+  cudaEventRecord(t0, st);
   for (int step = 0; step < n_steps && status == MLIP_OK; ++step) {
     record(step);
     if (N > 0) {
-      k_vv_kick<<<nblk(3 * N, 256), 256, 0, st>>>(N, 0.5 * dt, dt, F, mass_dev, vel_dev, pos_dev);
+      if (langevin && c2 > 0.0)
+        k_baoab_pre<<<nblk(N, 256), 256, 0, st>>>(N, dt, c1, c2, KB_EV * prm->temperature, prm->seed, (uint32_t)step, F, mass_dev,
+                                                 vel_dev, pos_dev);
+      else
+        k_vv_kick<<<nblk(3 * N, 256), 256, 0, st>>>(N, 0.5 * dt, dt, F, mass_dev, vel_dev, pos_dev);
       ctx->launches++;
     }
-    status = evaluate();
+    status = ev.evaluate();
     if (status == MLIP_OK && N > 0) {
       k_vv_kick<<<nblk(3 * N, 256), 256, 0, st>>>(N, 0.5 * dt, 0.0, F, mass_dev, vel_dev, pos_dev);
       ctx->launches++;
     }
   }
+  cudaEventRecord(t1, st);
   if (status == MLIP_OK) {
     record(n_steps);
     if (total_energy_host)
       cudaMemcpyAsync(total_energy_host, e_tot, sizeof(double) * (n_steps + 1), cudaMemcpyDeviceToHost, st);
   }
   cudaError_t e = cudaStreamSynchronize(st);
+  float ms = 0.f;
+  if (e == cudaSuccess) cudaEventElapsedTime(&ms, t0, t1);
+  ctx->event_pool.push_back(t0); ctx->event_pool.push_back(t1);
+  if (stats) { stats->n_rebuilds = ev.n_rebuilds; stats->n_graph_replays = ev.n_replays; stats->ms_total = ms; }
   if (status != MLIP_OK) return status;
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) { ctx->set_error(std::string("md: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
   return mlip_take_dev_status(ctx);
+}
+
+extern "C" int mlip_md_nve(mlip_ctx* ctx, const mlip_model* M, int L, double* pos_dev, double* vel_dev,
+                           const double* mass_dev, const double* cell_host, const int32_t* species_dev, int64_t N,
+                           const int grid[3], double halo, int precision, double dt, int n_steps,
+                           double* total_energy_host) {
+  mlip_md_params p;
+  memset(&p, 0, sizeof(p));
+  p.dt = dt; p.n_steps = n_steps; p.thermostat = MLIP_MD_NVE;
+  return mlip_md_run(ctx, M, L, pos_dev, vel_dev, mass_dev, cell_host, species_dev, N, grid, halo, precision, &p,
+                     total_energy_host, nullptr);
 }

@@ -23,7 +23,8 @@ __global__ void k_scale(const float* __restrict__ src, float* __restrict__ dst, 
 extern "C" size_t mlip_model_num_weights(const mlip_model_header* h) {
   if (!h) return 0;
   const size_t S = h->n_species, d = h->d, k = h->n_rbf, L = h->L_max;
-  const size_t per_layer = d * (2 * d + k) + d + d * d + d + d * 2 * d + d + d * d + d;
+  size_t per_layer = d * (2 * d + k) + d + d * d + d + d * 2 * d + d + d * d + d;
+  if (h->flags & MLIP_FLAG_THREE_BODY) per_layer += 16 * d + 16 + d * 16;
   return S * d + S + L * per_layer + d * d + d + d + 1;
 }
 
@@ -65,6 +66,10 @@ int mlip_take_dev_status(mlip_ctx* ctx) {
   }
   if (bits == 0) return MLIP_OK;
   cudaMemset(ctx->dev_status, 0, sizeof(int));
+  if (bits & MLIP_DEV_ROW_TOO_LONG) {
+    ctx->set_error("three-body variant: an atom has more than 128 neighbours within r_cut3");
+    return MLIP_ERR_UNSUPPORTED;
+  }
   if (bits & MLIP_DEV_NONFINITE) {
     ctx->set_error("non-finite energy or force: with MLIP_BF16 the edge operands are IEEE half, |pre-activations| and "
                    "|adjoints| must stay below 65504 (use MLIP_FP32 for this model)");
@@ -148,7 +153,16 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   if (!h || !w_host || !out) { ctx->set_error("mlip_model_load: null argument"); return MLIP_ERR_INVALID_ARG; }
   *out = nullptr;
   if (h->magic != MLIP_MAGIC || h->version != 1) { ctx->set_error("bad model header magic/version"); return MLIP_ERR_INVALID_ARG; }
-  if (h->flags != 0) { ctx->set_error("three-body variant not implemented"); return MLIP_ERR_UNSUPPORTED; }
+  if (h->flags & ~MLIP_FLAG_THREE_BODY) { ctx->set_error("unknown model flags"); return MLIP_ERR_UNSUPPORTED; }
+  if (h->flags & MLIP_FLAG_THREE_BODY) {
+    if (h->n_rbf3 != 4 || h->l_max != 3 || !(h->r_cut3 > 0.f) || h->r_cut3 > h->r_cut) {
+      ctx->set_error("three-body variant needs n_rbf3 = 4, l_max = 3 and 0 < r_cut3 <= r_cut");
+      return MLIP_ERR_UNSUPPORTED;
+    }
+  } else if (h->n_rbf3 != 0 || h->l_max != 0 || h->r_cut3 != 0.f) {
+    ctx->set_error("n_rbf3, l_max and r_cut3 must be 0 without MLIP_FLAG_THREE_BODY");
+    return MLIP_ERR_INVALID_ARG;
+  }
   if (!(h->d == 64 || h->d == 128 || h->d == 256) || h->n_rbf < 2 || h->n_rbf > 16 || h->n_species < 1 ||
       h->L_max < 0 || !(h->r_cut > 0.f)) {
     ctx->set_error("unsupported model shape (d in {64,128,256}, 2 <= n_rbf <= 16)");
@@ -172,14 +186,21 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     ptr = (T*)dalloc(sizeof(T) * (size_t)(count));                                     \
     if (!ptr) { ctx->set_error("out of device memory (model)"); return fail(MLIP_ERR_OUT_OF_MEMORY); } \
   } while (0)
-  M_ALLOC(M->blob, float, n);
-  if (cudaMemcpyAsync(M->blob, w_host, n * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) {
-    ctx->set_error("weight upload failed");
-    return fail(MLIP_ERR_CUDA);
-  }
-  const float* p = M->blob;
-  M->T = p; p += (size_t)S * d;
-  M->E0 = p; p += S;
+  // Device copy of the blob with every tensor on a 16-byte boundary: the kernels read weights as float4, and the
+  // offsets inside the caller's blob are arbitrary (E0 has S floats).
+  const size_t n_tensors = 2 + (size_t)L * 11 + 4;
+  M_ALLOC(M->blob, float, n + 4 * n_tensors);
+  size_t src_off = 0, dst_off = 0;
+  bool upload_ok = true;
+  auto take = [&](size_t count) -> const float* {
+    dst_off = (dst_off + 3) & ~(size_t)3;
+    float* dst = M->blob + dst_off;
+    if (cudaMemcpyAsync(dst, w_host + src_off, count * sizeof(float), cudaMemcpyHostToDevice, st) != cudaSuccess) upload_ok = false;
+    src_off += count; dst_off += count;
+    return dst;
+  };
+  M->T = take((size_t)S * d);
+  M->E0 = take(S);
   M->layers.resize(L);
   auto sub = [&](const float* src, int ld, int r0, int c0, int tr, float* dst, int ld_dst, int rows, int cols) {
     k_copy_sub<<<(rows * cols + 255) / 256, 256, 0, st>>>(src, ld, r0, c0, tr, dst, ld_dst, rows, cols);
@@ -191,14 +212,19 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   for (int l = 0; l < L; ++l) {
     LayerWeights& W = M->layers[l];
     memset(&W, 0, sizeof(W));
-    W.W1 = p; p += (size_t)d * (2 * d + k);
-    W.b1 = p; p += d;
-    W.W2 = p; p += (size_t)d * d;
-    W.b2 = p; p += d;
-    W.V1 = p; p += (size_t)d * 2 * d;
-    W.c1 = p; p += d;
-    W.V2 = p; p += (size_t)d * d;
-    W.c2 = p; p += d;
+    W.W1 = take((size_t)d * (2 * d + k));
+    W.b1 = take(d);
+    W.W2 = take((size_t)d * d);
+    W.b2 = take(d);
+    W.V1 = take((size_t)d * 2 * d);
+    W.c1 = take(d);
+    W.V2 = take((size_t)d * d);
+    W.c2 = take(d);
+    if (h->flags & MLIP_FLAG_THREE_BODY) {
+      W.G3 = take((size_t)16 * d);
+      W.g3 = take(16);
+      W.W3 = take((size_t)d * 16);
+    }
     M_ALLOC(W.W1ab, float, 2 * d * d); M_ALLOC(W.W1c, float, d * 16); M_ALLOC(W.W1abT, float, 2 * d * d);
     M_ALLOC(W.W2T, float, d * d); M_ALLOC(W.V2T, float, d * d); M_ALLOC(W.V1aT, float, d * d);
     M_ALLOC(W.V1bT, float, d * d); M_ALLOC(W.b1pad, float, 2 * d);
@@ -230,10 +256,11 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     M_ALLOC(W.W2img, __half, d * d); M_ALLOC(W.W1cimg, __half, d * 16);
     mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg);
   }
-  M->Wo = p; p += (size_t)d * d;
-  M->bo = p; p += d;
-  M->wo = p; p += d;
-  M->bE = p; p += 1;
+  M->Wo = take((size_t)d * d);
+  M->bo = take(d);
+  M->wo = take(d);
+  M->bE = take(1);
+  if (!upload_ok || src_off != n) { ctx->set_error("weight upload failed"); return fail(MLIP_ERR_CUDA); }
   M_ALLOC(M->WoT, float, d * d);
   sub(M->Wo, d, 0, 0, 1, M->WoT, d, d, d);
   M_ALLOC(M->Wo_bf, __nv_bfloat16, d * d); M_ALLOC(M->WoT_bf, __nv_bfloat16, d * d);

@@ -17,7 +17,8 @@ def oracle_model(spec, blob):
 def gpu_setup(spec, blob):
     import paper_2509_21694_b200 as mlip
     ctx = mlip.Context(0)
-    model = mlip.Model(ctx, spec.n_species, spec.d, spec.n_rbf, spec.L_max, spec.r_cut, spec.agg_scale, blob)
+    model = mlip.Model(ctx, spec.n_species, spec.d, spec.n_rbf, spec.L_max, spec.r_cut, spec.agg_scale, blob,
+                       r_cut3=getattr(spec, "r_cut3", 0.0))
     return mlip, ctx, model
 
 

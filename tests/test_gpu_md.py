@@ -1,0 +1,67 @@
+"""-m gpu: the on-device MD driver mlip_md_run against the oracle's integrators on the same
+start: Langevin (BAOAB + Philox4x32-10, reading R20) trajectories, the thermostat's temperature, and -- with a Verlet
+skin -- graph / partition reuse and CUDA-graph replay against the rebuild-every-step run."""
+import numpy as np
+import pytest
+
+from oracle import mlip_oracle as O
+from synth_inputs import ModelSpec, make_weights, small_system
+from tests.gpu_util import gpu_setup, oracle_model
+
+pytestmark = pytest.mark.gpu
+
+
+def _start(n_cells=6, seed=61, T0=0.004):
+    spec = ModelSpec(4, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 35)
+    s = small_system(n_cells, 0.08, seed=seed)
+    rng = np.random.default_rng(7)
+    masses = rng.uniform(10.0, 60.0, len(s.pos))
+    vel0 = rng.normal(0, T0, s.pos.shape); vel0 -= vel0.mean(0)
+    return spec, blob, s, masses, vel0
+
+
+def _gpu_md(spec, blob, s, masses, vel0, dt, n_steps, **kw):
+    import torch
+    mlip, ctx, model = gpu_setup(spec, blob)
+    pos = torch.tensor(s.pos, dtype=torch.float64, device="cuda:0").contiguous()
+    vel = torch.tensor(vel0, dtype=torch.float64, device="cuda:0").contiguous()
+    mass = torch.tensor(masses, dtype=torch.float64, device="cuda:0")
+    species = torch.tensor(s.species, dtype=torch.int32, device="cuda:0")
+    e, stats = mlip.md_run(ctx, model, 2, pos, vel, mass, s.cell, species, dt, n_steps, **kw)
+    return e, pos.cpu().numpy(), vel.cpu().numpy(), stats
+
+
+@pytest.mark.parametrize("grid,halo", [((1, 1, 1), 0.0), ((2, 1, 1), 6.0)])
+def test_langevin_matches_oracle_trajectory(grid, halo):
+    import paper_2509_21694_b200 as mlip
+    spec, blob, s, masses, vel0 = _start()
+    n_steps, dt, T, fr, seed = 20, 2.0, 600.0, 0.01, 20260101
+    e_ref, pos_ref, vel_ref = O.langevin_baoab(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses, vel0, dt, n_steps,
+                                               temperature=T, friction=fr, seed=seed)
+    e, pos, vel, stats = _gpu_md(spec, blob, s, masses, vel0, dt, n_steps, grid=grid, halo=halo,
+                                 thermostat=mlip.MLIP_MD_LANGEVIN, temperature=T, friction=fr, seed=seed)
+    kin0 = 0.5 * np.sum(masses[:, None] * vel0 ** 2) / O.ACC_UNIT
+    assert np.abs(e - e_ref).max() <= 1e-4 * kin0
+    assert np.abs(pos - pos_ref).max() <= 1e-5
+    assert np.abs(vel - vel_ref).max() <= 1e-5 * np.abs(vel_ref).max() + 1e-8
+    # the thermostat acted: the trajectory differs from the NVE one by far more than the tolerance
+    _, pos_nve, _ = O.nve_velocity_verlet(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses, vel0, dt, n_steps,
+                                          return_state=True)
+    assert np.abs(pos_ref - pos_nve).max() > 1e-3
+    assert stats["n_rebuilds"] == n_steps + 1
+
+
+def test_langevin_zero_friction_is_nve_and_thermostat_sets_temperature():
+    import paper_2509_21694_b200 as mlip
+    spec, blob, s, masses, vel0 = _start()
+    e_nve, p_nve, v_nve, _ = _gpu_md(spec, blob, s, masses, vel0, 2.0, 10)
+    e_l0, p_l0, v_l0, _ = _gpu_md(spec, blob, s, masses, vel0, 2.0, 10, thermostat=mlip.MLIP_MD_LANGEVIN, temperature=300.0,
+                                  friction=0.0, seed=5)
+    assert np.array_equal(p_nve, p_l0) and np.array_equal(v_nve, v_l0)
+    # strong coupling from a cold start: after 150 steps the kinetic temperature is the bath's (864 atoms: +-4 % 1 sigma)
+    T = 900.0
+    e, pos, vel, _ = _gpu_md(spec, blob, s, masses, np.zeros_like(vel0), 2.0, 150, thermostat=mlip.MLIP_MD_LANGEVIN,
+                             temperature=T, friction=0.05, seed=99)
+    T_kin = np.sum(masses[:, None] * vel ** 2) / O.ACC_UNIT / (3 * len(masses) * O.KB_EV)
+    assert abs(T_kin / T - 1.0) < 0.15, T_kin

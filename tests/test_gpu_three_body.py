@@ -1,0 +1,129 @@
+"""-m gpu: the three-body (angle) variant of BASELINE.json config 5 (oracle O7) through the C ABI
+against the float64 oracle: fp32 tolerances of north_star (per-atom energy 1e-5, max force error 1e-4 RMS F), partitioned
+== unpartitioned, stress, the two-body limit W3 = 0, and config 5 itself (98,304 atoms, 4 slabs, halo 20 A) on sampled
+atoms plus the properties that hold at any size."""
+import numpy as np
+import pytest
+
+from oracle import mlip_oracle as O
+from synth_inputs import ModelSpec, System, make_config, make_water_system, make_weights, small_system
+from tests.gpu_util import errors, gpu_energy_forces, gpu_graph, gpu_setup, oracle_model, rms
+
+pytestmark = pytest.mark.gpu
+FP32_EPS_E, FP32_MAX_F, FP32_REL_EI = 1e-5, 1e-4, 1e-5
+
+
+def _run(spec, blob, system, L, grid=None, halo=0.0, stress=False):
+    import torch
+    mlip, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlip, ctx, system, spec.r_cut)
+    part = mlip.Partition(ctx, g, halo, grid=grid) if grid is not None else None
+    if stress:
+        E, F, Ei, S = mlip.energy_forces_stress(ctx, model, L, g, part, 0)
+        ctx.status()
+        return float(E.item()), F.cpu().numpy().astype(np.float64), Ei.cpu().numpy().astype(np.float64), S.cpu().numpy()
+    return gpu_energy_forces(mlip, ctx, model, L, g, part, 0)
+
+
+@pytest.mark.parametrize("d,L,n_grid", [(64, 2, 4), (128, 4, 5), (128, 1, 3), (256, 2, 4)])
+def test_three_body_fp32_parity_water(d, L, n_grid):
+    spec = ModelSpec(2, d, 16 if d > 64 else 8, L, 5.0, 1.0 / np.sqrt(53.0), r_cut3=4.0)
+    blob = make_weights(spec, 500 + d)
+    s = make_water_system(n_grid, seed_pos=1100 + d, seed_orient=3100 + d)
+    ref = O.energy_forces(oracle_model(spec, blob), L, s.pos, s.cell, s.species)
+    E, F, Ei = _run(spec, blob, s, L)
+    err = errors(E, F, Ei, ref[0], ref[2], ref[1])
+    print(d, L, err)
+    assert err["eps_E"] <= FP32_EPS_E and err["rel_Ei"] <= FP32_REL_EI and err["max_F"] <= FP32_MAX_F
+
+
+def test_three_body_W3_zero_equals_two_body_gpu():
+    """With W3 = 0 the variant must give the two-body GPU result bit for bit (the angle term is added as W3 t_e)."""
+    spec3 = ModelSpec(2, 64, 8, 2, 5.0, 1.0 / np.sqrt(53.0), r_cut3=4.0)
+    blob3 = make_weights(spec3, 510).copy()
+    d, k, S = 64, 8, 2
+    two = d * (2 * d + k) + d + d * d + d + 2 * d * d + d + d * d + d
+    extra = 16 * d + 16 + 16 * d
+    head = S * d + S
+    parts = [blob3[:head]]
+    for l in range(2):
+        o = head + l * (two + extra)
+        blob3[o + two + 16 * d + 16: o + two + extra] = 0.0          # W3 of layer l
+        parts.append(blob3[o:o + two])
+    parts.append(blob3[head + 2 * (two + extra):])
+    spec2 = ModelSpec(2, 64, 8, 2, 5.0, spec3.agg_scale)
+    s = make_water_system(4)
+    a = _run(spec3, blob3, s, 2)
+    b = _run(spec2, np.concatenate(parts), s, 2)
+    assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+
+
+def test_three_body_partitioned_stress_and_reproducible():
+    spec = ModelSpec(2, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0), r_cut3=2.6)
+    blob = make_weights(spec, 520)
+    s = small_system(8, 0.08, seed=71, n_species=2)     # 28.8 A fcc box, first shell inside r3
+    E_ref, Ei_ref, F_ref, sig_ref = O.energy_forces_stress(oracle_model(spec, blob), 2, s.pos, s.cell, s.species)
+    E0, F0, Ei0, S0 = _run(spec, blob, s, 2, stress=True)
+    err = errors(E0, F0, Ei0, E_ref, F_ref, Ei_ref)
+    assert err["eps_E"] <= FP32_EPS_E and err["rel_Ei"] <= FP32_REL_EI and err["max_F"] <= FP32_MAX_F
+    assert np.abs(S0 - sig_ref).max() <= 1e-4 * np.abs(sig_ref).max()
+    again = _run(spec, blob, s, 2, stress=True)
+    assert again[0] == E0 and np.array_equal(again[1], F0) and np.array_equal(again[3], S0)   # no atomics: bitwise
+    for grid in [(2, 1, 1), (3, 1, 1), (2, 2, 1)]:
+        E, F, Ei, S = _run(spec, blob, s, 2, grid=grid, halo=6.0, stress=True)
+        assert np.abs(F - F0).max() <= 1e-5 * rms(F0) and abs(E - E0) <= 1e-5 * np.abs(Ei_ref).sum()
+        assert np.abs(S - S0).max() <= 1e-5 * np.abs(sig_ref).max()
+        err = errors(E, F, Ei, E_ref, F_ref, Ei_ref)
+        assert err["eps_E"] <= FP32_EPS_E and err["rel_Ei"] <= FP32_REL_EI and err["max_F"] <= FP32_MAX_F
+
+
+def test_three_body_rejects_bf16_and_bad_header():
+    import paper_2509_21694_b200 as mlip
+    spec = ModelSpec(2, 128, 16, 1, 5.0, 1.0 / np.sqrt(53.0), r_cut3=4.0)
+    blob = make_weights(spec, 530)
+    s = make_water_system(3)
+    mlipm, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlipm, ctx, s, spec.r_cut)
+    with pytest.raises(mlip.MlipError) as ei:
+        mlip.energy_forces(ctx, model, 1, g, None, mlip.MLIP_BF16)
+    assert ei.value.code == -2
+    with pytest.raises(mlip.MlipError) as ei:   # r_cut3 > r_cut would need a wider halo than L r_cut
+        mlip.Model(ctx, 2, 128, 16, 1, 5.0, spec.agg_scale, blob, r_cut3=5.5)
+    assert ei.value.code == -2
+
+
+def _ball(system, i, radius):
+    box = np.diag(system.cell)
+    dvec = system.pos - system.pos[i]
+    dvec -= np.round(dvec / box) * box
+    r = np.linalg.norm(dvec, axis=1)
+    keep = np.nonzero(r <= radius)[0]
+    side = 2.0 * radius + 20.0
+    return dvec[keep] + 0.5 * side, np.eye(3) * side, system.species[keep], int(np.nonzero(keep == i)[0][0]), r[keep]
+
+
+def test_config5_full_size_partitioned():
+    """BASELINE.json config 5 in the configuration bench.py --config 5 times: 98,304 atoms, L = 4, d = 128, fp32, 4 slabs
+    with a 20 A halo. Sampled E_i (oracle on the L r_c ball around an O atom on a slab face and an H atom mid-slab),
+    partitioned == unpartitioned, total force zero."""
+    cfg = make_config(5)
+    s, m = cfg.system, cfg.model
+    mlip, ctx, model = gpu_setup(m, cfg.weights)
+    g = gpu_graph(mlip, ctx, s, m.r_cut)
+    part = mlip.Partition(ctx, g, cfg.halo, grid=cfg.grid)
+    info = part.info()
+    assert len(info) == 4 and sum(i["n_owned"] for i in info) == 98304
+    E, F, Ei = gpu_energy_forces(mlip, ctx, model, cfg.L, g, part, 0)
+    E1, F1, Ei1 = gpu_energy_forces(mlip, ctx, model, cfg.L, g, None, 0)
+    assert np.isfinite(F).all()
+    assert np.abs(F - F1).max() <= 1e-5 * rms(F1) and abs(E - E1) <= 1e-5 * np.abs(Ei1).sum()
+    assert np.abs(F.sum(0)).max() <= 1e-3 * rms(F)
+    om = oracle_model(m, cfg.weights)
+    box = s.cell[0, 0]
+    x = s.pos[:, 0] % box
+    on_face = int(np.argmin(np.abs(x[:32768] - box / 4)))                        # an O atom on the slab 0 | slab 1 face
+    mid = 32768 + int(np.argmin(np.abs(x[32768:] - 0.625 * box)))                # an H atom in the middle of slab 2
+    for i in (on_face, mid):
+        pos, cell, sp, k, r = _ball(s, i, cfg.L * m.r_cut + 0.5)
+        E_ref = O.energy_forces(om, cfg.L, pos, cell, sp)[1][k]
+        assert abs(Ei[i] - E_ref) <= 1e-5 * max(abs(E_ref), rms(Ei)), (i, Ei[i], E_ref)
