@@ -172,6 +172,9 @@ struct SubGraph {
   // way an atom of class k only has neighbours of class >= k-1, so the root energies (and their gradient) need layer l
   // only on receivers of class <= L-1-l with senders of class <= L-l (each root atom keeps its K-hop
   // neighbourhood). Both sets are prefixes of the numbering.
+  // Verlet-skin mode (md.cu / skin.cu): the edge arrays are re-filtered on the device every step; E and E_le are then
+  // CAPACITIES (the candidate counts) and the actual numbers are rowptr[n] / rowptr[n_le[c]] on the device.
+  bool dyn = false;
   int n_cls = 0;
   int64_t n_le[MLIP_MAX_CLS] = {};   // atoms of class <= c
   int64_t E_le[MLIP_MAX_CLS] = {};   // edges whose receiver has class <= c  (= rowptr[n_le[c]])
@@ -209,6 +212,7 @@ struct PartSub {
           *rev = nullptr;
   float* omega = nullptr;
   float4* rvec = nullptr;
+  int32_t* geid = nullptr;   // [E] edge id in the parent graph (kept on request: mlip_partition_grid_ex)
 };
 
 struct mlip_part {
@@ -219,6 +223,9 @@ struct mlip_part {
   int64_t N = 0;
   std::vector<PartSub> subs;
 };
+
+int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo_box, double halo,
+                           double r_class, bool force_khop, bool keep_geid, mlip_part** out);
 
 // ---- launchers (each bumps ctx->launches by the number of kernels it enqueues) ---------------
 // scan.cu

@@ -5,6 +5,10 @@
 
 struct EdgeArgs {
   int64_t E = 0, n = 0;
+  // Verlet-skin mode of the MD driver: the edge list is re-filtered on the device every step, so its length is only known
+  // there. When given, the number of edges is *E_dyn (= rowptr[number of receivers of this launch]) and E above is the
+  // CAPACITY the launch dimensions are derived from (fixed between rebuilds, which is what lets a CUDA graph replay them).
+  const int32_t* E_dyn = nullptr;
   const int32_t* rowptr = nullptr;
   const int32_t* recv = nullptr;
   const int32_t* send = nullptr;
@@ -48,18 +52,18 @@ int mlip_triplet_forward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t*
                          const float4* rvec, const float* z, float* t);
 int mlip_triplet_backward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
                           const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta);
-int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                       const float* zeta, const float* z, const float* G, float* hbar);
+int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                       const int32_t* rev, const float* zeta, const float* z, const float* G, float* hbar);
 
 int64_t mlip_edge_f32_tiles(int64_t E);
 int mlip_edge_forward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
 // Qbar_j = sum over in-edges e of j, j < n, with rev[e] < E_act, of abar[rev[e]]
-int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                        const float* abar, float* Qbar);
+int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                        const int32_t* rev, const float* abar, float* Qbar);
 
 int64_t mlip_edge_tc_tiles(int64_t E);
 int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
-int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                       const __half* abar, __nv_bfloat16* Qbar /*[n,d] bf16*/);
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                       const int32_t* rev, const __half* abar, __nv_bfloat16* Qbar /*[n,d] bf16*/);

@@ -132,13 +132,15 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
   const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
   const int64_t tile = blockIdx.x;
   const int64_t e0 = tile * TE;
+  const int64_t n_edges = a.E_dyn ? (int64_t)__ldg(a.E_dyn) : a.E;   // Verlet-skin mode: a.E is only the capacity
+  if (e0 >= n_edges) return;
 
   // ---- tile metadata and edge features (A6) ----
   if (tid < TE) {
     const int64_t e = e0 + tid;
     int rc = -1, sd = 0;
     float r = 0.f, u = 0.f, du = 0.f;
-    if (e < a.E) {
+    if (e < n_edges) {
       rc = a.recv[e]; sd = a.send[e]; r = a.rvec[e].w;
       envelope_f(r, a.r_cut, u, du);
     }
@@ -146,7 +148,7 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
       float g = 0.f, dg;
-      if (e < a.E && k < a.n_rbf) rbf_f(r, a.r_cut, a.n_rbf, k, g, dg);
+      if (e < n_edges && k < a.n_rbf) rbf_f(r, a.r_cut, a.n_rbf, k, g, dg);
       ehat[tid * 16 + k] = u * g;
     }
   }
@@ -154,7 +156,7 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
     for (int idx = tid; idx < TE * 4; idx += 256) {
       const int64_t e = e0 + (idx >> 2);
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (e < a.E) v = *reinterpret_cast<const float4*>(a.t3 + (size_t)e * 16 + (idx & 3) * 4);
+      if (e < n_edges) v = *reinterpret_cast<const float4*>(a.t3 + (size_t)e * 16 + (idx & 3) * 4);
       *reinterpret_cast<float4*>(t3_s + idx * 4) = v;
     }
   }
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
       float4 ds = *reinterpret_cast<const float4*>(dS + row * LDS + c);
       ds.x *= acc[i][4 * j + 0]; ds.y *= acc[i][4 * j + 1]; ds.z *= acc[i][4 * j + 2]; ds.w *= acc[i][4 * j + 3];
       *reinterpret_cast<float4*>(dS + row * LDS + c) = ds;
-      if (e < a.E) *reinterpret_cast<float4*>(a.abar + (size_t)e * D + c) = ds;
+      if (e < n_edges) *reinterpret_cast<float4*>(a.abar + (size_t)e * D + c) = ds;
     }
   }
   __syncthreads();
@@ -287,7 +289,7 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
         const float4 w = *reinterpret_cast<const float4*>(a.W3 + (size_t)c * 16 + kq * 4);
         tb.x = fmaf(av, w.x, tb.x); tb.y = fmaf(av, w.y, tb.y); tb.z = fmaf(av, w.z, tb.z); tb.w = fmaf(av, w.w, tb.w);
       }
-      if (e0 + e < a.E) *reinterpret_cast<float4*>(a.tbar + (size_t)(e0 + e) * 16 + kq * 4) = tb;
+      if (e0 + e < n_edges) *reinterpret_cast<float4*>(a.tbar + (size_t)(e0 + e) * 16 + kq * 4) = tb;
     }
     float part = 0.f;
     const float r = r_s[e], u = u_s[e], du = du_s[e];
@@ -302,15 +304,17 @@ __global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
     }
     part += __shfl_xor_sync(0xffffffffu, part, 1);
     part += __shfl_xor_sync(0xffffffffu, part, 2);
-    if (kq == 0 && e0 + e < a.E) a.rbar[e0 + e] += fmaf(ubar_s[e], du, part);
+    if (kq == 0 && e0 + e < n_edges) a.rbar[e0 + e] += fmaf(ubar_s[e], du, part);
   }
   segmented_store<D>(dS, recv_s, a.rowptr, e0, tile, a.Pbar, a.head, a.tail, tid);
 }
 
 // out[i] = tail[t] + head[t+1] + ... for the segment that starts in tile t and continues beyond it
 template <int TILE>
-__global__ void k_segment_fixup(int64_t E, int D, const int32_t* __restrict__ rowptr, const int32_t* __restrict__ recv,
-                                const float* __restrict__ head, const float* __restrict__ tail, float* __restrict__ out) {
+__global__ void k_segment_fixup(int64_t E, const int32_t* __restrict__ E_dyn, int D, const int32_t* __restrict__ rowptr,
+                                const int32_t* __restrict__ recv, const float* __restrict__ head,
+                                const float* __restrict__ tail, float* __restrict__ out) {
+  if (E_dyn) E = *E_dyn;
   const int64_t t = blockIdx.x;
   const int64_t e0 = t * TILE, e1 = e0 + TILE;
   if (e1 >= E) return;  // last tile cannot have a continuing segment
@@ -325,9 +329,11 @@ __global__ void k_segment_fixup(int64_t E, int D, const int32_t* __restrict__ ro
 }
 
 // Qbar_j = sum_{e in in(j)} abar[rev[e]]  (sender-side adjoint gathered through the reverse index)
-__global__ void __launch_bounds__(256) k_gather_rev_f32(int64_t n, int64_t E_act, int D, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_gather_rev_f32(int64_t n, int64_t E_act, const int32_t* __restrict__ E_act_dyn, int D,
+                                                        const int32_t* __restrict__ rowptr,
                                                         const int32_t* __restrict__ rev, const float* __restrict__ abar,
                                                         float* __restrict__ Qbar) {
+  if (E_act_dyn) E_act = *E_act_dyn;
   const int lane = threadIdx.x & 31;
   const int64_t j = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (j >= n) return;
@@ -359,8 +365,8 @@ int launch_edge(mlip_ctx* ctx, const EdgeArgs& a, bool bwd) {
     MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_f32<D, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_edge_f32<D, false><<<(unsigned)tiles, 256, smem, ctx->stream>>>(a);
   }
-  k_segment_fixup<TE><<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, D, a.rowptr, a.recv, a.head, a.tail,
-                                                                           bwd ? a.Pbar : a.m);
+  k_segment_fixup<TE><<<(unsigned)tiles, D < 256 ? D : 256, 0, ctx->stream>>>(a.E, a.E_dyn, D, a.rowptr, a.recv, a.head,
+                                                                           a.tail, bwd ? a.Pbar : a.m);
   ctx->launches += 2;
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
   return MLIP_OK;
@@ -385,10 +391,10 @@ int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   }
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                        const float* abar, float* Qbar) {
+int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                        const int32_t* rev, const float* abar, float* Qbar) {
   if (n <= 0) return MLIP_OK;
-  k_gather_rev_f32<<<(unsigned)((n * 32 + 255) / 256), 256, 0, ctx->stream>>>(n, E_act, d, rowptr, rev, abar, Qbar);
+  k_gather_rev_f32<<<(unsigned)((n * 32 + 255) / 256), 256, 0, ctx->stream>>>(n, E_act, E_act_dyn, d, rowptr, rev, abar, Qbar);
   ctx->launches++;
   return MLIP_OK;
 }

@@ -199,8 +199,11 @@ __device__ __forceinline__ void segmented_store_tc(const unsigned char* __restri
 }
 
 template <int D, bool BWD>
-__global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_tiles) {
+__global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_tiles_cap) {
   extern __shared__ unsigned char smem_raw[];
+  // number of edges: by value, or read from the device in Verlet-skin mode (EdgeArgs::E_dyn; a.E is then the capacity)
+  const int64_t n_edges = a.E_dyn ? (int64_t)__ldg(a.E_dyn) : a.E;
+  const int64_t n_tiles = a.E_dyn ? (n_edges + TE - 1) / TE : n_tiles_cap;
   using SM = ES<D, BWD>;
   using Meta = TileMeta<BWD>;
   constexpr int NCH = SM::NCH;
@@ -249,7 +252,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
   const uint32_t tmem = *slot;
   const uint32_t TX = tmem, TY = tmem + D;  // accumulator regions: X = D1 / D3, Y = D2 / (segment sums, D4)
 
-  if (warp >= WARP_FEAT) {
+  if (blockIdx.x >= n_tiles) {
+    // no tile for this CTA (only possible with E_dyn: the grid is sized from the capacity)
+  } else if (warp >= WARP_FEAT) {
     // ============ feature producers: tile metadata (two tiles ahead) and the e_hat operand ============
     const float delta = a.r_cut / (float)(a.n_rbf - 1);
     const float inv_delta = 1.0f / delta;
@@ -267,7 +272,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       for (int k = 0; k < EPL; ++k) {
         const int64_t ge = e0 + ebase + 32 * k;
         rc[k] = -1; sd[k] = 0; rr[k] = 0.f;
-        if (ge < a.E) { rc[k] = a.recv[ge]; sd[k] = a.send[ge]; rr[k] = a.rvec[ge].w; }
+        if (ge < n_edges) { rc[k] = a.recv[ge]; sd[k] = a.send[ge]; rr[k] = a.rvec[ge].w; }
       }
       if (a.row_index) {  // M.send carries the ROW of the Q table: the sender itself, or its species in the first layer
 #pragma unroll
@@ -324,7 +329,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         const int64_t ge = e0 + e;
         bool flag = false;
         rc[k] = -1;
-        if (ge < a.E) {
+        if (ge < n_edges) {
           rc[k] = a.recv[ge];
           flag = e == 0 || a.recv[ge - 1] != rc[k];
         }
@@ -831,9 +836,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
 
 // out[i] = tail[t] + head[t+1] + ... for the segment that starts in tile t and continues beyond it.
 // D/4 threads per tile (one float4 of channels each), 1024/D tiles per 256-thread block.
-__global__ void __launch_bounds__(256) k_segment_fixup_tc(int64_t E, int D, int64_t n_tiles, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_segment_fixup_tc(int64_t E, const int32_t* __restrict__ E_dyn, int D, int64_t n_tiles,
+                                                          const int32_t* __restrict__ rowptr,
                                                           const int32_t* __restrict__ recv, const float* __restrict__ head,
                                                           const float* __restrict__ tail, float* __restrict__ out) {
+  if (E_dyn) { E = *E_dyn; n_tiles = (E + TE - 1) / TE; }
   const int tpt = D >> 2;  // threads per tile
   const int64_t t = (int64_t)blockIdx.x * (blockDim.x / tpt) + threadIdx.x / tpt;
   const int c = (threadIdx.x % tpt) * 4;
@@ -853,9 +860,11 @@ __global__ void __launch_bounds__(256) k_segment_fixup_tc(int64_t E, int D, int6
 
 // Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled f16 tile images written by E3
 template <int D>
-__global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act, const int32_t* __restrict__ E_act_dyn,
+                                                       const int32_t* __restrict__ rowptr,
                                                        const int32_t* __restrict__ rev, const __half* __restrict__ abar,
                                                        __nv_bfloat16* __restrict__ Qbar) {
+  if (E_act_dyn) E_act = *E_act_dyn;
   constexpr int CH = D / 8;        // 16-byte chunks per row
   constexpr int NSUB = 32 / CH;    // edges handled concurrently by one warp
   const int lane = threadIdx.x & 31;
@@ -900,7 +909,7 @@ int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   if (!BWD || a.node_adjoint) {
     const int64_t tiles_per_block = 256 / (D / 4);
     k_segment_fixup_tc<<<(unsigned)((tiles + tiles_per_block - 1) / tiles_per_block), 256, 0, ctx->stream>>>(
-        a.E, D, tiles, a.rowptr, a.recv, a.head, a.tail, BWD ? a.Pbar : a.m);
+        a.E, a.E_dyn, D, tiles, a.rowptr, a.recv, a.head, a.tail, BWD ? a.Pbar : a.m);
     ctx->launches++;
   }
   MLIP_CUDA_CHECK(ctx, cudaGetLastError());
@@ -922,12 +931,12 @@ int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   ctx->set_error("tensor-core edge kernels need d = 128 or 256");
   return MLIP_ERR_UNSUPPORTED;
 }
-int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                       const __half* abar, __nv_bfloat16* Qbar) {
+int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                       const int32_t* rev, const __half* abar, __nv_bfloat16* Qbar) {
   if (n <= 0) return MLIP_OK;
   const unsigned grid = (unsigned)((n * 32 + 255) / 256);
-  if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, E_act, rowptr, rev, abar, Qbar);
-  else if (d == 128) k_gather_rev_tc<128><<<grid, 256, 0, ctx->stream>>>(n, E_act, rowptr, rev, abar, Qbar);
+  if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, E_act, E_act_dyn, rowptr, rev, abar, Qbar);
+  else if (d == 128) k_gather_rev_tc<128><<<grid, 256, 0, ctx->stream>>>(n, E_act, E_act_dyn, rowptr, rev, abar, Qbar);
   else { ctx->set_error("tensor-core gather needs d = 128 or 256"); return MLIP_ERR_UNSUPPORTED; }
   ctx->launches++;
   return MLIP_OK;

@@ -171,12 +171,13 @@ __global__ void __launch_bounds__(256) k_forces(int64_t n, const int32_t* __rest
 
 // Virial of one sub-domain: W_ab += sum_e rbar_e r_a r_b / r over its directed edges (rbar is zero on the
 // edges no layer evaluated). float64 per-block partials in a fixed order, then one block: deterministic, no atomics.
-__global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const float4* __restrict__ rvec,
+__global__ void __launch_bounds__(256) k_virial_partial(int64_t E, const int32_t* __restrict__ E_dyn, const float4* __restrict__ rvec,
                                                         const float* __restrict__ rbar, const float* __restrict__ scale,
                                                         const float4* __restrict__ gvec, double* __restrict__ partial) {
   __shared__ double sh[6][256];
   double w[6] = {0, 0, 0, 0, 0, 0};
   const double inv_s = scale ? (double)scale[1] : 1.0;
+  if (E_dyn) E = *E_dyn;
   for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < E; e += (int64_t)gridDim.x * blockDim.x) {
     const float4 rv = rvec[e];
     if (rv.w > 0.f) {
@@ -364,7 +365,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
       cudaMemsetAsync(m, 0, sizeof(float) * nr * d, st);
     }
     set_layer(l);
-    ea.m = m; ea.E = e_recv(l); ea.n = nr;
+    ea.m = m; ea.E = e_recv(l); ea.n = nr; ea.E_dyn = g.dyn ? g.rowptr + nr : nullptr;
     if (tb) {
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
       W_TRY(mlip_gate_forward(ctx, ns, d, h[l], W.G3, W.g3, zg[l]));
@@ -447,6 +448,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     }
     set_layer(l);
     ea.E = Er; ea.n = nr; ea.node_adjoint = bf ? node_adjoint : true;
+    ea.E_dyn = g.dyn ? g.rowptr + nr : nullptr;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
     if (tb) {  // the angle terms are recomputed like every other edge activation
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
@@ -466,8 +468,8 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     {
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
       // Qbar_j over the senders of this layer, summing only the reverse edges that were evaluated (rev[e] < Er)
-      W_TRY(bf ? mlip_gather_rev_tc(ctx, ns, Er, d, g.rowptr, g.rev, abar_h, Qbar_b)
-               : mlip_gather_rev_f32(ctx, ns, Er, d, g.rowptr, g.rev, abar, Qbar));
+      W_TRY(bf ? mlip_gather_rev_tc(ctx, ns, Er, ea.E_dyn, d, g.rowptr, g.rev, abar_h, Qbar_b)
+               : mlip_gather_rev_f32(ctx, ns, Er, ea.E_dyn, d, g.rowptr, g.rev, abar, Qbar));
     }
     a = GemmArgs(); a.X1 = Pbar; a.ld1 = d; a.K1 = d; a.ld2 = d; a.K2 = d;
     if (bf) a.X2b = Qbar_b; else a.X2 = Qbar;
@@ -476,7 +478,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     W_TRY(gemm(ctx, a));
     if (tb) {  // adjoint of the gates of the senders (third atoms), through the reverse-edge index like Qbar
       ProfScope p(ctx, MLIP_PROF_GATHER_REV);
-      W_TRY(mlip_gate_backward(ctx, ns, Er, d, g.rowptr, g.rev, zeta, zg[l], W.G3, hbar));
+      W_TRY(mlip_gate_backward(ctx, ns, Er, ea.E_dyn, d, g.rowptr, g.rev, zeta, zg[l], W.G3, hbar));
     }
   }
   {
@@ -487,7 +489,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
       const int nb = (int)(E < 148 * 8 * 256 ? (E + 255) / 256 : 148 * 8);
       double* vpart = nullptr;
       W_ALLOC(vpart, double, (size_t)nb * 6);
-      k_virial_partial<<<nb, 256, 0, st>>>(E, g.rvec, rbar, rscale, gvec, vpart);
+      k_virial_partial<<<nb, 256, 0, st>>>(E, g.dyn ? g.rowptr + n : nullptr, g.rvec, rbar, rscale, gvec, vpart);
       k_virial_final<<<1, 32, 0, st>>>(nb, vpart, virial_accum);
       ctx->launches += 2;
     }

@@ -6,6 +6,7 @@
 // float32 output of mlip_energy_forces. Units: Angstrom, fs, amu, eV (1 eV/A/amu = 9.648533e-3 A/fs^2).
 #include <string.h>
 #include "common.cuh"
+#include "skin.cuh"
 
 namespace {
 constexpr double ACC_UNIT = 9.648533e-3;  // (eV/A)/amu -> A/fs^2
@@ -88,19 +89,48 @@ __global__ void k_total_energy(int n_partial, const double* __restrict__ partial
   out[0] = e_pot[0] + 0.5 * s / ACC_UNIT;
 }
 
-// Graph -> partition -> E, F at the current positions. skin = 0: everything is rebuilt on every call.
+// Graph -> partition -> E, F at the current positions. skin = 0: everything is rebuilt on every call. skin > 0: the candidate
+// graph (r_c + skin) and its partition are kept until an atom has moved more than skin/2 (skin.cu); the per-step work --
+// filter, layers, reverse pass, force assembly -- has fixed launch dimensions between rebuilds and can be replayed from a
+// CUDA graph.
+__global__ void k_md_check_finite(int64_t n, const float* __restrict__ F, const double* __restrict__ energy, int* __restrict__ status) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  bool bad = i < n && !isfinite(F[i]);
+  if (i == 0) bad = bad || !isfinite(energy[0]);
+  if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(status, MLIP_DEV_NONFINITE);
+}
+
 struct MdEvaluator {
   mlip_ctx* ctx; const mlip_model* M; int L; const double* pos; const double* cell; const int32_t* species; int64_t N;
   int grid[3]; double halo; int precision; double skin; bool use_graph; double* e_pot; float* F;
   int64_t n_rebuilds = 0, n_replays = 0;
+  // skin mode
+  mlip_graph* Gc = nullptr;
+  mlip_part* Pc = nullptr;
+  std::vector<SkinSub> subs;
+  double* pos0 = nullptr;
+  int* flag = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  bool capture_failed = false;
+  std::string capture_error;
   MdEvaluator(mlip_ctx* c, const mlip_model* m, int L_, const double* p, const double* cell_, const int32_t* sp, int64_t n,
               const int g[3], double h, int prec, double skin_, bool graph, double* e, float* f)
       : ctx(c), M(m), L(L_), pos(p), cell(cell_), species(sp), N(n), halo(h), precision(prec), skin(skin_), use_graph(graph),
         e_pot(e), F(f) {
     grid[0] = g[0]; grid[1] = g[1]; grid[2] = g[2];
   }
+  ~MdEvaluator() { drop(); ctx->free(pos0); ctx->free(flag); }
   bool split() const { return grid[0] > 1 || grid[1] > 1 || grid[2] > 1; }
-  int evaluate() {
+  void drop() {
+    if (exec) { cudaGraphExecDestroy(exec); exec = nullptr; }
+    for (auto& k : subs) k.release(ctx);
+    subs.clear();
+    mlip_part_destroy(Pc); Pc = nullptr;
+    mlip_graph_destroy(Gc); Gc = nullptr;
+  }
+  int evaluate() { return skin > 0.0 ? evaluate_skin() : evaluate_rebuild(); }
+
+  int evaluate_rebuild() {
     mlip_graph* G = nullptr;
     mlip_part* P = nullptr;
     int s = mlip_build_graph(ctx, pos, cell, species, N, (double)M->h.r_cut, &G);
@@ -110,6 +140,98 @@ struct MdEvaluator {
     mlip_graph_destroy(G);
     ++n_rebuilds;
     return s;
+  }
+
+  int rebuild() {
+    drop();
+    const double r_c = (double)M->h.r_cut;
+    MLIP_TRY(mlip_build_graph(ctx, pos, cell, species, N, r_c + skin, &Gc));
+    if (N > 0 && (Gc->species_min < 0 || Gc->species_max >= M->h.n_species)) {
+      ctx->set_error("species outside [0, n_species) of the model");
+      return MLIP_ERR_INVALID_ARG;
+    }
+    if (split()) {
+      if (halo < (double)L * r_c * (1.0 - 1e-12)) {
+        ctx->set_error("halo < L * r_cut: sub-graphs would not keep the K-hop neighbourhood of their root atoms");
+        return MLIP_ERR_HALO_TOO_SMALL;
+      }
+      MLIP_TRY(mlip_partition_grid_ex(ctx, Gc, grid, halo + skin, halo, r_c, true, true, &Pc));
+      subs.resize(Pc->subs.size());
+      for (size_t k = 0; k < subs.size(); ++k) MLIP_TRY(mlip_skin_sub_create(ctx, Gc, &Pc->subs[k], &subs[k]));
+    } else {
+      subs.resize(1);
+      MLIP_TRY(mlip_skin_sub_create(ctx, Gc, nullptr, &subs[0]));
+    }
+    if (!pos0) MLIP_TRY(ctx->alloc(&pos0, 3 * N));
+    cudaMemcpyAsync(pos0, pos, sizeof(double) * 3 * N, cudaMemcpyDeviceToDevice, ctx->stream);
+    ++n_rebuilds;
+    return MLIP_OK;
+  }
+
+  // filter + evaluate every sub-domain at the current positions (fixed launch dimensions)
+  int step_eager() {
+    cudaStream_t st = ctx->stream;
+    cudaMemsetAsync(F, 0, sizeof(float) * 3 * N, st);
+    cudaMemsetAsync(e_pot, 0, sizeof(double), st);
+    for (auto& k : subs) {
+      MLIP_TRY(mlip_skin_filter(ctx, k, pos, cell, (double)M->h.r_cut));
+      MLIP_TRY(mlip_eval_subgraph(ctx, M, L, k.g, precision, e_pot, F, nullptr, nullptr));
+    }
+    if (N > 0) {
+      k_md_check_finite<<<nblk(3 * N, 256), 256, 0, st>>>(3 * N, F, e_pot, ctx->dev_status);
+      ctx->launches++;
+    }
+    return MLIP_OK;
+  }
+
+  int evaluate_skin() {
+    cudaStream_t st = ctx->stream;
+    bool need = Gc == nullptr;
+    if (!need) {
+      if (!flag) MLIP_TRY(ctx->alloc(&flag, 1));
+      MLIP_TRY(mlip_skin_moved(ctx, N, pos, pos0, skin, flag));
+      int h = 0;
+      MLIP_CUDA_CHECK(ctx, cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+      MLIP_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+      need = h != 0;
+    }
+    if (need) MLIP_TRY(rebuild());
+    if (use_graph && !capture_failed) {
+      if (!exec) {
+        // capture one step: kernels, memsets and stream-ordered allocations become graph nodes
+        const bool was_profiling = ctx->profiling;
+        ctx->profiling = false;
+        cudaGraph_t graph = nullptr;
+        int s = MLIP_OK;
+        // the legacy default stream cannot be captured: record on a private stream, replay on the context stream
+        cudaStream_t cap = nullptr;
+        if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) == cudaSuccess) {
+          ctx->stream = cap;
+          cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+          if (e == cudaSuccess) {
+            s = step_eager();
+            e = cudaStreamEndCapture(cap, &graph);
+          }
+          ctx->stream = st;
+          if (s == MLIP_OK && e == cudaSuccess && graph) e = cudaGraphInstantiate(&exec, graph, 0);
+          if (s != MLIP_OK || e != cudaSuccess) {
+            exec = nullptr;
+            capture_error = e != cudaSuccess ? cudaGetErrorString(e) : ctx->err;
+          }
+          if (graph) cudaGraphDestroy(graph);
+          cudaStreamDestroy(cap);
+        }
+        ctx->profiling = was_profiling;
+        cudaGetLastError();
+        if (!exec) capture_failed = true;   // fall back to plain launches for the rest of the run
+      }
+      if (exec) {
+        MLIP_CUDA_CHECK(ctx, cudaGraphLaunch(exec, st));
+        ++n_replays;
+        return MLIP_OK;
+      }
+    }
+    return step_eager();
   }
 };
 }  // namespace
@@ -181,6 +303,7 @@ extern "C" int mlip_md_run(mlip_ctx* ctx, const mlip_model* M, int L, double* po
   if (e == cudaSuccess) cudaEventElapsedTime(&ms, t0, t1);
   ctx->event_pool.push_back(t0); ctx->event_pool.push_back(t1);
   if (stats) { stats->n_rebuilds = ev.n_rebuilds; stats->n_graph_replays = ev.n_replays; stats->ms_total = ms; }
+  if (ev.capture_failed) ctx->set_error("md: CUDA-graph capture failed (" + ev.capture_error + "); the run used plain launches");
   if (status != MLIP_OK) return status;
   if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) { ctx->set_error(std::string("md: ") + cudaGetErrorString(e)); return MLIP_ERR_CUDA; }
   return mlip_take_dev_status(ctx);

@@ -140,7 +140,7 @@ inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); 
 
 void free_sub(mlip_ctx* c, PartSub& s) {
   c->free(s.gid); c->free(s.species); c->free(s.rowptr); c->free(s.recv); c->free(s.send); c->free(s.rev);
-  c->free(s.omega); c->free(s.rvec);
+  c->free(s.omega); c->free(s.rvec); c->free(s.geid);
 }
 }  // namespace
 
@@ -153,7 +153,20 @@ extern "C" void mlip_part_destroy(mlip_part* p) {
 extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo,
                                    mlip_part** out) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
-  if (!G || !grid || !out || grid[0] < 1 || grid[1] < 1 || grid[2] < 1 || !(halo >= 0.0)) {
+  if (!G) { ctx->set_error("mlip_partition_grid: invalid argument"); return MLIP_ERR_INVALID_ARG; }
+  return mlip_partition_grid_ex(ctx, G, grid, halo, halo, G->r_cut, false, false, out);
+}
+
+// halo_box: width of the geometric box the extended set is searched in; halo / r_class: the number of shells
+// K = ceil(halo / r_class) (depth classes, levels of the K-hop search). The public call uses halo_box = halo and
+// r_class = the graph's cutoff; the Verlet-skin MD driver partitions the CANDIDATE graph (cutoff r_c + skin) with
+// halo_box = halo + skin (atoms move by up to skin/2 each before the next rebuild) and r_class = r_c, forces the K-hop
+// rule (hop counts over the candidate graph are lower bounds of the hop counts over any later exact graph) and keeps the
+// global edge id of every sub-domain edge.
+int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo_box, double halo,
+                           double r_class, bool force_khop, bool keep_geid, mlip_part** out) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!G || !grid || !out || grid[0] < 1 || grid[1] < 1 || grid[2] < 1 || !(halo >= 0.0) || !(halo_box >= halo) || !(r_class > 0.0)) {
     ctx->set_error("mlip_partition_grid: invalid argument");
     return MLIP_ERR_INVALID_ARG;
   }
@@ -168,13 +181,13 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
   ProfScope prof(ctx, MLIP_PROF_PARTITION);
 #define P_TRY(x) do { int _s = (x); if (_s != MLIP_OK) return fail(_s); } while (0)
   // depth classes 0 .. n_cls-1 (see SubGraph): the halo spans ceil(halo / r_c) shells of thickness r_c
-  int n_cls = 1 + (int)ceil(halo / G->r_cut - 1e-9);
+  int n_cls = 1 + (int)ceil(halo / r_class - 1e-9);
   if (n_cls < 2) n_cls = 2;
   if (n_cls > MLIP_MAX_CLS) {
     ctx->set_error("partition: halo spans more than 31 shells of thickness r_cut (ceil(halo / r_cut) > 31)");
     return fail(MLIP_ERR_UNSUPPORTED);
   }
-  const bool bfs = ctx->khop_halo;
+  const bool bfs = ctx->khop_halo || force_khop;
   P->khop = bfs;
   const int64_t CN = (int64_t)n_cls * N;
   if (CN >= (int64_t)1 << 31) { ctx->set_error("partition: n_cls * N >= 2^31"); return fail(MLIP_ERR_OVERFLOW); }
@@ -189,7 +202,7 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
         BinGeom b;
         b.bin[0] = bx; b.bin[1] = by; b.bin[2] = bz;
         for (int k = 0; k < 3; ++k) {
-          b.grid[k] = grid[k]; b.halo_frac[k] = halo / G->width[k]; b.width_over_rc[k] = G->width[k] / G->r_cut;
+          b.grid[k] = grid[k]; b.halo_frac[k] = halo_box / G->width[k]; b.width_over_rc[k] = G->width[k] / r_class;
         }
         P->subs.emplace_back();
         PartSub& S = P->subs.back();
@@ -238,7 +251,8 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
           ctx->launches += 2;
         }
         ctx->free(deg); deg = nullptr;
-        ctx->free(geid); geid = nullptr;
+        if (keep_geid) S.geid = geid; else ctx->free(geid);
+        geid = nullptr;
         S.g.n = n_ext; S.g.n_owned = N > 0 ? cls_start[1] : 0; S.g.E = E;
         S.g.n_cls = n_cls;
         for (int c = 0; c < n_cls; ++c) { S.g.n_le[c] = N > 0 ? cls_start[c + 1] : 0; S.g.E_le[c] = E_at[c]; }

@@ -263,10 +263,12 @@ __global__ void __launch_bounds__(WARPS * 32) k_triplet_bwd(int64_t n, float r3,
 }
 
 // zbar_k = sum over in-edges e of k with rev[e] < E_act of zeta[rev[e]]; hbar_k += G^T (zbar_k * z_k (1 - z_k))
-__global__ void __launch_bounds__(256) k_gate_bwd(int64_t n, int64_t E_act, int d, const int32_t* __restrict__ rowptr,
+__global__ void __launch_bounds__(256) k_gate_bwd(int64_t n, int64_t E_act, const int32_t* __restrict__ E_act_dyn, int d,
+                                                  const int32_t* __restrict__ rowptr,
                                                   const int32_t* __restrict__ rev, const float* __restrict__ zeta,
                                                   const float* __restrict__ z, const float* __restrict__ G,
                                                   float* __restrict__ hbar) {
+  if (E_act_dyn) E_act = *E_act_dyn;
   const int lane = threadIdx.x & 31;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (k >= n) return;
@@ -309,10 +311,10 @@ int mlip_triplet_backward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t
   ctx->launches++;
   return MLIP_OK;
 }
-int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, int d, const int32_t* rowptr, const int32_t* rev,
-                       const float* zeta, const float* z, const float* G, float* hbar) {
+int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
+                       const int32_t* rev, const float* zeta, const float* z, const float* G, float* hbar) {
   if (n_send <= 0) return MLIP_OK;
-  k_gate_bwd<<<nblk(n_send * 32, 256), 256, 0, ctx->stream>>>(n_send, E_act, d, rowptr, rev, zeta, z, G, hbar);
+  k_gate_bwd<<<nblk(n_send * 32, 256), 256, 0, ctx->stream>>>(n_send, E_act, E_act_dyn, d, rowptr, rev, zeta, z, G, hbar);
   ctx->launches++;
   return MLIP_OK;
 }

@@ -65,3 +65,42 @@ def test_langevin_zero_friction_is_nve_and_thermostat_sets_temperature():
                              temperature=T, friction=0.05, seed=99)
     T_kin = np.sum(masses[:, None] * vel ** 2) / O.ACC_UNIT / (3 * len(masses) * O.KB_EV)
     assert abs(T_kin / T - 1.0) < 0.15, T_kin
+
+
+@pytest.mark.parametrize("grid,halo,graph", [((1, 1, 1), 0.0, False), ((2, 1, 1), 6.0, False), ((1, 1, 1), 0.0, True),
+                                             ((2, 1, 1), 6.0, True)])
+def test_verlet_skin_reuse_matches_rebuild_every_step(grid, halo, graph):
+    """skin > 0: graph and partition are kept until an atom has moved skin/2; every step the candidate list is filtered
+    with the canonical predicate, so the edge set of every step is the one a rebuild gives and the trajectory agrees
+    with the rebuild-every-step run and with the oracle to fp32 accuracy; with cuda_graph the steps between rebuilds are
+    replays of one captured CUDA graph."""
+    spec, blob, s, masses, vel0 = _start(T0=0.006)
+    n_steps, dt = 30, 2.0
+    e0, p0, v0, st0 = _gpu_md(spec, blob, s, masses, vel0, dt, n_steps, grid=grid, halo=halo)
+    e1, p1, v1, st1 = _gpu_md(spec, blob, s, masses, vel0, dt, n_steps, grid=grid, halo=halo, skin=0.4, cuda_graph=graph)
+    kin0 = 0.5 * np.sum(masses[:, None] * vel0 ** 2) / O.ACC_UNIT
+    assert st0["n_rebuilds"] == n_steps + 1
+    assert 1 < st1["n_rebuilds"] < n_steps / 2, st1          # rebuilt when needed (atoms move ~0.7 A), not every step
+    assert np.abs(e1 - e0).max() <= 1e-4 * kin0
+    assert np.abs(p1 - p0).max() <= 1e-5 and np.abs(v1 - v0).max() <= 1e-5 * np.abs(v0).max() + 1e-8
+    if graph:
+        assert st1["n_graph_replays"] == n_steps + 1, st1
+    e_ref, pos_ref, _ = O.nve_velocity_verlet(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses, vel0, dt, n_steps,
+                                              return_state=True)
+    assert np.abs(e1 - e_ref).max() <= 1e-4 * kin0 and np.abs(p1 - pos_ref).max() <= 1e-5
+
+
+def test_verlet_skin_bf16_partitioned_langevin():
+    import paper_2509_21694_b200 as mlip
+    spec = ModelSpec(4, 128, 16, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 36)
+    s = small_system(8, 0.08, seed=62)
+    rng = np.random.default_rng(8)
+    masses = rng.uniform(10.0, 60.0, len(s.pos))
+    vel0 = rng.normal(0, 0.005, s.pos.shape); vel0 -= vel0.mean(0)
+    kw = dict(grid=(2, 2, 1), halo=6.0, precision=mlip.MLIP_BF16, thermostat=mlip.MLIP_MD_LANGEVIN, temperature=500.0,
+              friction=0.01, seed=3)
+    e0, p0, v0, _ = _gpu_md(spec, blob, s, masses, vel0, 2.0, 20, **kw)
+    e1, p1, v1, st = _gpu_md(spec, blob, s, masses, vel0, 2.0, 20, skin=0.5, cuda_graph=True, **kw)
+    assert st["n_graph_replays"] == 21 and st["n_rebuilds"] < 10
+    assert np.abs(p1 - p0).max() <= 2e-3      # 16-bit forces, different tile boundaries: agreement to bf16-path accuracy
