@@ -41,6 +41,7 @@
 // waited for once per tile, after that G1; the first layer runs with node_adjoint = false (no spill, no
 // segmented sum) and with row_index = species (P, Q are S-row tables).
 #include <cuda_fp16.h>
+#include <type_traits>
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
@@ -669,6 +670,10 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
       // ---- E1: a' = X + P'_i + Q'_j ; s = a' + a' tanh(a') ----
       tc::mbar_wait(bar(B_D1_FULL), par);
       tc::fence_after_sync();
+      // (the loop exists twice, for tiles whose receiver rows are staged in shared memory and for the others: a per-load
+      // select between the two sources costs the staged path the registers and scoreboards of the global loads)
+      auto e1_loop = [&](auto staged) {
+      constexpr bool STAGED = decltype(staged)::value;
 #pragma unroll
       for (int s = 0; s < NCH; ++s) {
         uint32_t acc[16];
@@ -676,7 +681,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         const uint4 q0 = qb[s % QD][0], q1 = qb[s % QD][1];
         if (s + QD - 1 < NCH) ldg_nc_v8(Qrow + 64 * (s + QD - 1), qb[(s + QD - 1) % QD][0], qb[(s + QD - 1) % QD][1]);
         uint4 p0, p1;
-        if (fast) {
+        if constexpr (STAGED) {
           p0 = *reinterpret_cast<const uint4*>(prow + 128 * s);
           p1 = *reinterpret_cast<const uint4*>(prow + 128 * s + 16);
         } else {
@@ -708,6 +713,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         }
         publish_tmem(s);
       }
+      };
+      if (fast) e1_loop(std::true_type{}); else e1_loop(std::false_type{});
       if (!BWD && lane == 0) mbar_arrive(bar(B_X_FREE));  // X is dead: G1 of the next tile may run
       if (lane == 0) mbar_arrive(bar(B_P_FREE));           // staged P rows may be replaced
 
@@ -758,6 +765,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
         float ub = 0.f;
         tc::mbar_wait(bar(B_D2_FULL), par);
         tc::fence_after_sync();
+        auto e2_loop = [&](auto staged) {
+        constexpr bool STAGED = decltype(staged)::value;
 #pragma unroll
         for (int s = 0; s < NCH; ++s) {
           if (s == NCH / 2) { tc::mbar_wait(bar(B_D2B_FULL), par); tc::fence_after_sync(); }
@@ -767,7 +776,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           const uint4 c1 = *reinterpret_cast<const uint4*>(b2h + 128 * s + 16);
           const uint32_t bw[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
           uint32_t mb[8];
-          if (fast) {
+          if constexpr (STAGED) {
             const uint4 m0 = *reinterpret_cast<const uint4*>(mrow + 128 * s);
             const uint4 m1 = *reinterpret_cast<const uint4*>(mrow + 128 * s + 16);
             mb[0] = m0.x; mb[1] = m0.y; mb[2] = m0.z; mb[3] = m0.w; mb[4] = m1.x; mb[5] = m1.y; mb[6] = m1.z; mb[7] = m1.w;
@@ -792,6 +801,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
           tc::tmem_st8(TY + tlane + (uint32_t)(64 * s + 16 * g), v);
           publish_tmem(s);
         }
+        };
+        if (fast) e2_loop(std::true_type{}); else e2_loop(std::false_type{});
         if (lane == 0) mbar_arrive(bar(B_MB_FREE));
         ubar_s[g * TE + row] = ub;
         fetch_next();
