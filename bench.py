@@ -47,6 +47,11 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-active-sets", action="store_true",
                     help="evaluate every layer on the whole extended sub-graph (A/B against the per-layer active sets)")
+    ap.add_argument("--md", action="store_true",
+                    help="time the on-device MD driver mlip_md_run (Langevin, --steps steps) instead of single evaluations; "
+                         "--skin / --cuda-graph select Verlet-skin reuse and CUDA-graph replay")
+    ap.add_argument("--skin", type=float, default=0.0)
+    ap.add_argument("--cuda-graph", action="store_true")
     ap.add_argument("--n-cells", type=int, default=None, help="shrink the fcc box (debugging only; not a bench line)")
     return ap.parse_args()
 
@@ -428,9 +433,50 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_md(args):
+    """atom-steps/s of the MD driver: K Langevin steps of 2 fs at 300 K on the configuration's
+    system, device-timed inside mlip_md_run (CUDA events around the K steps). Not the BASELINE metric: a secondary line."""
+    import torch
+
+    import paper_2509_21694_b200 as mlip
+    from synth_inputs import make_config
+
+    cfg = make_config(args.config, n_cells_override=args.n_cells)
+    s, m = cfg.system, cfg.model
+    prec_name = cfg.precision if args.precision == "auto" else args.precision
+    prec = mlip.MLIP_BF16 if prec_name == "bf16" else mlip.MLIP_FP32
+    N = len(s.pos)
+    dev = "cuda:0"
+    ctx = mlip.Context(0)
+    model = mlip.Model(ctx, m.n_species, m.d, m.n_rbf, m.L_max, m.r_cut, m.agg_scale, cfg.weights, r_cut3=m.r_cut3)
+    rng = np.random.default_rng(5000 + args.config)
+    mass = torch.full((N,), 30.0, dtype=torch.float64, device=dev)
+    species = torch.tensor(s.species, dtype=torch.int32, device=dev)
+    kw = dict(grid=cfg.grid, halo=cfg.halo, precision=prec, thermostat=mlip.MLIP_MD_LANGEVIN, temperature=300.0, friction=0.01,
+              seed=1, skin=args.skin, cuda_graph=args.cuda_graph)
+    out = None
+    for it in range(2):   # the first run warms up (allocator pool, kernel images)
+        pos = torch.tensor(s.pos, dtype=torch.float64, device=dev).contiguous()
+        vel = torch.tensor(rng.normal(0, 0.003, s.pos.shape), dtype=torch.float64, device=dev).contiguous()
+        launches0 = ctx.launches
+        e, st = mlip.md_run(ctx, model, cfg.L, pos, vel, mass, s.cell, species, 2.0, args.steps if it else max(2, args.warmup), **kw)
+        out = (e, st, ctx.launches - launches0)
+    e, st, launches = out
+    ms = st["ms_total"] / args.steps
+    line = {"metric": "atom-steps/s (MD, Langevin)", "value": N / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f16/bf16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, N), "dt_fs": 2.0, "temperature_K": 300.0, "skin": args.skin,
+                       "cuda_graph": bool(args.cuda_graph)},
+            "md_stats": st, "gpu_launches": int(launches), "energy_first_last": [float(e[0]), float(e[-1])]}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.md:
+        run_md(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -47,7 +47,8 @@ MLIP_MD_LANGEVIN = 1
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, "libmlip_b200.so")
+    """The in-tree library; MLIP_B200_LIB selects another build of the same sources (A/B measurements)."""
+    return os.environ.get("MLIP_B200_LIB") or os.path.join(_HERE, "libmlip_b200.so")
 
 
 def load_library():
