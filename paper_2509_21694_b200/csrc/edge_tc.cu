@@ -40,6 +40,8 @@
 // slab by slab as E3 publishes (X columns released), ahead of that slab's G4 / GS; the spill copies are only
 // waited for once per tile, after that G1; the first layer runs with node_adjoint = false (no spill, no
 // segmented sum) and with row_index = species (P, Q are S-row tables).
+#include <cuda.h>
+#include <string.h>
 #include <cuda_fp16.h>
 #include <type_traits>
 #include "common.cuh"
@@ -200,7 +202,8 @@ __device__ __forceinline__ void segmented_store_tc(const unsigned char* __restri
 }
 
 template <int D, bool BWD>
-__global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_tiles_cap) {
+__global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_tiles_cap,
+                                                          const __grid_constant__ CUtensorMap spill_map) {
   extern __shared__ unsigned char smem_raw[];
   // number of edges: by value, or read from the device in Verlet-skin mode (EdgeArgs::E_dyn; a.E is then the capacity)
   const int64_t n_edges = a.E_dyn ? (int64_t)__ldg(a.E_dyn) : a.E;
@@ -522,8 +525,9 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
             if (s == NCH - 1) tc::mma_commit(bar(B_D1_FULL));
           }
           if (BWD) {
-            if (a.node_adjoint)
-              tc::bulk_s2g(a.abar_h + (size_t)tile * TE * D + (size_t)s * TE * 64, base + SM::ring + s * SLOT_BYTES, SLOT_BYTES);
+            // ā slab -> ROW-MAJOR spill [edge][channel] by a tensor-map store (the copy engine undoes the 128-byte swizzle),
+            // so that the sender-side gather reads 2 d contiguous bytes per reverse edge
+            if (a.node_adjoint) tc::tma_store_2d(&spill_map, base + SM::ring + s * SLOT_BYTES, 64 * s, (int)(tile * TE));
             tc::bulk_commit();  // one bulk group per slab: a slab is released as soon as ITS copy has read it
             // G4: ebar/2 = abar . (W1c/2). B = the G1 image [channel][16] read MN-major (N = rbf index, K = channel),
             // no swizzle: N-direction core-matrix stride (SBO) 128 B, K-direction 8-channel group stride (LBO) 256 B
@@ -869,7 +873,7 @@ __global__ void __launch_bounds__(256) k_segment_fixup_tc(int64_t E, const int32
   *reinterpret_cast<float4*>(out + (size_t)i * D + c) = sum;
 }
 
-// Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar rows live in the swizzled f16 tile images written by E3
+// Qbar_j = sum_{e in in(j)} abar[rev[e]]; abar is the row-major f16 spill [edge][channel] written by the tensor-map stores
 template <int D>
 __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act, const int32_t* __restrict__ E_act_dyn,
                                                        const int32_t* __restrict__ rowptr,
@@ -888,8 +892,7 @@ __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act,
   for (int e = lo + sub; e < hi; e += NSUB) {
     const int re = rev[e];
     if (re >= E_act) continue;  // reverse edge outside this layer's active set: its adjoint is zero and was not written
-    const int t = re >> 7, rw = re & 127;
-    const uint4 v = *reinterpret_cast<const uint4*>(base + (size_t)t * TE * D * 2 + tc::sw128_chunk_off(TE, rw, ch));
+    const uint4 v = *reinterpret_cast<const uint4*>(base + (size_t)re * (D * 2) + ch * 16);
     const float2 f0 = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
     const float2 f1 = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
     const float2 f2 = __half22float2(*reinterpret_cast<const __half2*>(&v.z));
@@ -908,14 +911,46 @@ __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act,
   }
 }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+encode_tiled_fn get_encode_tiled() {
+  static encode_tiled_fn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
+      fn = (encode_tiled_fn)p;
+  }
+  return fn;
+}
+// row-major f16 spill [rows][d], stored in boxes of 64 channels x 128 edges out of SWIZZLE_128B slabs
+int make_spill_map(mlip_ctx* ctx, __half* abar, int64_t rows, int d, CUtensorMap* map) {
+  memset(map, 0, sizeof(*map));
+  if (!abar || rows <= 0) return MLIP_OK;
+  encode_tiled_fn enc = get_encode_tiled();
+  if (!enc) { ctx->set_error("cuTensorMapEncodeTiled not available"); return MLIP_ERR_CUDA; }
+  const cuuint64_t gdim[2] = {(cuuint64_t)d, (cuuint64_t)rows};
+  const cuuint64_t gstride[1] = {(cuuint64_t)d * 2};
+  const cuuint32_t box[2] = {64, (cuuint32_t)TE};
+  const cuuint32_t estr[2] = {1, 1};
+  const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, abar, gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { ctx->set_error("cuTensorMapEncodeTiled failed"); return MLIP_ERR_CUDA; }
+  return MLIP_OK;
+}
+
 template <int D, bool BWD>
 int launch_edge_dir(mlip_ctx* ctx, const EdgeArgs& a) {
   const int64_t tiles = (a.E + TE - 1) / TE;
   if (tiles == 0) return MLIP_OK;
+  CUtensorMap spill_map;
+  MLIP_TRY(make_spill_map(ctx, (BWD && a.node_adjoint) ? a.abar_h : nullptr, tiles * TE, D, &spill_map));
   const size_t smem = ES<D, BWD>::bytes;
   const unsigned grid = (unsigned)(tiles < ctx->num_sms ? tiles : ctx->num_sms);
   MLIP_CUDA_CHECK(ctx, cudaFuncSetAttribute(k_edge_tc<D, BWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  k_edge_tc<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles);
+  k_edge_tc<D, BWD><<<grid, N_THREADS, smem, ctx->stream>>>(a, tiles, spill_map);
   ctx->launches++;
   if (!BWD || a.node_adjoint) {
     const int64_t tiles_per_block = 256 / (D / 4);

@@ -174,6 +174,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t saddr, const void* gmem, uint3
 __device__ __forceinline__ void bulk_s2g(void* gmem, uint32_t saddr, uint32_t bytes) {
   asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gmem), "r"(saddr), "r"(bytes) : "memory");
 }
+// 2-D tensor-map (TMA) store shared -> global, bulk async-group: the box of the map (SWIZZLE_128B in shared memory) goes
+// to element coordinates (x = innermost, y) of the global tensor, un-swizzled by the copy engine
+__device__ __forceinline__ void tma_store_2d(const void* tmap, uint32_t saddr, int x, int y) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(tmap), "r"(saddr), "r"(x), "r"(y)
+               : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>  // at most N of the newest bulk groups may still be reading their shared-memory source
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
