@@ -113,7 +113,7 @@ __device__ __forceinline__ void segmented_store(const float* __restrict__ X, con
 }
 
 template <int D, bool BWD>
-__global__ void __launch_bounds__(256, 1) k_edge_f32(EdgeArgs a) {
+__global__ void __launch_bounds__(256, (D <= 128 ? (BWD ? 2 : 3) : 1)) k_edge_f32(EdgeArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   using SM = Smem<D>;
   constexpr int LDS = SM::LDS;
