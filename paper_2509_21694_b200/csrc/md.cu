@@ -241,7 +241,7 @@ extern "C" int mlip_md_run(mlip_ctx* ctx, const mlip_model* M, int L, double* po
                            const int grid[3], double halo, int precision, const mlip_md_params* prm,
                            double* total_energy_host, mlip_md_stats* stats) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
-  if (!M || !pos_dev || !vel_dev || !mass_dev || !cell_host || !species_dev || !grid || !prm || N < 0 || prm->n_steps < 0 ||
+  if (!M || (N > 0 && (!pos_dev || !vel_dev || !mass_dev || !species_dev)) || !cell_host || !grid || !prm || N < 0 || prm->n_steps < 0 ||
       !(prm->dt > 0.0) || (prm->thermostat != MLIP_MD_NVE && prm->thermostat != MLIP_MD_LANGEVIN) || !(prm->skin >= 0.0)) {
     ctx->set_error("mlip_md_run: invalid argument");
     return MLIP_ERR_INVALID_ARG;

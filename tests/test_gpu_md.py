@@ -123,3 +123,29 @@ def test_md_three_body_skin_and_graph():
     e_ref, pos_ref, _ = O.nve_velocity_verlet(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses, vel0, 0.5, 20,
                                               return_state=True)
     assert np.abs(p1 - pos_ref).max() <= 1e-5
+
+
+def test_md_degenerate_calls():
+    """Zero steps (one evaluation, the initial total energy only), an empty system, and argument errors."""
+    import torch
+    import paper_2509_21694_b200 as mlip
+    spec, blob, s, masses, vel0 = _start(n_cells=3)
+    e, pos, vel, st = _gpu_md(spec, blob, s, masses, vel0, 2.0, 0, skin=0.3)
+    assert e.shape == (1,) and np.isfinite(e[0]) and np.array_equal(pos, s.pos) and st["n_rebuilds"] == 1
+    mlipm, ctx, model = gpu_setup(spec, blob)
+    z3 = torch.zeros((0, 3), dtype=torch.float64, device="cuda:0")
+    z1 = torch.zeros(0, dtype=torch.float64, device="cuda:0")
+    zi = torch.zeros(0, dtype=torch.int32, device="cuda:0")
+    for skin in (0.0, 0.3):
+        e, st = mlip.md_run(ctx, model, 2, z3, z3.clone(), z1, s.cell, zi, 2.0, 3, skin=skin)
+        assert np.all(e == 0.0)
+    pos = torch.tensor(s.pos, dtype=torch.float64, device="cuda:0")
+    vel = torch.zeros_like(pos)
+    mass = torch.tensor(masses, dtype=torch.float64, device="cuda:0")
+    sp = torch.tensor(s.species, dtype=torch.int32, device="cuda:0")
+    with pytest.raises(mlip.MlipError) as ei:      # CUDA-graph replay needs fixed launch dimensions, i.e. a skin
+        mlip.md_run(ctx, model, 2, pos, vel, mass, s.cell, sp, 2.0, 2, cuda_graph=True)
+    assert ei.value.code == -1
+    with pytest.raises(mlip.MlipError) as ei:      # halo < L r_cut is refused in skin mode too
+        mlip.md_run(ctx, model, 2, pos, vel, mass, s.cell, sp, 2.0, 2, grid=(2, 1, 1), halo=3.0, skin=0.3)
+    assert ei.value.code == -3
