@@ -4,6 +4,7 @@
 // (sender, shift), reverse-edge index. Steps A1-A4 of SURVEY.md 8(a).
 #include <math.h>
 #include <string.h>
+#include "canon.cuh"
 #include "common.cuh"
 
 namespace {
@@ -143,15 +144,9 @@ __global__ void __launch_bounds__(256) k_neighbors(int64_t N, CellGeom g,
             const int nx = s0 - wrap_s[3 * j] + wi0;
             const int ny = s1 - wrap_s[3 * j + 1] + wi1;
             const int nz = s2 - wrap_s[3 * j + 2] + wi2;
-            // canonical predicate (O1): t = (nx*a1 + ny*a2) + nz*a3; r = (xj - xi) + t
-            const double fx = (double)nx, fy = (double)ny, fz = (double)nz;
-            const double tx = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[0]), __dmul_rn(fy, g.cell[3])), __dmul_rn(fz, g.cell[6]));
-            const double ty = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[1]), __dmul_rn(fy, g.cell[4])), __dmul_rn(fz, g.cell[7]));
-            const double tz = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[2]), __dmul_rn(fy, g.cell[5])), __dmul_rn(fz, g.cell[8]));
-            const double rx = __dadd_rn(__dadd_rn(pos_s[3 * j], -xi), tx);
-            const double ry = __dadd_rn(__dadd_rn(pos_s[3 * j + 1], -yi), ty);
-            const double rz = __dadd_rn(__dadd_rn(pos_s[3 * j + 2], -zi), tz);
-            const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(rx, rx), __dmul_rn(ry, ry)), __dmul_rn(rz, rz));
+            // canonical predicate (O1): t = (nx*a1 + ny*a2) + nz*a3; r = (xj - xi) + t   (canon.cuh)
+            double rx, ry, rz;
+            const double d2 = canonical_rvec(g.cell, nx, ny, nz, xi, yi, zi, pos_s[3 * j], pos_s[3 * j + 1], pos_s[3 * j + 2], rx, ry, rz);
             ok = d2 < g.rc2 && !(j == i && nx == 0 && ny == 0 && nz == 0);
             if (ok && (nx < -127 || nx > 127 || ny < -127 || ny > 127 || nz < -127 || nz > 127)) {
               atomicOr(err_flag, 1);
@@ -245,15 +240,9 @@ __global__ void __launch_bounds__(256) k_finalize_edges(int64_t N, CellGeom g,
     const unsigned long long k = keys[e];
     const int j = (int)(k >> 24);
     const uint32_t ps = (uint32_t)(k & 0xffffffu);
-    const double fx = (double)((int)((ps >> 16) & 255) - 128), fy = (double)((int)((ps >> 8) & 255) - 128),
-                 fz = (double)((int)(ps & 255) - 128);
-    const double tx = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[0]), __dmul_rn(fy, g.cell[3])), __dmul_rn(fz, g.cell[6]));
-    const double ty = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[1]), __dmul_rn(fy, g.cell[4])), __dmul_rn(fz, g.cell[7]));
-    const double tz = __dadd_rn(__dadd_rn(__dmul_rn(fx, g.cell[2]), __dmul_rn(fy, g.cell[5])), __dmul_rn(fz, g.cell[8]));
-    const double rx = __dadd_rn(__dadd_rn(pos_s[3 * j], -xi), tx);
-    const double ry = __dadd_rn(__dadd_rn(pos_s[3 * j + 1], -yi), ty);
-    const double rz = __dadd_rn(__dadd_rn(pos_s[3 * j + 2], -zi), tz);
-    const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(rx, rx), __dmul_rn(ry, ry)), __dmul_rn(rz, rz));
+    double rx, ry, rz;
+    const double d2 = canonical_rvec(g.cell, (int)((ps >> 16) & 255) - 128, (int)((ps >> 8) & 255) - 128, (int)(ps & 255) - 128, xi, yi, zi,
+                                     pos_s[3 * j], pos_s[3 * j + 1], pos_s[3 * j + 2], rx, ry, rz);
     recv[e] = (int32_t)i;
     send[e] = j;
     shift[e] = (int32_t)ps;
