@@ -101,7 +101,17 @@ int mlip_ctx_status(mlip_ctx* ctx);
 /* Load a weight blob (HOST pointer, fp32, `n` floats, copied). Order, every matrix row-major
  * [out,in]:  T[S,d], E0[S], then for each of the L_max layers
  *   W1[d, 2d+n_rbf] (columns: receiver h_i | sender h_j | e_hat), b1[d], W2[d,d], b2[d],
- *   V1[d, 2d] (columns: h | m), c1[d], V2[d,d], c2[d];   finally Wo[d,d], bo[d], wo[d], b_E. */
+ *   V1[d, 2d] (columns: h | m), c1[d], V2[d,d], c2[d]
+ *   (and, with MLIP_FLAG_THREE_BODY, G[16,d], g[16], W3[d,16]);   finally Wo[d,d], bo[d], wo[d], b_E.
+ *
+ * Three-body (angle) variant, BASELINE.json config 5 (the paper's workhorse MatterSim is an M3GNet-type model,
+ * PAPER.md:91,119,131; the paper gives no equations -- definition O7 of DESIGN.md): for edges with
+ * r_e < r_cut3 the first edge linear gets the extra term W3 t_e with
+ *   t_e = u3(r_e) sum over in-edges e' = (i <- k) != e of the same receiver, r_e' < r_cut3, of
+ *         u3(r_e') [Y_l^0(cos theta_ee') g3_n(r_e')]_{4l+n} * sigmoid(G h_k + g),     l = 0..3, n = 0..3,
+ * u3 the cosine envelope on [0, r_cut3], g3_n Gaussians centred at n r_cut3 / 3 of width r_cut3 / 3, theta the angle at
+ * the receiver. Needs n_rbf3 = 4, l_max = 3, 0 < r_cut3 <= r_cut (the halo stays L r_cut); evaluated in MLIP_FP32 only;
+ * at most 128 neighbours inside r_cut3 per atom (else MLIP_ERR_UNSUPPORTED from the next synchronising call). */
 int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const float* w_host, size_t n,
                     mlip_model** out);
 void mlip_model_destroy(mlip_model* m);
