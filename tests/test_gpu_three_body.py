@@ -127,3 +127,20 @@ def test_config5_full_size_partitioned():
         pos, cell, sp, k, r = _ball(s, i, cfg.L * m.r_cut + 0.5)
         E_ref = O.energy_forces(om, cfg.L, pos, cell, sp)[1][k]
         assert abs(Ei[i] - E_ref) <= 1e-5 * max(abs(E_ref), rms(Ei)), (i, Ei[i], E_ref)
+
+
+def test_three_body_too_many_short_neighbours_is_reported():
+    """More than 128 neighbours inside r3 (a dense random cluster): the staging area of the triplet kernels does not hold the
+    row; the outcome is the defined status MLIP_ERR_UNSUPPORTED (-2) at the next synchronising call, not a wrong force."""
+    import paper_2509_21694_b200 as mlip
+    rng = np.random.default_rng(3)
+    pos = rng.uniform(0.0, 6.0, (400, 3)) + 12.0        # 400 atoms in a 6 A cube: > 128 neighbours within 4 A
+    s = System(pos, np.eye(3) * 30.0, rng.integers(0, 2, 400).astype(np.int32))
+    spec = ModelSpec(2, 64, 8, 1, 5.0, 1.0 / np.sqrt(200.0), r_cut3=4.0)
+    blob = make_weights(spec, 540)
+    mlipm, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(mlipm, ctx, s, spec.r_cut)
+    mlip.energy_forces(ctx, model, 1, g, None, 0)
+    with pytest.raises(mlip.MlipError) as ei:
+        ctx.status()
+    assert ei.value.code == -2
