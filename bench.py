@@ -416,7 +416,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-        "dtype": "f16/bf16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
+        "dtype": "f16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg, N), "n_atoms": N, "n_edges": info["edges"],
                    "sub_domains": len(info["subs"]), "edges_in_subgraphs": int(edges_total),
                    "edge_layers_evaluated_per_step": int(edge_layers), "active_sets": not args.no_active_sets,
@@ -465,7 +465,7 @@ def run_md(args):
     ms = st["ms_total"] / args.steps
     line = {"metric": "atom-steps/s (MD, Langevin)", "value": N / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": "f16/bf16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
+            "dtype": "f16 operands, f32 accumulate (MLIP_BF16)" if prec_name == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": workload_name(cfg, N), "dt_fs": 2.0, "temperature_K": 300.0, "skin": args.skin,
                        "cuda_graph": bool(args.cuda_graph)},
             "md_stats": st, "gpu_launches": int(launches), "energy_first_last": [float(e[0]), float(e[-1])]}

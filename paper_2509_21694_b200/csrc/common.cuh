@@ -9,6 +9,13 @@
 #include <vector>
 #include "../../include/mlip.h"
 
+// 16-bit operand type of the node contractions (see tc_ptx.cuh): IEEE half unless MLIP_NODE_OPERANDS_BF16
+#ifdef MLIP_NODE_OPERANDS_BF16
+typedef __nv_bfloat16 mlip_nodeop;
+#else
+typedef __half mlip_nodeop;
+#endif
+
 #define MLIP_CUDA_CHECK(ctx, expr)                                                        \
   do {                                                                                    \
     cudaError_t _e = (expr);                                                              \
@@ -136,7 +143,7 @@ struct LayerWeights {
   float* b1h;     // [d] = b1 / 2 (bias of the halved receiver pre-projection of the bf16 path)
   // bf16 operand images for the tensor-core path (device, owned); see tc_common.cuh
   __half *W2img, *W1cimg;
-  __nv_bfloat16 *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;
+  mlip_nodeop *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;
 };
 
 struct mlip_model {
@@ -145,7 +152,7 @@ struct mlip_model {
   float* blob = nullptr;  // device copy of the caller's blob
   const float *T, *E0, *Wo, *bo, *wo, *bE;
   float* WoT = nullptr;   // [d,d]
-  __nv_bfloat16 *Wo_bf = nullptr, *WoT_bf = nullptr;
+  mlip_nodeop *Wo_bf = nullptr, *WoT_bf = nullptr;
   std::vector<LayerWeights> layers;
   std::vector<void*> owned;  // everything to cudaFree
 };
@@ -238,21 +245,21 @@ struct GemmArgs {
   const float* X2 = nullptr; int ld2 = 0; int K2 = 0;
   // tensor-core path only: a column block may be given as bf16 instead (same ld / K fields); it is then copied
   // into the operand slab as it is -- the value the fp32 form would have been rounded to on load
-  const __nv_bfloat16* X1b = nullptr;
-  const __nv_bfloat16* X2b = nullptr;
+  const mlip_nodeop* X1b = nullptr;
+  const mlip_nodeop* X2b = nullptr;
   int act_in = 0;                 // 1: SiLU applied to X on load
   const void* B = nullptr;        // [N, K1+K2] row-major (fp32 path) / bf16 SW128 operand image (tensor path)
   const float* bias = nullptr;    // [N]
   const float* mul_dsilu = nullptr; int ldz = 0;  // epilogue: y *= SiLU'(Z[row, col])
   const float* residual = nullptr; int ldr = 0;   // epilogue: y += R[row, col] (may alias Y)
   float* Y = nullptr; int ldy = 0;                // fp32 output (or)
-  __nv_bfloat16* Ybf = nullptr;                   // bf16 output (same ldy)
+  mlip_nodeop* Ybf = nullptr;                   // bf16 output (same ldy)
   __half* Yh = nullptr;                           // f16 output (same ldy)
   int64_t n = 0; int N = 0;
 };
 int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a);
 int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a);  // B = image built by mlip_make_gemm_image
-void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, __nv_bfloat16* img);
+void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, mlip_nodeop* img);
 
 // energy_forces.cu
 int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* m, int L, const SubGraph& g, int precision,

@@ -66,4 +66,4 @@ int64_t mlip_edge_tc_tiles(int64_t E);
 int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);
 int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
-                       const int32_t* rev, const __half* abar, __nv_bfloat16* Qbar /*[n,d] bf16*/);
+                       const int32_t* rev, const __half* abar, mlip_nodeop* Qbar /*[n,d] bf16*/);

@@ -878,7 +878,7 @@ template <int D>
 __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act, const int32_t* __restrict__ E_act_dyn,
                                                        const int32_t* __restrict__ rowptr,
                                                        const int32_t* __restrict__ rev, const __half* __restrict__ abar,
-                                                       __nv_bfloat16* __restrict__ Qbar) {
+                                                       mlip_nodeop* __restrict__ Qbar) {
   if (E_act_dyn) E_act = *E_act_dyn;
   constexpr int CH = D / 8;        // 16-byte chunks per row
   constexpr int NSUB = 32 / CH;    // edges handled concurrently by one warp
@@ -907,7 +907,7 @@ __global__ void __launch_bounds__(256) k_gather_rev_tc(int64_t n, int64_t E_act,
   if (sub == 0) {
     // Qbar is only ever read as a bf16 GEMM operand: stored as the value the operand producer would round it to
     *reinterpret_cast<uint4*>(Qbar + (size_t)j * D + ch * 8) =
-        make_uint4(tc::pack_bf16(acc[0], acc[1]), tc::pack_bf16(acc[2], acc[3]), tc::pack_bf16(acc[4], acc[5]), tc::pack_bf16(acc[6], acc[7]));
+        make_uint4(tc::pack_op(acc[0], acc[1]), tc::pack_op(acc[2], acc[3]), tc::pack_op(acc[4], acc[5]), tc::pack_op(acc[6], acc[7]));
   }
 }
 
@@ -978,7 +978,7 @@ int mlip_edge_backward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   return MLIP_ERR_UNSUPPORTED;
 }
 int mlip_gather_rev_tc(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
-                       const int32_t* rev, const __half* abar, __nv_bfloat16* Qbar) {
+                       const int32_t* rev, const __half* abar, mlip_nodeop* Qbar) {
   if (n <= 0) return MLIP_OK;
   const unsigned grid = (unsigned)((n * 32 + 255) / 256);
   if (d == 256) k_gather_rev_tc<256><<<grid, 256, 0, ctx->stream>>>(n, E_act, E_act_dyn, rowptr, rev, abar, Qbar);

@@ -5,12 +5,13 @@
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
+#include "tc_ptx.cuh"
 
 namespace {
 inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 __global__ void k_embed(int64_t n, int d, const int32_t* __restrict__ species, const float* __restrict__ T,
-                        float* __restrict__ h, __nv_bfloat16* __restrict__ hb /*bf16 copy for the GEMM operands, or null*/) {
+                        float* __restrict__ h, mlip_nodeop* __restrict__ hb /*bf16 copy for the GEMM operands, or null*/) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= n * (d / 4)) return;
   const int64_t i = idx / (d / 4);
@@ -18,8 +19,7 @@ __global__ void k_embed(int64_t n, int d, const int32_t* __restrict__ species, c
   const float4 v = *reinterpret_cast<const float4*>(T + (size_t)species[i] * d + c);
   *reinterpret_cast<float4*>(h + i * d + c) = v;
   if (hb) {
-    __nv_bfloat162 lo = __floats2bfloat162_rn(v.x, v.y), hi = __floats2bfloat162_rn(v.z, v.w);
-    *reinterpret_cast<uint2*>(hb + i * d + c) = make_uint2(*reinterpret_cast<uint32_t*>(&lo), *reinterpret_cast<uint32_t*>(&hi));
+    *reinterpret_cast<uint2*>(hb + i * d + c) = make_uint2(tc::pack_op(v.x, v.y), tc::pack_op(v.z, v.w));
   }
 }
 
@@ -280,13 +280,13 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   // tensor-core path: tensors that are only ever read as bf16 GEMM operands are STORED as bf16 -- the value the operand
   // producer would round the fp32 form to, so results do not change while the HBM-bound node GEMMs move fewer bytes:
   // hb = copy of the residual stream h^l (two buffers, alternating), cbar_b, Qbar_b
-  __nv_bfloat16 *hb[2] = {nullptr, nullptr}, *cbar_b = nullptr, *Qbar_b = nullptr;
+  mlip_nodeop *hb[2] = {nullptr, nullptr}, *cbar_b = nullptr, *Qbar_b = nullptr;
   double* partial = nullptr;
   float* scale = nullptr;  // [2 + 1184]: s, 1/s of the reverse pass (MLIP_BF16), then the per-block maxima
   if (bf) {
     W_ALLOC(scale, float, 2 + 148 * 8);
-    W_ALLOC(hb[0], __nv_bfloat16, n * d); W_ALLOC(hb[1], __nv_bfloat16, n * d);
-    W_ALLOC(cbar_b, __nv_bfloat16, n * d); W_ALLOC(Qbar_b, __nv_bfloat16, n * d);
+    W_ALLOC(hb[0], mlip_nodeop, n * d); W_ALLOC(hb[1], mlip_nodeop, n * d);
+    W_ALLOC(cbar_b, mlip_nodeop, n * d); W_ALLOC(Qbar_b, mlip_nodeop, n * d);
   }
   auto from_h = [&](GemmArgs& a, int l) {  // X1 = h^l
     if (bf) a.X1b = hb[l & 1]; else a.X1 = h[l];

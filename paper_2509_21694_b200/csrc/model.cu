@@ -206,7 +206,7 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     k_copy_sub<<<(rows * cols + 255) / 256, 256, 0, st>>>(src, ld, r0, c0, tr, dst, ld_dst, rows, cols);
   };
   // bf16 SWIZZLE_128B operand image of a row-major [N, K] weight (node_bf16.cu streams it slab by slab)
-  auto toimg = [&](const float* src, __nv_bfloat16* dst, int N, int K, float scale = 1.0f) {
+  auto toimg = [&](const float* src, mlip_nodeop* dst, int N, int K, float scale = 1.0f) {
     mlip_make_gemm_image(st, src, N, K, scale, dst);
   };
   for (int l = 0; l < L; ++l) {
@@ -242,10 +242,10 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     cudaMemsetAsync(W.b1pad, 0, sizeof(float) * 2 * d, st);
     cudaMemcpyAsync(W.b1pad, W.b1, sizeof(float) * d, cudaMemcpyDeviceToDevice, st);
     // bf16 operand images for the tensor-core node GEMMs (B operands are [N, K])
-    M_ALLOC(W.W1a_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1b_bf, __nv_bfloat16, d * d);
-    M_ALLOC(W.V1_bf, __nv_bfloat16, 2 * d * d); M_ALLOC(W.V2_bf, __nv_bfloat16, d * d);
-    M_ALLOC(W.V2T_bf, __nv_bfloat16, d * d); M_ALLOC(W.V1aT_bf, __nv_bfloat16, d * d);
-    M_ALLOC(W.V1bT_bf, __nv_bfloat16, d * d); M_ALLOC(W.W1abT_bf, __nv_bfloat16, 2 * d * d);
+    M_ALLOC(W.W1a_bf, mlip_nodeop, d * d); M_ALLOC(W.W1b_bf, mlip_nodeop, d * d);
+    M_ALLOC(W.V1_bf, mlip_nodeop, 2 * d * d); M_ALLOC(W.V2_bf, mlip_nodeop, d * d);
+    M_ALLOC(W.V2T_bf, mlip_nodeop, d * d); M_ALLOC(W.V1aT_bf, mlip_nodeop, d * d);
+    M_ALLOC(W.V1bT_bf, mlip_nodeop, d * d); M_ALLOC(W.W1abT_bf, mlip_nodeop, 2 * d * d);
     // the tensor-core edge kernels consume HALVED pre-projections P' = (W1a h + b1)/2, Q' = (W1b h)/2 (exact scaling)
     toimg(W.W1ab, W.W1a_bf, d, d, 0.5f); toimg(W.W1ab + (size_t)d * d, W.W1b_bf, d, d, 0.5f);
     M_ALLOC(W.b1h, float, d);
@@ -263,7 +263,7 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   if (!upload_ok || src_off != n) { ctx->set_error("weight upload failed"); return fail(MLIP_ERR_CUDA); }
   M_ALLOC(M->WoT, float, d * d);
   sub(M->Wo, d, 0, 0, 1, M->WoT, d, d, d);
-  M_ALLOC(M->Wo_bf, __nv_bfloat16, d * d); M_ALLOC(M->WoT_bf, __nv_bfloat16, d * d);
+  M_ALLOC(M->Wo_bf, mlip_nodeop, d * d); M_ALLOC(M->WoT_bf, mlip_nodeop, d * d);
   toimg(M->Wo, M->Wo_bf, d, d); toimg(M->WoT, M->WoT_bf, d, d);
 #undef M_ALLOC
   if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {

@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
       const bool first = k0 < a.K1;
       const int ld = first ? a.ld1 : a.ld2;
       const int kx = (first ? k0 : k0 - a.K1) + c4 * 4;
-      const __nv_bfloat16* Xb = first ? a.X1b : a.X2b;
+      const mlip_nodeop* Xb = first ? a.X1b : a.X2b;
       if (Xb) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -143,8 +143,8 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
           pk = make_uint2(__float_as_uint(x.x), __float_as_uint(x.y));
         } else {
           if (a.act_in) { x.x = silu_f(x.x); x.y = silu_f(x.y); x.z = silu_f(x.z); x.w = silu_f(x.w); }
-          pk.x = tc::pack_bf16(x.x, x.y);
-          pk.y = tc::pack_bf16(x.z, x.w);
+          pk.x = tc::pack_op(x.x, x.y);
+          pk.y = tc::pack_op(x.z, x.w);
         }
         *reinterpret_cast<uint2*>(gen + SM::a_off(s) + tc::sw128_chunk_off(BM, r, c4 >> 1) + (c4 & 1) * 8) = pk;
       }
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
         const int64_t row0 = ((int64_t)blockIdx.x + (int64_t)(g / nk) * gridDim.x) * BM;
         const int k0 = (g % nk) * BK;
         const bool first = k0 < a.K1;
-        const __nv_bfloat16* Xb = (first ? a.X1b : a.X2b) + (first ? k0 : k0 - a.K1) + c8 * 8;
+        const mlip_nodeop* Xb = (first ? a.X1b : a.X2b) + (first ? k0 : k0 - a.K1) + c8 * 8;
         const int ld = first ? a.ld1 : a.ld2;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -216,7 +216,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
   } else if (warp == WARP_MMA) {
     // ======================= MMA issuer (one thread) =======================
     if (lane == 0) {
-      constexpr uint32_t IDESC = tc::idesc_bf16(128, N, 0, 0);
+      constexpr uint32_t IDESC = tc::idesc_op(128, N, 0, 0);
       int g = 0;
       if (RES) tc::mbar_wait(w_full, 0u);
       for (int it = 0; it < my_tiles; ++it) {
@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
           if (ok) {
             if (OM & 1) *reinterpret_cast<float4*>(a.Y + r * a.ldy + c) = w;
             if (OM & 2) *reinterpret_cast<uint2*>(a.Yh + r * a.ldy + c) = make_uint2(tc::pack_f16(w.x, w.y), tc::pack_f16(w.z, w.w));
-            if (OM & 4) *reinterpret_cast<uint2*>(a.Ybf + r * a.ldy + c) = make_uint2(tc::pack_bf16(w.x, w.y), tc::pack_bf16(w.z, w.w));
+            if (OM & 4) *reinterpret_cast<uint2*>(a.Ybf + r * a.ldy + c) = make_uint2(tc::pack_op(w.x, w.y), tc::pack_op(w.z, w.w));
           }
         }
       }
@@ -310,11 +310,11 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
 
 // W [N, K] fp32 row-major -> scale * W as the bf16 SWIZZLE_128B K-major operand image the kernel streams:
 // K/64 slabs of [N x 64] (N * 128 bytes each), element (n, k) at tc_sw128_index(N, n, k)
-__global__ void k_gemm_image(const float* __restrict__ W, int N, int K, float scale, __nv_bfloat16* __restrict__ img) {
+__global__ void k_gemm_image(const float* __restrict__ W, int N, int K, float scale, mlip_nodeop* __restrict__ img) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= N * K) return;
   const int n = idx / K, k = idx % K;
-  img[tc_sw128_index(N, n, k)] = __float2bfloat16_rn(scale * W[idx]);
+  img[tc_sw128_index(N, n, k)] = tc::float_to_op(scale * W[idx]);
 }
 
 template <int N, int ZM, int OM, bool RES, bool RAW>
@@ -361,7 +361,7 @@ int launch(mlip_ctx* ctx, const GemmArgs& a) {
 }
 }  // namespace
 
-void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, __nv_bfloat16* img) {
+void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, mlip_nodeop* img) {
   k_gemm_image<<<(N * K + 255) / 256, 256, 0, st>>>(W, N, K, scale, img);
 }
 

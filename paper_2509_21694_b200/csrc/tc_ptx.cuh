@@ -3,6 +3,7 @@
 // descriptor encodings used by the edge and node kernels (layouts documented in tc_images.cuh).
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -231,6 +232,22 @@ __device__ __forceinline__ float h2_hi(uint32_t v) {
   asm("{.reg .b16 l, h; mov.b32 {l, h}, %1; cvt.f32.f16 %0, h;}" : "=f"(f) : "r"(v));
   return f;
 }
+
+// ---- operand format of the node contractions ---------------------------------------------------------------------------
+// IEEE half by default: same tensor-core rate and bytes as bf16, three more mantissa bits (the L = 15 force error of BASELINE
+// config 3 is dominated by the operand rounding of the node GEMMs); the range contract of DESIGN.md R21 covers it, and the
+// reverse pass is scaled. -DMLIP_NODE_OPERANDS_BF16 restores bf16 operands (A/B measurements).
+#ifdef MLIP_NODE_OPERANDS_BF16
+typedef __nv_bfloat16 nodeop_t;
+__device__ __forceinline__ uint32_t pack_op(float lo, float hi) { return pack_bf16(lo, hi); }
+__device__ __forceinline__ nodeop_t float_to_op(float x) { return __float2bfloat16_rn(x); }
+__host__ __device__ constexpr uint32_t idesc_op(int M, int N, int a_mn, int b_mn) { return idesc_bf16(M, N, a_mn, b_mn); }
+#else
+typedef __half nodeop_t;
+__device__ __forceinline__ uint32_t pack_op(float lo, float hi) { return pack_f16(lo, hi); }
+__device__ __forceinline__ nodeop_t float_to_op(float x) { return __float2half_rn(x); }
+__host__ __device__ constexpr uint32_t idesc_op(int M, int N, int a_mn, int b_mn) { return idesc_f16(M, N, a_mn, b_mn); }
+#endif
 
 // byte offset of the 16-byte chunk `chunk` (8 bf16) of row `row` inside a K-major SWIZZLE_128B
 // operand tile of `rows` rows: 64-element slabs of rows x 128 B, chunk index XOR (row % 8)

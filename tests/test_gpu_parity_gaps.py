@@ -45,7 +45,7 @@ def test_full_size_config_2_and_3_bf16(c, name):
     assert np.isfinite(F).all()
     assert err["rms_F"] <= BF16_RMS_F                       # north_star: force RMS relative error of the bf16-GEMM path
     # not north_star bounds (the bf16-GEMM path is bounded on forces only): gross-error guards on the energies. Measured
-    # at L = 15: rms_F 1.66e-2, eps_E 4.7e-3, max |dE_i| / RMS E_i 6.5e-2 (a common shift, which cancels in the forces)
+    # at L = 15: rms_F 4.5e-3, eps_E 2.4e-3, max |dE_i| / RMS E_i 1.4e-2 (f16 node operands; 1.66e-2 / 4.7e-3 / 6.5e-2 with bf16)
     assert err["eps_E"] <= 1e-2 and err["max_Ei"] <= 1e-1
 
 
