@@ -143,6 +143,7 @@ struct LayerWeights {
   float* b1h;     // [d] = b1 / 2 (bias of the halved receiver pre-projection of the bf16 path)
   // bf16 operand images for the tensor-core path (device, owned); see tc_common.cuh
   __half *W2img, *W1cimg;
+  __nv_bfloat16 *W2x3 = nullptr, *W13x3 = nullptr;  // three-term split images of the fp32 tensor-core edge kernels (d = 128)
   mlip_nodeop *W1a_bf, *W1b_bf, *V1_bf, *V2_bf, *V2T_bf, *V1aT_bf, *V1bT_bf, *W1abT_bf;
 };
 

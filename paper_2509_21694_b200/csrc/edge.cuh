@@ -1,5 +1,6 @@
 // Argument block and launchers of the fused edge kernels (fp32 CUDA-core and bf16 tcgen05 paths).
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include "common.cuh"
 
@@ -25,6 +26,8 @@ struct EdgeArgs {
   const float* W2T = nullptr;                      // [in,out] fp32
   const float* W2 = nullptr;                       // [out,in] fp32
   const __half *W2img = nullptr, *W1cimg = nullptr;  // f16 operand images, tc_images.cuh
+  // fp32 path on the tensor cores (edge_x3.cu, d = 128): three-term bf16 split images of W2 and of [W1c | W3], or null
+  const __nv_bfloat16 *W2x3 = nullptr, *W13x3 = nullptr;
   const float* b2 = nullptr;
   float r_cut = 0.f, alpha = 0.f;
   int n_rbf = 0;
@@ -61,6 +64,11 @@ int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a);
 // Qbar_j = sum over in-edges e of j, j < n, with rev[e] < E_act, of abar[rev[e]]
 int mlip_gather_rev_f32(mlip_ctx* ctx, int64_t n, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
                         const int32_t* rev, const float* abar, float* Qbar);
+
+// fp32 operands split into three bf16 terms on tcgen05 (d = 128; mlip_edge_*_f32 dispatch to it)
+bool mlip_edge_x3_supported(int d, const EdgeArgs& a);
+int mlip_edge_forward_x3(mlip_ctx* ctx, const EdgeArgs& a);
+int mlip_edge_backward_x3(mlip_ctx* ctx, const EdgeArgs& a);
 
 int64_t mlip_edge_tc_tiles(int64_t E);
 int mlip_edge_forward_tc(mlip_ctx* ctx, int d, const EdgeArgs& a);

@@ -8,6 +8,8 @@
 // CUDA cores with W2 streamed through shared memory by cp.async. Segments that straddle tiles
 // are written as per-tile head/tail partial rows and combined in a fixed order by
 // k_segment_fixup: no floating-point atomics anywhere.
+#include <stdlib.h>
+#include <string.h>
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
@@ -375,7 +377,14 @@ int launch_edge(mlip_ctx* ctx, const EdgeArgs& a, bool bwd) {
 
 int64_t mlip_edge_f32_tiles(int64_t E) { return (E + TE - 1) / TE; }
 
+// MLIP_B200_FP32_EDGE=cuda keeps the CUDA-core kernels of this file at d = 128 too (A/B measurements)
+static bool use_x3(int d, const EdgeArgs& a) {
+  static const bool cuda_cores = [] { const char* v = getenv("MLIP_B200_FP32_EDGE"); return v && !strcmp(v, "cuda"); }();
+  return !cuda_cores && mlip_edge_x3_supported(d, a);
+}
+
 int mlip_edge_forward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a) {
+  if (use_x3(d, a)) return mlip_edge_forward_x3(ctx, a);
   switch (d) {
     case 64: return launch_edge<64>(ctx, a, false);
     case 128: return launch_edge<128>(ctx, a, false);
@@ -384,6 +393,7 @@ int mlip_edge_forward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a) {
   return MLIP_ERR_UNSUPPORTED;
 }
 int mlip_edge_backward_f32(mlip_ctx* ctx, int d, const EdgeArgs& a) {
+  if (use_x3(d, a)) return mlip_edge_backward_x3(ctx, a);
   switch (d) {
     case 64: return launch_edge<64>(ctx, a, true);
     case 128: return launch_edge<128>(ctx, a, true);

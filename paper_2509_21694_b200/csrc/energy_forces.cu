@@ -328,7 +328,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     ea.P = P[l]; ea.ldp = 2 * d; ea.Q = Qf[l]; ea.ldq = 2 * d; ea.Ph = Ph[l]; ea.Qh = Qh[l];
     ea.row_index = (bf && l == 0) ? g.species : nullptr;  // P^0, Q^0 are per-species tables (below)
     ea.W1c = W.W1c; ea.W2T = W.W2T; ea.W2 = W.W2; ea.b2 = W.b2;
-    ea.W2img = W.W2img; ea.W1cimg = W.W1cimg;
+    ea.W2img = W.W2img; ea.W1cimg = W.W1cimg; ea.W2x3 = W.W2x3; ea.W13x3 = W.W13x3;
   };
 
   // Active sets (SubGraph depth classes): layer l runs on receivers [0, nr) = classes <= L-1-l, reads senders

@@ -255,6 +255,10 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
     // operand images of the fused edge kernels (tc_images.cuh documents the layouts)
     M_ALLOC(W.W2img, __half, d * d); M_ALLOC(W.W1cimg, __half, d * 16);
     mlip_make_edge_images(st, W.W2, W.W1c, d, W.W2img, W.W1cimg);
+    if (d == 128) {
+      M_ALLOC(W.W2x3, __nv_bfloat16, 3 * d * d); M_ALLOC(W.W13x3, __nv_bfloat16, 3 * d * 32);
+      mlip_make_edge_images_x3(st, W.W2, W.W1c, W.W3, d, W.W2x3, W.W13x3);
+    }
   }
   M->Wo = take((size_t)d * d);
   M->bo = take(d);

@@ -12,6 +12,7 @@
 //    element (r, k) at (r/8)*SBO_e + (k/8)*LBO_e + (r%8)*8 + k%8 with LBO_e = 64 (128 B) and
 //    SBO_e = (K/8)*64.
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
@@ -29,3 +30,9 @@ __host__ __device__ inline int tc_nosw_index(int K, int r, int k) {
 // W1c [d,16] (padded)         -> W1cimg : no-swizzle K-major, rows = channel, K = 16, values W1c/2
 //                                         (read MN-major, N = rbf index, K = channel, for ebar = abar . W1c)
 void mlip_make_edge_images(cudaStream_t st, const float* W2, const float* W1c, int d, __half* W2img, __half* W1cimg);
+
+// fp32 path on the tensor cores (edge_x3.cu): x = x1 + x2 + x3, x1 = bf16(x), x2 = bf16(x - x1), x3 = bf16(x - x1 - x2).
+// W2x3  [3][d*d]  : the three terms of W2 (not halved), each in the SW128 K-major layout of W2img
+// W13x3 [3][d*32] : the three terms of [W1c | W3] [d,32] (W3 = 0 when null), no-swizzle K-major, rows = channel, K = 32
+void mlip_make_edge_images_x3(cudaStream_t st, const float* W2, const float* W1c, const float* W3, int d, __nv_bfloat16* W2x3,
+                              __nv_bfloat16* W13x3);
