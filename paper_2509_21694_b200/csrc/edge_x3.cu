@@ -197,80 +197,80 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
   constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);
   const float4* b2v = reinterpret_cast<const float4*>(a.b2);
 
+  // row metadata of a tile: fetched one tile ahead by every thread of the row
+  int rc_n = -1, sd_n = 0;
+  float r_n = 0.f;
+  auto fetch_meta = [&](int64_t tile) {
+    const int64_t e = tile * TE + row;
+    rc_n = -1; sd_n = 0; r_n = 0.f;
+    if (tile < n_tiles && e < n_edges) { rc_n = __ldg(a.recv + e); sd_n = __ldg(a.send + e); r_n = __ldg(&a.rvec[e].w); }
+  };
+  fetch_meta(blockIdx.x);
+
   for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
     const int64_t e0 = tile * TE;
+    const int rc = rc_n, sd = sd_n;
+    const float r_e = r_n;
+    const bool valid = rc >= 0;
+    // sender rows Q_j: random rows out of L2, requested before anything else of the tile is computed
+    float4 qf[NCH][4];
+    {
+      const float* Qrow = a.Q + (size_t)sd * a.ldq + 16 * g;
+#pragma unroll
+      for (int s = 0; s < NCH; ++s)
+#pragma unroll
+        for (int k4 = 0; k4 < 4; ++k4) qf[s][k4] = ldg4(Qrow + 64 * s + 4 * k4);
+    }
+    fetch_meta(tile + gridDim.x);
     // ================= P0: metadata, features, selector =================
-    if (tid < TE) {
-      const int64_t e = e0 + tid;
-      int rc = -1, sd = 0;
-      float r = 0.f, u = 0.f, du = 0.f;
-      if (e < n_edges) {
-        rc = a.recv[e]; sd = a.send[e]; r = a.rvec[e].w;
-        envelope_f(r, a.r_cut, u, du);
-      }
-      recv_s[tid] = rc; send_s[tid] = sd; u_s[tid] = u; du_s[tid] = du; r_s[tid] = r; w_s[tid] = a.alpha * u;
-      float eh[16];
-#pragma unroll
-      for (int k = 0; k < 16; ++k) {
-        float gk = 0.f, dg;
-        if (rc >= 0 && k < a.n_rbf) rbf_f(r, a.r_cut, a.n_rbf, k, gk, dg);
-        eh[k] = u * gk;
-      }
-      // A0 (row, k) -> (row/8)*512 + (k/8)*128 + (row%8)*16 + (k%8)*2, split i at i * 8192
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        uint32_t p[3][4];
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          uint32_t h[3];
-          split3(eh[8 * j + 2 * t], eh[8 * j + 2 * t + 1], h);
-          p[0][t] = h[0]; p[1][t] = h[1]; p[2][t] = h[2];
+    // A0 (row, k) -> (row/8)*512 + (k/8)*128 + (row%8)*16 + (k%8)*2, split i at i * 8192; column group g writes k = 8g..8g+7
+    {
+      float f[8];
+      if (g < 2) {
+        float u = 0.f, du = 0.f;
+        if (valid) envelope_f(r_e, a.r_cut, u, du);
+        if (g == 0) {
+          recv_s[row] = rc; send_s[row] = sd; u_s[row] = u; du_s[row] = du; r_s[row] = r_e; w_s[row] = a.alpha * u;
         }
 #pragma unroll
-        for (int i = 0; i < 3; ++i)
-          *reinterpret_cast<uint4*>(Aop + i * (TE * K1 * 2) + (tid >> 3) * 512 + j * 128 + (tid & 7) * 16) =
-              make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
-      }
-    } else if (tid < 2 * TE) {
-      const int er = tid - TE;
-      const int64_t e = e0 + er;
-      float t3[16];
+        for (int k = 0; k < 8; ++k) {
+          float gk = 0.f, dg;
+          if (valid && 8 * g + k < a.n_rbf) rbf_f(r_e, a.r_cut, a.n_rbf, 8 * g + k, gk, dg);
+          f[k] = u * gk;
+        }
+      } else {
 #pragma unroll
-      for (int k = 0; k < 16; ++k) t3[k] = 0.f;
-      if (a.t3 && e < n_edges) {
-#pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-          const float4 v = ldg4(a.t3 + (size_t)e * 16 + k4 * 4);
-          t3[4 * k4] = v.x; t3[4 * k4 + 1] = v.y; t3[4 * k4 + 2] = v.z; t3[4 * k4 + 3] = v.w;
+        for (int k = 0; k < 8; ++k) f[k] = 0.f;
+        if (a.t3 && valid) {
+          const float4 v0 = ldg4(a.t3 + (size_t)(e0 + row) * 16 + 8 * (g - 2)), v1 = ldg4(a.t3 + (size_t)(e0 + row) * 16 + 8 * (g - 2) + 4);
+          f[0] = v0.x; f[1] = v0.y; f[2] = v0.z; f[3] = v0.w; f[4] = v1.x; f[5] = v1.y; f[6] = v1.z; f[7] = v1.w;
         }
       }
+      uint32_t p[3][4];
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        uint32_t p[3][4];
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          uint32_t h[3];
-          split3(t3[8 * j + 2 * t], t3[8 * j + 2 * t + 1], h);
-          p[0][t] = h[0]; p[1][t] = h[1]; p[2][t] = h[2];
-        }
-#pragma unroll
-        for (int i = 0; i < 3; ++i)
-          *reinterpret_cast<uint4*>(Aop + i * (TE * K1 * 2) + (er >> 3) * 512 + (2 + j) * 128 + (er & 7) * 16) =
-              make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
+      for (int t = 0; t < 4; ++t) {
+        uint32_t h[3];
+        split3(f[2 * t], f[2 * t + 1], h);
+        p[0][t] = h[0]; p[1][t] = h[1]; p[2][t] = h[2];
       }
-    } else if (warp == SEG_WARP) {
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+        *reinterpret_cast<uint4*>(Aop + i * (TE * K1 * 2) + (row >> 3) * 512 + g * 128 + (row & 7) * 16) =
+            make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
+    }
+    if (warp == SEG_WARP) {
       // receivers of the tile in order of appearance, destination of each segment sum, 0/1 selector
-      int rc[4];
+      int rcv[4];
       uint32_t fm[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int e = lane + 32 * k;
         const int64_t ge = e0 + e;
         bool flag = false;
-        rc[k] = -1;
+        rcv[k] = -1;
         if (ge < n_edges) {
-          rc[k] = a.recv[ge];
-          flag = e == 0 || a.recv[ge - 1] != rc[k];
+          rcv[k] = a.recv[ge];
+          flag = e == 0 || a.recv[ge - 1] != rcv[k];
         }
         fm[k] = __ballot_sync(0xffffffffu, flag);
       }
@@ -280,8 +280,8 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       for (int k = 0; k < 4; ++k) {
         rloc[k] = before + __popc(fm[k] & (0xffffffffu >> (31 - lane))) - 1;
         if (((fm[k] >> lane) & 1u) && rloc[k] < MAX_SEG) {
-          const int64_t s0 = a.rowptr[rc[k]], s1 = a.rowptr[rc[k] + 1];
-          G.dst[rloc[k]] = (s0 >= e0 && s1 <= e0 + TE) ? (BWD ? a.Pbar : a.m) + (size_t)rc[k] * D
+          const int64_t s0 = a.rowptr[rcv[k]], s1 = a.rowptr[rcv[k] + 1];
+          G.dst[rloc[k]] = (s0 >= e0 && s1 <= e0 + TE) ? (BWD ? a.Pbar : a.m) + (size_t)rcv[k] * D
                                                        : (s0 < e0 ? a.head : a.tail) + (size_t)tile * D;
         }
         before += __popc(fm[k]);
@@ -295,7 +295,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         const int e = lane + 32 * k;
-        if (rc[k] >= 0 && rloc[k] < MAX_SEG)
+        if (rcv[k] >= 0 && rloc[k] < MAX_SEG)
           *reinterpret_cast<unsigned short*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 +
                                              (e & 7) * 2) = (unsigned short)0x3F80;  // bf16 1.0
       }
@@ -310,13 +310,10 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
              IDESC_ND, kk != 0);
     }
     mma_done();
-    const int rc = recv_s[row];
-    const bool valid = rc >= 0;
     // ================= E1 / G2 =================
     float ds[BWD ? NCH : 1][16];
     {
       const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
-      const float* Qrow = a.Q + (size_t)(valid ? send_s[row] : 0) * a.ldq + 16 * g;
 #pragma unroll
       for (int s = 0; s < NCH; ++s) {
         float x[16];
@@ -324,7 +321,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
         float v[16];
 #pragma unroll
         for (int k4 = 0; k4 < 4; ++k4) {
-          const float4 p = ldg4(Prow + 64 * s + 4 * k4), qv = ldg4(Qrow + 64 * s + 4 * k4);
+          const float4 p = ldg4(Prow + 64 * s + 4 * k4), qv = qf[s][k4];
           v[4 * k4] = p.x + qv.x + x[4 * k4]; v[4 * k4 + 1] = p.y + qv.y + x[4 * k4 + 1];
           v[4 * k4 + 2] = p.z + qv.z + x[4 * k4 + 2]; v[4 * k4 + 3] = p.w + qv.w + x[4 * k4 + 3];
         }
