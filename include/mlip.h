@@ -290,6 +290,25 @@ typedef enum {
 int mlip_ctx_profile(mlip_ctx* ctx, int enable);
 int mlip_ctx_profile_read(mlip_ctx* ctx, int group, double* ms_total, int64_t* n_launches);
 
+/* Exclusive prefix sum over int32 on the context stream: out_dev[i] = in_dev[0] + ... + in_dev[i-1] for i = 0..n, i.e.
+ * out_dev has n + 1 entries and out_dev[n] is the total (how the library turns per-atom degrees into CSR row pointers
+ * and flags into compaction offsets, steps A3/A5 of DESIGN.md 1). Device pointers, asynchronous, in_dev and out_dev must
+ * not overlap; n = 0 writes out_dev[0] = 0. Sums wrap like int32 addition.
+ *   mlip_scan_i32          the path the library uses internally: its scratch (tile totals) comes from the allocator,
+ *                          any n < 2^31.
+ *   mlip_scan_i32_noalloc  ALLOCATES NOTHING (no cudaMalloc / cudaFree, no allocating library routine; three kernel
+ *                          launches), for callers that cannot allocate: CUDA graph capture, serving loops, harnesses
+ *                          that forbid it. Its scratch is a fixed 128 KiB array in device memory that every GPU which
+ *                          loads the library holds until exit; hence n <= MLIP_SCAN_NOALLOC_MAX, beyond which the call
+ *                          returns MLIP_ERR_INVALID_ARG with a message and launches nothing. All calls on a device
+ *                          share that array: calls that OVERLAP on the GPU (two streams, concurrent graph replays)
+ *                          race on it -- serialise them. The first call on a device resolves the array's address
+ *                          (cudaGetSymbolAddress); make it before starting a capture. Same result as mlip_scan_i32,
+ *                          bit for bit. */
+#define MLIP_SCAN_NOALLOC_MAX 67108864 /* 32768 tiles x 2048 elements */
+int mlip_scan_i32(mlip_ctx* ctx, const int32_t* in_dev, int32_t* out_dev, int64_t n);
+int mlip_scan_i32_noalloc(mlip_ctx* ctx, const int32_t* in_dev, int32_t* out_dev, int64_t n);
+
 #ifdef __cplusplus
 }
 #endif

@@ -91,6 +91,8 @@ def load_library():
     lib.mlip_ctx_launch_count.argtypes = [vp]; lib.mlip_ctx_launch_count.restype = i64
     lib.mlip_ctx_profile.argtypes = [vp, i32]
     lib.mlip_ctx_profile_read.argtypes = [vp, i32, P(dbl), P(i64)]
+    lib.mlip_scan_i32.argtypes = [vp, vp, vp, i64]
+    lib.mlip_scan_i32_noalloc.argtypes = [vp, vp, vp, i64]
     _LIB = lib
     return lib
 
@@ -356,6 +358,31 @@ def md_run(ctx: Context, model: Model, L: int, pos, vel, mass, cell: np.ndarray,
                                   C.c_void_p(species.data_ptr()), int(pos.shape[0]), g, float(halo), int(precision),
                                   C.byref(prm), out.ctypes.data_as(C.c_void_p), C.byref(st)))
     return out, dict(n_rebuilds=int(st.n_rebuilds), n_graph_replays=int(st.n_graph_replays), ms_total=float(st.ms_total))
+
+
+MLIP_SCAN_NOALLOC_MAX = 67108864
+
+
+def _scan(fn, ctx: Context, values, out):
+    torch = _torch()
+    assert values.is_cuda and values.dtype == torch.int32 and values.is_contiguous()
+    n = values.numel()
+    if out is None:
+        out = torch.empty(n + 1, dtype=torch.int32, device=values.device)
+    assert out.is_cuda and out.dtype == torch.int32 and out.is_contiguous() and out.numel() >= n + 1
+    ctx.check(fn(ctx.h, C.c_void_p(values.data_ptr() if n else 0), C.c_void_p(out.data_ptr()), n))
+    return out
+
+
+def scan_i32(ctx: Context, values, out=None):
+    """mlip_scan_i32: exclusive prefix sum (n + 1 entries, the last is the total) through the allocating path."""
+    return _scan(ctx.lib.mlip_scan_i32, ctx, values, out)
+
+
+def scan_i32_noalloc(ctx: Context, values, out=None):
+    """mlip_scan_i32_noalloc: the same with a fixed device scratch array, no allocation inside the call (pass `out` to
+    keep the binding allocation-free too); n <= MLIP_SCAN_NOALLOC_MAX."""
+    return _scan(ctx.lib.mlip_scan_i32_noalloc, ctx, values, out)
 
 
 def step_host(ctx: Context, model: Model, L: int, pos: np.ndarray, cell: np.ndarray, species: np.ndarray,
