@@ -4,26 +4,36 @@
 // range contract as in the MLIP_BF16 path). A product a b is evaluated as the six terms a1 b1 + a1 b2 + a2 b1 +
 // a1 b3 + a2 b2 + a3 b1 accumulated in fp32 in tensor memory; what is dropped is below 2^-24 |a b|. Six bf16 MMAs
 // at 8192 flop/clk/SM replace fp32 FMAs at 256 flop/clk/SM. Everything between the contractions (gathers, SiLU,
-// envelope, radial basis) is the fp32 arithmetic of edge_f32.cu, so the two kernels agree to fp32 rounding.
+// envelope, radial basis) is fp32 arithmetic (MUFU ex2 / rcp approximations of 1-2 ulp, as in edge_f32.cu).
 //
-// One persistent CTA per SM (16 warps, all in lock step, thread 0 issues the MMAs) walks over tiles of 128
-// receiver-sorted edges. The split images of W2 [d,d] and of [W1c | W3] [d,32] stay in shared memory.
-//   P0  edge metadata, envelope, radial basis; A0 = [e_hat | t_e] [128,32] split into three operand tiles;
-//       receivers of the tile and the 0/1 selector of the segmented sum
+// One persistent CTA per SM walks over tiles of 128 receiver-sorted edges; the split images of W2 [d,d] and of
+// [W1c | W3] [d,32] stay in shared memory (120 KB), one set of split operand slabs (96 KB) is rewritten per phase.
+//   warps 0..15  epilogue: thread = (edge row, 16 of every 64 channels); TMEM -> registers -> fp32 arithmetic -> three
+//                bf16 terms -> SW128 slabs; publishes per K step (the four warps of a column group = 16 channels)
+//   warp 16      MMA issuer: the whole warp follows the barriers, one ELECTED lane issues (tc::elect_one: a divergent
+//                `if (lane == 0)` costs 60 cycles per MMA in uniformisation loops, measured)
+//   warp 17      segment analysis of the tile: receivers in order of appearance, destinations, 0/1 selector
+// Per tile:
+//   P0  envelope, radial basis; A0 = [e_hat | t_e] [128,32] in three terms. Computed in registers under the last MMAs
+//       of the previous tile and stored as soon as they are done (A0 aliases the slabs).
 //   G1  X = A0 . [W1c | W3]^T                               (K = 32; t_e = 0 without the three-body term)
-//   E1  a = X + P_i + Q_j ; s = SiLU(a) -> split slabs ; the reverse pass keeps SiLU'(a) in registers
-//   G2  Y = s . W2^T            issued per 64-channel K slab as soon as E1 has written it
-//   E2  forward : phi = alpha u_e SiLU(Y + b2) -> split slabs
-//       reverse : pbar = alpha u_e mbar_i SiLU'(p) -> split slabs ; ubar_e = alpha <mbar_i, phi_e>
+//   E1  a = X + P_i + Q_j ; s = SiLU(a) -> slabs ; the reverse pass keeps SiLU'(a) in registers
+//   G2  Y = s . W2^T
+//   E2  forward : phi = alpha u_e SiLU(Y + b2) -> slabs
+//       reverse : pbar = alpha u_e mbar_i SiLU'(p) -> slabs ; ubar_e = alpha <mbar_i, phi_e>
 //   G3  X = pbar . W2           (reverse; the same W2 images read MN-major)
-//   E3  abar = X SiLU'(a) -> global spill (fp32, read back through rev[] by k_gather_rev_f32) and split slabs
+//   E3  abar = X SiLU'(a) -> slabs, and -> global spill (fp32, read back through rev[] by k_gather_rev_f32) AFTER the
+//       last slab is published: the proxy fence of a publication waits for global stores issued before it (measured)
 //   G4  [ebar | tbar] = abar . [W1c | W3]   (N = 32, the G1 images read MN-major)
 //   GS  segmented sum over runs of equal receiver as an MMA with the 0/1 selector (three terms: the selector is
 //       exact): Yseg[channel, r] = slab^T . Sel ; m_i (forward) / Pbar_i (reverse). Tiles with more than 16
 //       receivers sum the slabs in a shared-memory loop.
-//   E4  rbar_e += ubar_e u' + sum_k ebar_k (u' g_k + u g'_k) ; tbar_e -> global
-// Segments that straddle tiles go through per-tile head / tail rows and a fix-up kernel, as in edge_f32.cu. No
-// floating-point atomics: results are bitwise reproducible.
+//   E4  rbar_e += ubar_e u' + sum_k ebar_k (u' g_k + u g'_k) ; tbar_e -> global. E4 and the read-out of Yseg are
+//       deferred until A0 of the next tile is published, so they run under its G1.
+// All row gathers (P_i, Q_j, mbar_i, t_e) and the spill use 256-bit accesses: the rows of a tile are 512 bytes apart,
+// every lane costs an L1 tag cycle per instruction. Segments that straddle tiles go through per-tile head / tail rows
+// and a fix-up kernel, as in edge_f32.cu. The only reduction instruction is the one addition per edge and launch into
+// rbar (order fixed by the launch order): results are bitwise reproducible.
 #include <cuda_bf16.h>
 #include "common.cuh"
 #include "edge.cuh"
@@ -34,12 +44,14 @@
 namespace {
 constexpr int D = 128;            // channels (the only width this kernel is built for)
 constexpr int TE = 128;           // edges per tile = MMA M
-constexpr int NT = 512;           // threads: warp = (lane quarter q = warp % 4, column group g = warp / 4)
+constexpr int N_EPI_WARPS = 16;   // epilogue warp = (lane quarter q = warp % 4, column group g = warp / 4)
+constexpr int MMA_WARP = 16;      // one elected lane issues every MMA
+constexpr int SEG_WARP = 17;      // segment analysis of the tile, ahead of its read-out
+constexpr int NT = 18 * 32;
 constexpr int NCH = D / 64;       // 64-channel operand slabs
 constexpr int K1 = 32;            // K of G1: 16 radial + 16 angle terms
 constexpr int SLAB = TE * 128;    // one [128 x 64] bf16 SW128 slab
 constexpr int MAX_SEG = 16;       // receivers per tile handled by the selector MMA
-constexpr int SEG_WARP = 15;
 
 struct Seg {
   float* dst[MAX_SEG];
@@ -52,21 +64,25 @@ struct SM {  // shared-memory carve-up, byte offsets from the (1024-byte aligned
   static constexpr uint32_t w13 = w2 + 3 * D * D * 2;             // [3][D x 32] bf16, K-major no swizzle
   static constexpr uint32_t A = w13 + 3 * D * K1 * 2;             // [3][NCH] slabs; A0 [3][128 x 32] aliases the start
   static constexpr uint32_t sel = A + 3 * NCH * SLAB;             // [16 x 128] bf16, K-major no swizzle
-  static constexpr uint32_t recv = sel + MAX_SEG * TE * 2;        // int[128]
-  static constexpr uint32_t send = recv + TE * 4;                 // int[128]
-  static constexpr uint32_t u = send + TE * 4;                    // float[128] each: u, du, r, w = alpha u
-  static constexpr uint32_t du = u + TE * 4;
-  static constexpr uint32_t r = du + TE * 4;
-  static constexpr uint32_t w = r + TE * 4;
+  static constexpr uint32_t recv = sel + MAX_SEG * TE * 2;        // int[128] receivers (fallback of the segmented sum)
+  static constexpr uint32_t w = recv + TE * 4;                    // float[128] alpha u_e
   static constexpr uint32_t ubar = w + TE * 4;                    // float[4][128]
   static constexpr uint32_t seg = ubar + 4 * TE * 4;              // Seg
-  static constexpr uint32_t bar = seg + sizeof(Seg);              // one mbarrier
-  static constexpr uint32_t slot = bar + 8;                       // TMEM base address
+  static constexpr uint32_t bar = seg + sizeof(Seg);              // mbarriers
+  static constexpr uint32_t slot = bar + 16 * 8;                  // TMEM base address
   static constexpr uint32_t bytes = slot + 8;
-  static_assert(bytes <= 232448, "shared memory budget of one SM exceeded");
+  static_assert(bytes <= 232448 - 1024, "shared memory budget of one SM exceeded");
 };
 constexpr int TMEM_COLS = 512;    // X [0,128) | Y [128,256) | Yseg [256,272) | D4 [288,320)
+// B_S + 4 s + g: the 16 channels 64 s + 16 g .. + 15 (= one K step of the MMAs) of an operand are written by the four
+// warps of column group g
+enum { B_A0 = 0, B_S = 1 /* .. + 4 NCH */, B_G1 = 1 + 4 * NCH, B_G2, B_G3, B_FIN, B_SEG, B_RO, N_BARS };
+static_assert(N_BARS <= 16, "barrier area");
 
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 // x = h[0] + h[1] + h[2] (bf16 each), two values per register
 __device__ __forceinline__ void split3(float x0, float x1, uint32_t (&h)[3]) {
 #pragma unroll
@@ -91,7 +107,54 @@ __device__ __forceinline__ void store_split16(unsigned char* slab0, uint32_t so0
     *reinterpret_cast<uint4*>(s + so1) = make_uint4(p[i][4], p[i][5], p[i][6], p[i][7]);
   }
 }
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+// SiLU and its derivative in seven instructions: sigma = rcp(1 + ex2(-x log2 e)) with the two MUFU approximations (2 ulp /
+// 1 ulp, flush-to-zero: no denormal fix-up code), y = x sigma, y' = sigma + y (1 - sigma). x -> -inf gives ex2 = inf, sigma = 0.
+__device__ __forceinline__ float sigmoid_x3(float x) {
+  float t, sg;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(t) : "f"(-1.4426950408889634f * x));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(sg) : "f"(1.0f + t));
+  return sg;
+}
+__device__ __forceinline__ float silu_x3(float x) { return x * sigmoid_x3(x); }
+__device__ __forceinline__ void silu_both_x3(float x, float& y, float& dy) {
+  const float sg = sigmoid_x3(x);
+  y = x * sg;
+  dy = fmaf(y, 1.0f - sg, sg);
+}
+// Gaussian radial basis g_k(r) = exp(-gamma (r - k Delta)^2) with the constants hoisted out of the per-edge code
+struct Rbf {
+  float delta, neg_gamma_l2e, two_gamma;
+  __device__ __forceinline__ Rbf(float r_cut, int n_rbf) {
+    delta = r_cut / (float)(n_rbf - 1);
+    const float gamma = 0.5f / (delta * delta);
+    neg_gamma_l2e = -1.4426950408889634f * gamma;
+    two_gamma = 2.0f * gamma;
+  }
+  __device__ __forceinline__ float g(float r, int k) const {
+    const float diff = r - (float)k * delta;
+    float v;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(v) : "f"(neg_gamma_l2e * diff * diff));
+    return v;
+  }
+  // u' g_k + u g_k' = g_k (u' - 2 gamma u (r - k Delta))
+  __device__ __forceinline__ float dug(float r, int k, float u, float du) const {
+    const float diff = r - (float)k * delta;
+    return g(r, k) * fmaf(-two_gamma * u, diff, du);
+  }
+};
+// 8 consecutive floats (one 32-byte sector) per lane in ONE request: the rows of a gather are 512 bytes apart, so every lane
+// costs an L1 tag cycle per instruction, and a 256-bit access halves the instructions
+__device__ __forceinline__ void ldg8(const float* p, float* v) {
+  asm volatile("ld.global.nc.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]), "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7])
+               : "l"(p));
+}
+__device__ __forceinline__ void stg8(float* p, const float* v) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(__float_as_uint(v[0])),
+               "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])), "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])),
+               "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7]))
+               : "memory");
+}
 
 // the six product terms of one K = 16 step, smallest first
 template <class FA, class FB>
@@ -141,25 +204,16 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
   const uint32_t base = (tc::smem_u32(smem_raw) + 1023u) & ~1023u;
   unsigned char* gen = smem_raw + (base - tc::smem_u32(smem_raw));
   int* recv_s = reinterpret_cast<int*>(gen + SM::recv);
-  int* send_s = reinterpret_cast<int*>(gen + SM::send);
-  float* u_s = reinterpret_cast<float*>(gen + SM::u);
-  float* du_s = reinterpret_cast<float*>(gen + SM::du);
-  float* r_s = reinterpret_cast<float*>(gen + SM::r);
   float* w_s = reinterpret_cast<float*>(gen + SM::w);
   float* ubar_s = reinterpret_cast<float*>(gen + SM::ubar);
   Seg& G = *reinterpret_cast<Seg*>(gen + SM::seg);
   uint32_t* slot = reinterpret_cast<uint32_t*>(gen + SM::slot);
   unsigned char* Aop = gen + SM::A;
-  const uint32_t bar = base + SM::bar;
+  auto bar = [&](int i) -> uint32_t { return base + SM::bar + 8u * (uint32_t)i; };
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int q = warp & 3, g = warp >> 2;
-  const int row = q * 32 + lane;
-  const uint32_t tlane = (uint32_t)(q * 32) << 16;
-  const uint32_t so0 = (uint32_t)(row * 128 + (((2 * g) ^ (row & 7)) << 4));
-  const uint32_t so1 = (uint32_t)(row * 128 + (((2 * g + 1) ^ (row & 7)) << 4));
 
-  // ---- one-time setup: resident weight images, barrier, TMEM ----
+  // ---- one-time setup: resident weight images, barriers, TMEM ----
   {
     const uint4* src = reinterpret_cast<const uint4*>(W2x3);
     uint4* dst = reinterpret_cast<uint4*>(gen + SM::w2);
@@ -168,7 +222,13 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
     dst = reinterpret_cast<uint4*>(gen + SM::w13);
     for (int i = tid; i < 3 * D * K1 * 2 / 16; i += NT) dst[i] = __ldg(src + i);
   }
-  if (tid == 0) { tc::mbar_init(bar, 1); tc::fence_mbar_init(); }
+  if (tid == 0) {
+    tc::mbar_init(bar(B_A0), N_EPI_WARPS);
+    for (int s = 0; s < 4 * NCH; ++s) tc::mbar_init(bar(B_S + s), 4);
+    tc::mbar_init(bar(B_G1), 1); tc::mbar_init(bar(B_G2), 1); tc::mbar_init(bar(B_G3), 1); tc::mbar_init(bar(B_FIN), 1);
+    tc::mbar_init(bar(B_SEG), 1); tc::mbar_init(bar(B_RO), N_EPI_WARPS);
+    tc::fence_mbar_init();
+  }
   if (warp == 0) tc::tmem_alloc<TMEM_COLS>(slot);
   tc::fence_proxy_async();
   tc::fence_before_sync();
@@ -176,116 +236,141 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
   tc::fence_after_sync();
   const uint32_t tmem = *slot;
   const uint32_t TX = tmem, TY = tmem + D, TS = tmem + 2 * D, T4 = tmem + 2 * D + 32;
-  uint32_t phase = 0;
-  // all MMAs issued so far are complete and their results visible to every thread
-  auto mma_done = [&]() {
-    if (tid == 0) tc::mma_commit(bar);
-    tc::mbar_wait_warp(bar, phase);
-    phase ^= 1u;
-    tc::fence_after_sync();
-  };
-  // shared-memory operands written by all threads -> visible to the tensor core; tensor-memory reads of all threads done
-  auto operands_ready = [&]() {
-    tc::fence_proxy_async();
-    tc::fence_before_sync();
-    __syncthreads();
-    tc::fence_after_sync();
-  };
-  constexpr uint32_t IDESC_ND = tc::idesc_bf16(128, D, 0, 0);
-  constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);
-  constexpr uint32_t IDESC_N32_BT = tc::idesc_bf16(128, K1, 0, 1);
-  constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);
-  const float4* b2v = reinterpret_cast<const float4*>(a.b2);
 
-  // row metadata of a tile: fetched one tile ahead by every thread of the row
-  int rc_n = -1, sd_n = 0;
-  float r_n = 0.f;
-  auto fetch_meta = [&](int64_t tile) {
-    const int64_t e = tile * TE + row;
-    rc_n = -1; sd_n = 0; r_n = 0.f;
-    if (tile < n_tiles && e < n_edges) { rc_n = __ldg(a.recv + e); sd_n = __ldg(a.send + e); r_n = __ldg(&a.rvec[e].w); }
-  };
-  fetch_meta(blockIdx.x);
-
-  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    const int64_t e0 = tile * TE;
-    const int rc = rc_n, sd = sd_n;
-    const float r_e = r_n;
-    const bool valid = rc >= 0;
-    // sender rows Q_j: random rows out of L2, requested before anything else of the tile is computed
-    float4 qf[NCH][4];
-    {
-      const float* Qrow = a.Q + (size_t)sd * a.ldq + 16 * g;
+  if (blockIdx.x >= n_tiles) {
+    // no tile for this CTA (only possible with E_dyn: the grid is sized from the capacity)
+  } else if (warp == MMA_WARP) {
+    // ====== MMA issuer: the whole warp follows the barriers, one elected lane issues ======
+    constexpr uint32_t IDESC_ND = tc::idesc_bf16(128, D, 0, 0);
+    constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);
+    constexpr uint32_t IDESC_N32_BT = tc::idesc_bf16(128, K1, 0, 1);
+    constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);
+    uint32_t ph_a0 = 0, ph_seg = 0, ph_s = 0;  // parities of the next completion of B_A0 / B_SEG / B_S + i (bit i)
+    auto wait_kstep = [&](int s, int kk) {
+      tc::mbar_wait(bar(B_S + 4 * s + kk), (ph_s >> (4 * s + kk)) & 1u);
+      ph_s ^= 1u << (4 * s + kk);
+      tc::fence_after_sync();
+    };
+    auto a_slab = [&](int i, int s, int kk) {
+      return tc::smem_desc(base + SM::A + i * (NCH * SLAB) + s * SLAB + kk * 32, 16, 1024, tc::LAYOUT_SW128);
+    };
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      // A0 of this tile written by every epilogue warp; G4 / GS of the previous tile are complete (the epilogue waited
+      // for B_FIN before it overwrote the slabs), so X is free
+      tc::mbar_wait(bar(B_A0), ph_a0);
+      ph_a0 ^= 1u;
+      tc::fence_after_sync();
+      if (tc::elect_one()) {
 #pragma unroll
-      for (int s = 0; s < NCH; ++s)
+        for (int kk = 0; kk < K1 / 16; ++kk)
+          mma6(TX, [&](int i) { return tc::smem_desc(base + SM::A + i * (TE * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
+               [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
+               IDESC_ND, kk != 0);
+        tc::mma_commit(bar(B_G1));
+      }
+      __syncwarp();
+      // ---- G2: Y = s . W2^T, one K step (16 channels) at a time ----
 #pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) qf[s][k4] = ldg4(Qrow + 64 * s + 4 * k4);
-    }
-    fetch_meta(tile + gridDim.x);
-    // ================= P0: metadata, features, selector =================
-    // A0 (row, k) -> (row/8)*512 + (k/8)*128 + (row%8)*16 + (k%8)*2, split i at i * 8192; column group g writes k = 8g..8g+7
-    {
-      float f[8];
-      if (g < 2) {
-        float u = 0.f, du = 0.f;
-        if (valid) envelope_f(r_e, a.r_cut, u, du);
-        if (g == 0) {
-          recv_s[row] = rc; send_s[row] = sd; u_s[row] = u; du_s[row] = du; r_s[row] = r_e; w_s[row] = a.alpha * u;
-        }
+      for (int s = 0; s < NCH; ++s) {
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-          float gk = 0.f, dg;
-          if (valid && 8 * g + k < a.n_rbf) rbf_f(r_e, a.r_cut, a.n_rbf, 8 * g + k, gk, dg);
-          f[k] = u * gk;
-        }
-      } else {
-#pragma unroll
-        for (int k = 0; k < 8; ++k) f[k] = 0.f;
-        if (a.t3 && valid) {
-          const float4 v0 = ldg4(a.t3 + (size_t)(e0 + row) * 16 + 8 * (g - 2)), v1 = ldg4(a.t3 + (size_t)(e0 + row) * 16 + 8 * (g - 2) + 4);
-          f[0] = v0.x; f[1] = v0.y; f[2] = v0.z; f[3] = v0.w; f[4] = v1.x; f[5] = v1.y; f[6] = v1.z; f[7] = v1.w;
+        for (int kk = 0; kk < 4; ++kk) {
+          wait_kstep(s, kk);
+          if (tc::elect_one()) {
+            mma6(TY, [&](int i) { return a_slab(i, s, kk); },
+                 [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
+                 IDESC_ND, (s | kk) != 0);
+            if (s == NCH - 1 && kk == 3) tc::mma_commit(bar(B_G2));
+          }
+          __syncwarp();
         }
       }
-      uint32_t p[3][4];
+      if (BWD) {
+        // ---- G3: X = pbar . W2 (the W2 images read MN-major) ----
 #pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        uint32_t h[3];
-        split3(f[2 * t], f[2 * t + 1], h);
-        p[0][t] = h[0]; p[1][t] = h[1]; p[2][t] = h[2];
+        for (int s = 0; s < NCH; ++s) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk) {
+            wait_kstep(s, kk);
+            if (tc::elect_one()) {
+              mma6(TX, [&](int i) { return a_slab(i, s, kk); },
+                   [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128); },
+                   IDESC_ND_BT, (s | kk) != 0);
+              if (s == NCH - 1 && kk == 3) tc::mma_commit(bar(B_G3));
+            }
+            __syncwarp();
+          }
+        }
       }
+      // ---- G4 (reverse): [ebar | tbar] = abar . [W1c | W3]; B = the G1 images [channel][32] read MN-major (N = 32,
+      // K = channel): K-direction 8-channel group stride (LBO) 512 B, N-direction core-matrix stride (SBO) 128 B ----
 #pragma unroll
-      for (int i = 0; i < 3; ++i)
-        *reinterpret_cast<uint4*>(Aop + i * (TE * K1 * 2) + (row >> 3) * 512 + g * 128 + (row & 7) * 16) =
-            make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
+      for (int s = 0; s < NCH; ++s) {
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+          wait_kstep(s, kk);
+          if (BWD && tc::elect_one()) {
+            mma6(T4, [&](int i) { return a_slab(i, s, kk); },
+                 [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + (4 * s + kk) * 1024, 512, 128, tc::LAYOUT_NONE); },
+                 IDESC_N32_BT, (s | kk) != 0);
+          }
+          __syncwarp();
+        }
+      }
+      // ---- GS: segmented sum of the slabs (phi / abar) with the 0/1 selector of the segment warp ----
+      tc::mbar_wait(bar(B_SEG), ph_seg);
+      ph_seg ^= 1u;
+      tc::fence_after_sync();
+      const int R = *reinterpret_cast<volatile int*>(&G.R);
+      if (tc::elect_one()) {
+        if (R <= MAX_SEG) {
+          constexpr int IS[3] = {2, 1, 0};
+#pragma unroll
+          for (int j = 0; j < TE / 16; ++j)
+#pragma unroll
+            for (int t = 0; t < 3; ++t)
+              tc::mma_bf16(TS, tc::smem_desc(base + SM::A + IS[t] * (NCH * SLAB) + j * 2048, SLAB, 1024, tc::LAYOUT_SW128),
+                           tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, (j | t) != 0);
+        }
+        tc::mma_commit(bar(B_FIN));
+      }
+      __syncwarp();
     }
-    if (warp == SEG_WARP) {
-      // receivers of the tile in order of appearance, destination of each segment sum, 0/1 selector
-      int rcv[4];
-      uint32_t fm[4];
+  } else if (warp == SEG_WARP) {
+    // ====== segment analysis: receivers of the tile in order of appearance, destination of each sum, 0/1 selector ======
+    uint32_t ph_ro = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int64_t e0 = tile * TE;
+      int rcv[4], prv[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
-        const int e = lane + 32 * k;
-        const int64_t ge = e0 + e;
-        bool flag = false;
-        rcv[k] = -1;
-        if (ge < n_edges) {
-          rcv[k] = a.recv[ge];
-          flag = e == 0 || a.recv[ge - 1] != rcv[k];
-        }
-        fm[k] = __ballot_sync(0xffffffffu, flag);
+        const int64_t ge = e0 + lane + 32 * k;
+        rcv[k] = ge < n_edges ? __ldg(a.recv + ge) : -1;
+        prv[k] = (ge < n_edges && ge > e0) ? __ldg(a.recv + ge - 1) : -2;
       }
+      uint32_t fm[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) fm[k] = __ballot_sync(0xffffffffu, rcv[k] >= 0 && rcv[k] != prv[k]);
       int rloc[4];
+      int64_t s0[4], s1[4];
       int before = 0;
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         rloc[k] = before + __popc(fm[k] & (0xffffffffu >> (31 - lane))) - 1;
-        if (((fm[k] >> lane) & 1u) && rloc[k] < MAX_SEG) {
-          const int64_t s0 = a.rowptr[rcv[k]], s1 = a.rowptr[rcv[k] + 1];
-          G.dst[rloc[k]] = (s0 >= e0 && s1 <= e0 + TE) ? (BWD ? a.Pbar : a.m) + (size_t)rcv[k] * D
-                                                       : (s0 < e0 ? a.head : a.tail) + (size_t)tile * D;
-        }
+        const bool first = ((fm[k] >> lane) & 1u) && rloc[k] < MAX_SEG;
+        s0[k] = first ? __ldg(a.rowptr + rcv[k]) : 0;
+        s1[k] = first ? __ldg(a.rowptr + rcv[k] + 1) : -1;   // s1 < 0: not the first edge of a receiver
         before += __popc(fm[k]);
       }
+      // the selector and the segment table are free once every epilogue warp has read out the previous tile
+      if (tile != blockIdx.x) {
+        tc::mbar_wait_warp(bar(B_RO), ph_ro);
+        ph_ro ^= 1u;
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (s1[k] >= 0)
+          G.dst[rloc[k]] = (s0[k] >= e0 && s1[k] <= e0 + TE) ? (BWD ? a.Pbar : a.m) + (size_t)rcv[k] * D
+                                                            : (s0[k] < e0 ? a.head : a.tail) + (size_t)tile * D;
       if (lane == 0) G.R = before;
       uint4* z = reinterpret_cast<uint4*>(gen + SM::sel);
 #pragma unroll
@@ -299,178 +384,235 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
           *reinterpret_cast<unsigned short*>(gen + SM::sel + (rloc[k] >> 3) * 2048 + (e >> 3) * 128 + (rloc[k] & 7) * 16 +
                                              (e & 7) * 2) = (unsigned short)0x3F80;  // bf16 1.0
       }
+      tc::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_SEG));
     }
-    operands_ready();
-    // ================= G1 =================
-    if (tid == 0) {
+  } else {
+    // =========================== epilogue warps ===========================
+    const int q = warp & 3, g = warp >> 2;
+    const int row = q * 32 + lane;
+    const uint32_t tlane = (uint32_t)(q * 32) << 16;
+    const uint32_t so0 = (uint32_t)(row * 128 + (((2 * g) ^ (row & 7)) << 4));
+    const uint32_t so1 = (uint32_t)(row * 128 + (((2 * g + 1) ^ (row & 7)) << 4));
+    const float4* b2v = reinterpret_cast<const float4*>(a.b2);
+    const Rbf rbf(a.r_cut, a.n_rbf);
+    uint32_t ph = 0;  // bit i: parity of the next completion of barrier i
+    auto wait_bar = [&](int i) {
+      tc::mbar_wait_warp(bar(i), (ph >> i) & 1u);
+      ph ^= 1u << i;
+      tc::fence_after_sync();
+    };
+    // this warp's part of an operand is written (shared memory -> async proxy) and its tensor-memory reads are done
+    auto publish = [&](int i) {
+      tc::fence_proxy_async();
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(i));
+    };
+    // row metadata of a tile: fetched one tile ahead by every thread of the row
+    int rc_n = -1, sd_n = 0;
+    float r_n = 0.f;
+    auto fetch_meta = [&](int64_t tile) {
+      const int64_t e = tile * TE + row;
+      rc_n = -1; sd_n = 0; r_n = 0.f;
+      if (tile < n_tiles && e < n_edges) { rc_n = __ldg(a.recv + e); sd_n = __ldg(a.send + e); r_n = __ldg(&a.rvec[e].w); }
+    };
+    // P0 of a tile: features computed in registers (under the last MMAs of the previous tile), stored once the operand
+    // region is free. A0 (row, k) -> (row/8)*512 + (k/8)*128 + (row%8)*16 + (k%8)*2, split i at i * 8192; column group g
+    // writes k = 8g..8g+7
+    struct Feat { uint32_t p[3][4]; float u, du; };
+    auto features = [&](int64_t tile, int rc, float r_e, Feat& o) {
+      float f[8];
+      o.u = 0.f; o.du = 0.f;
+      if (g < 2) {
+        if (rc >= 0) envelope_f(r_e, a.r_cut, o.u, o.du);
 #pragma unroll
-      for (int kk = 0; kk < K1 / 16; ++kk)
-        mma6(TX, [&](int i) { return tc::smem_desc(base + SM::A + i * (TE * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
-             [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
-             IDESC_ND, kk != 0);
-    }
-    mma_done();
-    // ================= E1 / G2 =================
-    float ds[BWD ? NCH : 1][16];
-    {
-      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
+        for (int k = 0; k < 8; ++k) f[k] = 8 * g + k < a.n_rbf ? o.u * rbf.g(r_e, 8 * g + k) : 0.f;   // u = 0 beyond the edge list
+      } else {
 #pragma unroll
-      for (int s = 0; s < NCH; ++s) {
-        float x[16];
-        tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), x);
-        float v[16];
-#pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-          const float4 p = ldg4(Prow + 64 * s + 4 * k4), qv = qf[s][k4];
-          v[4 * k4] = p.x + qv.x + x[4 * k4]; v[4 * k4 + 1] = p.y + qv.y + x[4 * k4 + 1];
-          v[4 * k4 + 2] = p.z + qv.z + x[4 * k4 + 2]; v[4 * k4 + 3] = p.w + qv.w + x[4 * k4 + 3];
-        }
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-          float sv, dv;
-          silu_both_f(v[k], sv, dv);
-          v[k] = valid ? sv : 0.f;
-          if (BWD) ds[s][k] = valid ? dv : 0.f;
-        }
-        store_split16(Aop + s * SLAB, so0, so1, v);
-        operands_ready();
-        if (tid == 0) {
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)
-            mma6(TY, [&](int i) { return tc::smem_desc(base + SM::A + i * (NCH * SLAB) + s * SLAB + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
-                 [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
-                 IDESC_ND, (s | kk) != 0);
-        }
+        for (int k = 0; k < 8; ++k) f[k] = 0.f;
+        if (a.t3 && rc >= 0) ldg8(a.t3 + (size_t)(tile * TE + row) * 16 + 8 * (g - 2), f);
       }
-    }
-    mma_done();
-    // ================= E2 =================
-    if (!BWD) {
-      const float wr = w_s[row];
 #pragma unroll
-      for (int s = 0; s < NCH; ++s) {
-        float y[16];
-        tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
-#pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-          const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
-          y[4 * k4] = wr * silu_f(y[4 * k4] + b.x); y[4 * k4 + 1] = wr * silu_f(y[4 * k4 + 1] + b.y);
-          y[4 * k4 + 2] = wr * silu_f(y[4 * k4 + 2] + b.z); y[4 * k4 + 3] = wr * silu_f(y[4 * k4 + 3] + b.w);
-        }
-        store_split16(Aop + s * SLAB, so0, so1, y);
+      for (int t = 0; t < 4; ++t) {
+        uint32_t h[3];
+        split3(f[2 * t], f[2 * t + 1], h);
+        o.p[0][t] = h[0]; o.p[1][t] = h[1]; o.p[2][t] = h[2];
       }
-      operands_ready();
-    } else {
-      const float au = w_s[row];
-      const float* Mrow = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
-      float up = 0.f;
+    };
+    auto store_a0 = [&](const Feat& o, int rc) {
+      if (g == 0) { recv_s[row] = rc; w_s[row] = a.alpha * o.u; }
 #pragma unroll
-      for (int s = 0; s < NCH; ++s) {
-        float y[16];
-        tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
-#pragma unroll
-        for (int k4 = 0; k4 < 4; ++k4) {
-          const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
-          float4 mb = ldg4(Mrow + 64 * s + 4 * k4);
-          if (!valid) mb = make_float4(0.f, 0.f, 0.f, 0.f);
-          float phi, dphi;
-          silu_both_f(y[4 * k4] + b.x, phi, dphi); up = fmaf(mb.x, phi, up); y[4 * k4] = au * mb.x * dphi;
-          silu_both_f(y[4 * k4 + 1] + b.y, phi, dphi); up = fmaf(mb.y, phi, up); y[4 * k4 + 1] = au * mb.y * dphi;
-          silu_both_f(y[4 * k4 + 2] + b.z, phi, dphi); up = fmaf(mb.z, phi, up); y[4 * k4 + 2] = au * mb.z * dphi;
-          silu_both_f(y[4 * k4 + 3] + b.w, phi, dphi); up = fmaf(mb.w, phi, up); y[4 * k4 + 3] = au * mb.w * dphi;
-        }
-        store_split16(Aop + s * SLAB, so0, so1, y);
-        if (s == NCH - 1) ubar_s[g * TE + row] = up;
-        operands_ready();
-        // ================= G3: X = pbar . W2 (W2 images read MN-major) =================
-        if (tid == 0) {
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)
-            mma6(TX, [&](int i) { return tc::smem_desc(base + SM::A + i * (NCH * SLAB) + s * SLAB + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
-                 [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128); },
-                 IDESC_ND_BT, (s | kk) != 0);
-        }
-      }
-      mma_done();
-      // ================= E3 / G4 =================
-#pragma unroll
-      for (int s = 0; s < NCH; ++s) {
-        float x[16];
-        tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), x);
-#pragma unroll
-        for (int k = 0; k < 16; ++k) x[k] *= ds[s][k];
-        if (valid) {
-          float4* dst = reinterpret_cast<float4*>(a.abar + (size_t)(e0 + row) * D + 64 * s + 16 * g);
-#pragma unroll
-          for (int k4 = 0; k4 < 4; ++k4) dst[k4] = make_float4(x[4 * k4], x[4 * k4 + 1], x[4 * k4 + 2], x[4 * k4 + 3]);
-        }
-        store_split16(Aop + s * SLAB, so0, so1, x);
-        operands_ready();
-        if (tid == 0) {
-          // B = the G1 images [channel][32] read MN-major (N = 32, K = channel): K-direction 8-channel group stride
-          // (LBO) 512 B, N-direction core-matrix stride (SBO) 128 B
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)
-            mma6(T4, [&](int i) { return tc::smem_desc(base + SM::A + i * (NCH * SLAB) + s * SLAB + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
-                 [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + (4 * s + kk) * 1024, 512, 128, tc::LAYOUT_NONE); },
-                 IDESC_N32_BT, (s | kk) != 0);
-        }
-      }
-    }
-    // ================= GS: segmented sum of the slabs =================
-    const int R = G.R;
-    if (R <= MAX_SEG) {
-      if (tid == 0) {
-        constexpr int IS[3] = {2, 1, 0};
-#pragma unroll
-        for (int j = 0; j < TE / 16; ++j)
-#pragma unroll
-          for (int t = 0; t < 3; ++t)
-            tc::mma_bf16(TS, tc::smem_desc(base + SM::A + IS[t] * (NCH * SLAB) + j * 2048, SLAB, 1024, tc::LAYOUT_SW128),
-                         tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, (j | t) != 0);
-      }
-      mma_done();
-      if (g == 0) {
+      for (int i = 0; i < 3; ++i)
+        *reinterpret_cast<uint4*>(Aop + i * (TE * K1 * 2) + (row >> 3) * 512 + g * 128 + (row & 7) * 16) =
+            make_uint4(o.p[i][0], o.p[i][1], o.p[i][2], o.p[i][3]);
+      publish(B_A0);
+    };
+    // Read-out of a finished tile (segment sums out of Yseg, E4), deferred until A0 of the NEXT tile is published so that
+    // it runs under that tile's G1 instead of ending every tile with idle tensor cores.
+    auto read_out = [&](int64_t tile, bool valid, float r_e, float u, float du) {
+      const int64_t e0 = tile * TE;
+      const int R = G.R;
+      if (R <= MAX_SEG && g == 0) {
         float acc[16];
         tc::tmem_ld16(TS + tlane, acc);
 #pragma unroll
         for (int r = 0; r < MAX_SEG; ++r)
           if (r < R) G.dst[r][row] = acc[r];
       }
-    } else {
-      if (BWD) mma_done();  // G4
-      if (tid < D) segmented_store_x3(Aop, recv_s, a.rowptr, e0, tile, BWD ? a.Pbar : a.m, a.head, a.tail, tid);
-    }
-    if (BWD && g == 1) {
-      // ================= E4 =================
-      float eb[16], tb[16];
-      tc::tmem_ld16(T4 + tlane, eb);
-      tc::tmem_ld16(T4 + tlane + 16u, tb);
-      if (valid) {
-        if (a.tbar) {
-          float4* dst = reinterpret_cast<float4*>(a.tbar + (size_t)(e0 + row) * 16);
+      if (BWD && g == 1) {
+        // E4; one addition per edge and launch: a fire-and-forget reduction is deterministic and has no load latency
+        float eb[16];
+        tc::tmem_ld16(T4 + tlane, eb);
+        if (valid) {
+          float part = 0.f;
 #pragma unroll
-          for (int k4 = 0; k4 < 4; ++k4) dst[k4] = make_float4(tb[4 * k4], tb[4 * k4 + 1], tb[4 * k4 + 2], tb[4 * k4 + 3]);
+          for (int k = 0; k < 16; ++k) {
+            if (k < a.n_rbf) part = fmaf(eb[k], rbf.dug(r_e, k, u, du), part);
+          }
+          const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
+          atomicAdd(a.rbar + e0 + row, fmaf(ubar, du, part));
         }
-        const float r = r_s[row], u = u_s[row], du = du_s[row];
-        float part = 0.f;
+      }
+      if (BWD && g == 2 && a.tbar) {
+        float tb[16];
+        tc::tmem_ld16(T4 + tlane + 16u, tb);
+        if (valid) {
+          stg8(a.tbar + (size_t)(e0 + row) * 16, tb);
+          stg8(a.tbar + (size_t)(e0 + row) * 16 + 8, tb + 8);
+        }
+      }
+      // the segment table, Yseg, D4 and the u-bar partials of the tile are read: the segment warp, the next GS / G4 and
+      // the next E2 may overwrite them
+      tc::fence_before_sync();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_RO));
+    };
+
+    fetch_meta(blockIdx.x);
+    float u_e, du_e;
+    {
+      Feat ft;
+      features(blockIdx.x, rc_n, r_n, ft);
+      store_a0(ft, rc_n);
+      u_e = ft.u; du_e = ft.du;
+    }
+    bool ro_valid = false;
+    float ro_r = 0.f, ro_u = 0.f, ro_du = 0.f;
+
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int64_t e0 = tile * TE;
+      const int rc = rc_n, sd = sd_n;
+      const float r_e = r_n;
+      const bool valid = rc >= 0;
+      // sender rows Q_j: random rows out of L2; the first slab is requested before anything else of the tile is computed
+      const float* Qrow = a.Q + (size_t)sd * a.ldq + 16 * g;
+      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
+      float qf[16], pf[16];
+      ldg8(Qrow, qf); ldg8(Qrow + 8, qf + 8);
+      ldg8(Prow, pf); ldg8(Prow + 8, pf + 8);
+      fetch_meta(tile + gridDim.x);
+      if (tile != blockIdx.x) read_out(tile - gridDim.x, ro_valid, ro_r, ro_u, ro_du);
+      ro_valid = valid; ro_r = r_e; ro_u = u_e; ro_du = du_e;
+      // ================= E1 =================
+      float ds[BWD ? NCH : 1][16];
+      wait_bar(B_G1);
+#pragma unroll
+      for (int s = 0; s < NCH; ++s) {
+        float v[16];
+        tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] += pf[k] + qf[k];
+        if (s + 1 < NCH) {
+          ldg8(Prow + 64 * (s + 1), pf); ldg8(Prow + 64 * (s + 1) + 8, pf + 8);
+          ldg8(Qrow + 64 * (s + 1), qf); ldg8(Qrow + 64 * (s + 1) + 8, qf + 8);
+        }
 #pragma unroll
         for (int k = 0; k < 16; ++k) {
-          if (k < a.n_rbf) {
-            float gk, dg;
-            rbf_f(r, a.r_cut, a.n_rbf, k, gk, dg);
-            part = fmaf(eb[k], fmaf(du, gk, u * dg), part);
-          }
+          if (BWD) silu_both_x3(v[k], v[k], ds[s][k]);
+          else v[k] = silu_x3(v[k]);
         }
-        const float ubar = a.alpha * ((ubar_s[row] + ubar_s[TE + row]) + (ubar_s[2 * TE + row] + ubar_s[3 * TE + row]));
-        a.rbar[e0 + row] += fmaf(ubar, du, part);
+        store_split16(Aop + s * SLAB, so0, so1, v);
+        publish(B_S + 4 * s + g);
       }
+      // ================= E2 =================
+      wait_bar(B_G2);
+      if (!BWD) {
+        const float wr = w_s[row];
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          float y[16];
+          tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
+#pragma unroll
+          for (int k4 = 0; k4 < 4; ++k4) {
+            const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
+            y[4 * k4] = wr * silu_x3(y[4 * k4] + b.x); y[4 * k4 + 1] = wr * silu_x3(y[4 * k4 + 1] + b.y);
+            y[4 * k4 + 2] = wr * silu_x3(y[4 * k4 + 2] + b.z); y[4 * k4 + 3] = wr * silu_x3(y[4 * k4 + 3] + b.w);
+          }
+          store_split16(Aop + s * SLAB, so0, so1, y);
+          publish(B_S + 4 * s + g);
+        }
+      } else {
+        const float au = w_s[row];
+        const float* Mrow = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        float up = 0.f;
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          float y[16], mb[16];
+          ldg8(Mrow + 64 * s, mb); ldg8(Mrow + 64 * s + 8, mb + 8);
+          tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
+#pragma unroll
+          for (int k4 = 0; k4 < 4; ++k4) {
+            const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
+            const float bb[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              float phi, dphi;
+              silu_both_x3(y[4 * k4 + j] + bb[j], phi, dphi);
+              up = fmaf(mb[4 * k4 + j], phi, up);
+              y[4 * k4 + j] = au * mb[4 * k4 + j] * dphi;
+            }
+          }
+          store_split16(Aop + s * SLAB, so0, so1, y);
+          if (s == NCH - 1) ubar_s[g * TE + row] = up;
+          publish(B_S + 4 * s + g);
+        }
+        // ================= E3 =================
+        wait_bar(B_G3);
+#pragma unroll
+        for (int s = 0; s < NCH; ++s) {
+          float x[16];
+          tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), x);
+#pragma unroll
+          for (int k = 0; k < 16; ++k) ds[s][k] *= x[k];   // abar, kept for the spill below
+          store_split16(Aop + s * SLAB, so0, so1, ds[s]);
+          publish(B_S + 4 * s + g);
+        }
+        // The fp32 spill goes out after the last slab is published: the fences of publish() wait for global stores issued
+        // before them (measured: 3.4 k cycles per slab). It drains under the wait for G4 / GS.
+        if (valid) {
+          float* dst = a.abar + (size_t)(e0 + row) * D + 16 * g;
+#pragma unroll
+          for (int s = 0; s < NCH; ++s) { stg8(dst + 64 * s, ds[s]); stg8(dst + 64 * s + 8, ds[s] + 8); }
+        }
+      }
+      // ================= P0 of the next tile under G4 / GS of this one =================
+      const int64_t next = tile + gridDim.x;
+      Feat ft;
+      if (next < n_tiles) features(next, rc_n, r_n, ft);
+      wait_bar(B_FIN);
+      wait_bar(B_SEG);
+      if (G.R > MAX_SEG) {  // rare: more receivers than the selector holds, sum the slabs before they are overwritten
+        if (warp < D / 32)
+          segmented_store_x3(Aop, recv_s, a.rowptr, e0, tile, BWD ? a.Pbar : a.m, a.head, a.tail, warp * 32 + lane);
+        named_bar_sync(1, N_EPI_WARPS * 32);
+      }
+      if (next < n_tiles) { store_a0(ft, rc_n); u_e = ft.u; du_e = ft.du; }
     }
-    // the next tile overwrites the metadata, the selector and the operand slabs, and its G1 region X
-    tc::fence_before_sync();
-    __syncthreads();
-    tc::fence_after_sync();
+    read_out(n_tiles - 1 - (n_tiles - 1 - blockIdx.x) % gridDim.x, ro_valid, ro_r, ro_u, ro_du);
   }
+  tc::fence_before_sync();
   __syncthreads();
   if (warp == 0) tc::tmem_dealloc<TMEM_COLS>(tmem);
 }

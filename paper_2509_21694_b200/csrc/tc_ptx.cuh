@@ -158,6 +158,15 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 
+// One lane of a fully active warp (the lowest): the issue path of tcgen05.mma. Unlike `lane == 0`, the compiler keeps the
+// operands of the region in uniform registers and emits the MMAs back to back (a divergent `if (lane == 0)` wraps every
+// UTCHMMA in an ELECT / BRA.U.ANY loop: about 60 cycles per MMA, measured).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 // ---- copies -----------------------------------------------------------------------------------
 __device__ __forceinline__ void cp_async16(uint32_t saddr, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(saddr), "l"(gmem) : "memory");
