@@ -285,7 +285,8 @@ typedef enum {
   MLIP_GROUP_READOUT_FORCES = 4, /* embedding, readout, energy sum, force assembly (A9, A11) */
   MLIP_GROUP_GRAPH = 5,          /* mlip_build_graph (A1-A4) */
   MLIP_GROUP_PARTITION = 6,      /* mlip_partition / mlip_partition_grid (A5) */
-  MLIP_GROUP_COUNT = 7
+  MLIP_GROUP_THREE_BODY = 7,     /* gates, triplet sums and their adjoints of the three-body variant (O7) */
+  MLIP_GROUP_COUNT = 8
 } mlip_group;
 int mlip_ctx_profile(mlip_ctx* ctx, int enable);
 int mlip_ctx_profile_read(mlip_ctx* ctx, int group, double* ms_total, int64_t* n_launches);

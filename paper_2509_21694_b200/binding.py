@@ -14,7 +14,7 @@ import numpy as np
 MLIP_FP32 = 0
 MLIP_BF16 = 1
 MLIP_MAGIC = 0x50494C4D
-GROUPS = ("edge_fwd", "edge_bwd", "gather_rev", "node_gemm", "readout_forces", "graph", "partition")
+GROUPS = ("edge_fwd", "edge_bwd", "gather_rev", "node_gemm", "readout_forces", "graph", "partition", "three_body")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None

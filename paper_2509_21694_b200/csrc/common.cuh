@@ -40,7 +40,8 @@ enum {
   MLIP_PROF_READOUT_FORCES = 4,  // embedding, readout, energy sum, force assembly
   MLIP_PROF_GRAPH = 5,      // mlip_build_graph
   MLIP_PROF_PARTITION = 6,  // mlip_partition*
-  MLIP_PROF_COUNT = 7
+  MLIP_PROF_THREE_BODY = 7, // gate, triplet and their adjoint kernels of the three-body variant
+  MLIP_PROF_COUNT = 8
 };
 
 struct mlip_ctx {

@@ -302,11 +302,13 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   const bool tb = (M->h.flags & MLIP_FLAG_THREE_BODY) != 0 && L > 0;
   const float r3 = M->h.r_cut3;
   std::vector<float*> zg(L, nullptr);
-  float *t3 = nullptr, *tbar3 = nullptr;
+  std::vector<float*> t3(L, nullptr);   // angle terms t_e of every layer, kept for the reverse pass (64 B per edge-layer)
+  float* tbar3 = nullptr;
   float4* gvec = nullptr;
   if (tb) {
     for (int l = 0; l < L; ++l) W_ALLOC(zg[l], float, n * 16);
-    W_ALLOC(t3, float, (E + 1) * 16); W_ALLOC(tbar3, float, (E + 1) * 16); W_ALLOC(gvec, float4, E + 1);
+    for (int l = 0; l < L; ++l) W_ALLOC(t3[l], float, (E + 1) * 16);
+    W_ALLOC(tbar3, float, (E + 1) * 16); W_ALLOC(gvec, float4, E + 1);
     cudaMemsetAsync(gvec, 0, sizeof(float4) * (E + 1), st);
   }
   float* mbar = m;           // m is dead after the forward pass
@@ -367,10 +369,10 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     set_layer(l);
     ea.m = m; ea.E = e_recv(l); ea.n = nr; ea.E_dyn = g.dyn ? g.rowptr + nr : nullptr;
     if (tb) {
-      ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
+      ProfScope p(ctx, MLIP_PROF_THREE_BODY);
       W_TRY(mlip_gate_forward(ctx, ns, d, h[l], W.G3, W.g3, zg[l]));
-      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3));
-      ea.t3 = t3; ea.W3 = W.W3;
+      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3[l]));
+      ea.t3 = t3[l]; ea.W3 = W.W3;
     }
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_FWD);
@@ -450,18 +452,16 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     ea.E = Er; ea.n = nr; ea.node_adjoint = bf ? node_adjoint : true;
     ea.E_dyn = g.dyn ? g.rowptr + nr : nullptr;
     ea.mbar = mbar; ea.mbar_h = mbar_h; ea.abar = abar; ea.abar_h = abar_h; ea.Pbar = Pbar; ea.rbar = rbar;
-    if (tb) {  // the angle terms are recomputed like every other edge activation
-      ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
-      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3));
-      ea.t3 = t3; ea.W3 = W.W3; ea.tbar = tbar3;
+    if (tb) {  // the angle terms of the forward pass were kept (16 floats per edge-layer; the d-wide activations are recomputed)
+      ea.t3 = t3[l]; ea.W3 = W.W3; ea.tbar = tbar3;
     }
     {
       ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
       W_TRY(bf ? mlip_edge_backward_tc(ctx, d, ea) : mlip_edge_backward_f32(ctx, d, ea));
     }
-    float* zeta = t3;  // the angle terms are dead after the edge kernel: their buffer takes the per-edge gate adjoints
+    float* zeta = tb ? t3[l] : nullptr;  // the angle terms are dead after the edge kernel: their buffer takes the per-edge gate adjoints
     if (tb) {
-      ProfScope p(ctx, MLIP_PROF_EDGE_BWD);
+      ProfScope p(ctx, MLIP_PROF_THREE_BODY);
       W_TRY(mlip_triplet_backward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], tbar3, rbar, gvec, zeta));
     }
     if (!node_adjoint) continue;
@@ -477,7 +477,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     a.n = ns; a.N = d;
     W_TRY(gemm(ctx, a));
     if (tb) {  // adjoint of the gates of the senders (third atoms), through the reverse-edge index like Qbar
-      ProfScope p(ctx, MLIP_PROF_GATHER_REV);
+      ProfScope p(ctx, MLIP_PROF_THREE_BODY);
       W_TRY(mlip_gate_backward(ctx, ns, Er, ea.E_dyn, d, g.rowptr, g.rev, zeta, zg[l], W.G3, hbar));
     }
   }
