@@ -47,7 +47,9 @@ typedef enum {
 } mlip_status;
 
 /* Arithmetic of the contractions.
- *   MLIP_FP32  fp32 CUDA-core FMA everywhere.
+ *   MLIP_FP32  fp32 arithmetic everywhere (north_star tolerances 1e-5 / 1e-4). Contractions by CUDA-core FMA, except the fused
+ *              edge kernels at d = 128: tcgen05 with every fp32 operand split exactly into three bf16 terms, six MMAs per
+ *              product, fp32 accumulation (24 significant bits, fp32 range).
  *   MLIP_BF16  16-bit tensor-core operands with fp32 accumulation (tcgen05, accumulators in TMEM). The name follows
  *              BASELINE.json ("bf16 GEMM inputs"); what runs is IEEE HALF (f16) operands in every contraction -- same
  *              tensor-core rate and bytes as bf16, three more mantissa bits (force RMS error of the unpruned L = 15
@@ -171,7 +173,7 @@ void mlip_part_destroy(mlip_part* p);
  * sub-domains of the gradient of that sub-domain's root energy w.r.t. ALL of its atoms
  * (reading R1). part == NULL evaluates the whole box as one domain.
  * Sub-domains are evaluated one after another on the context stream.
- *   precision       MLIP_FP32 (fp32 CUDA-core contractions) or MLIP_BF16 (16-bit tensor-core contractions
+ *   precision       MLIP_FP32 (fp32 contractions) or MLIP_BF16 (16-bit tensor-core contractions
  *                   with fp32 accumulation, see the enum; requires d = 256 or 128)
  *   energy_dev      [1] float64, device
  *   forces_dev      [n_atoms,3] float32, device, caller's atom numbering (eV/Angstrom)
