@@ -425,7 +425,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_edge_tc(EdgeArgs a, int64_t n_
     }
   } else if (warp == WARP_MMA) {
     // =========================== MMA issuer (one thread) ===========================
-    if (tc::elect_one()) {  // not `lane == 0`: see tc::elect_one
+    if (lane == 0) {
       constexpr uint32_t IDESC_ND = tc::idesc_f16(128, D, 0, 0);     // K-major A and B, N = D
       constexpr uint32_t IDESC_ND_BT = tc::idesc_f16(128, D, 0, 1);  // B read MN-major
       // the last K slab of G2 / G3 is issued as two N halves with a commit each, so that the epilogue of

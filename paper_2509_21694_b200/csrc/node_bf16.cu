@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
     }
   } else if (warp == WARP_B) {
     // ======================= weight slab producer (one thread) =======================
-    if (tc::elect_one()) {
+    if (lane == 0) {
       const unsigned char* img = reinterpret_cast<const unsigned char*>(a.B);
       if (RES) {
         tc::mbar_expect_tx(w_full, (uint32_t)nk * SM::b_bytes);
@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(N_THREADS, 1) k_gemm_bf16(GemmArgs a, int n_ti
     }
   } else if (warp == WARP_MMA) {
     // ======================= MMA issuer (one thread) =======================
-    if (tc::elect_one()) {  // not `lane == 0`: see tc::elect_one
+    if (lane == 0) {
       constexpr uint32_t IDESC = tc::idesc_op(128, N, 0, 0);
       int g = 0;
       if (RES) tc::mbar_wait(w_full, 0u);

@@ -160,7 +160,9 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 
 // One lane of a fully active warp (the lowest): the issue path of tcgen05.mma. Unlike `lane == 0`, the compiler keeps the
 // operands of the region in uniform registers and emits the MMAs back to back (a divergent `if (lane == 0)` wraps every
-// UTCHMMA in an ELECT / BRA.U.ANY loop: about 60 cycles per MMA, measured).
+// UTCHMMA in an ELECT / BRA.U.ANY loop: about 60 cycles per MMA, measured in edge_x3.cu, whose issue region sits inside a
+// whole-warp loop). edge_tc.cu and node_bf16.cu keep `lane == 0` around their whole single-thread role: there the compiler
+// emits the MMAs back to back already, and elect_one measured 1 % SLOWER (A/B on one box, config 4).
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
