@@ -8,8 +8,9 @@
 //
 // One persistent CTA per SM walks over tiles of 128 receiver-sorted edges; the split images of W2 [d,d] and of
 // [W1c | W3] [d,32] stay in shared memory (120 KB), one set of split operand slabs (96 KB) is rewritten per phase.
-//   warps 0..15  epilogue: thread = (edge row, 16 of every 64 channels); TMEM -> registers -> fp32 arithmetic -> three
-//                bf16 terms -> SW128 slabs; publishes per K step (the four warps of a column group = 16 channels)
+//   warps 0..15  epilogue: thread = (edge row, 8 channels per step, 4 steps); TMEM -> registers -> fp32 arithmetic -> three
+//                bf16 terms -> SW128 slabs. A step completes TWO K steps of the MMAs (16 channels each, 8 warps each), so
+//                the tensor core trails the epilogue by a quarter of a phase instead of half of it
 //   warp 16      MMA issuer: the whole warp follows the barriers, one ELECTED lane issues (tc::elect_one: a divergent
 //                `if (lane == 0)` costs 60 cycles per MMA in uniformisation loops, measured)
 //   warp 17      segment analysis of the tile: receivers in order of appearance, destinations, 0/1 selector
@@ -74,8 +75,8 @@ struct SM {  // shared-memory carve-up, byte offsets from the (1024-byte aligned
   static_assert(bytes <= 232448 - 1024, "shared memory budget of one SM exceeded");
 };
 constexpr int TMEM_COLS = 512;    // X [0,128) | Y [128,256) | Yseg [256,272) | D4 [288,320)
-// B_S + 4 s + g: the 16 channels 64 s + 16 g .. + 15 (= one K step of the MMAs) of an operand are written by the four
-// warps of column group g
+// B_S + k: the 16 channels 16 k .. 16 k + 15 (= K step k of the MMAs, slab k / 4) of an operand are written by the eight
+// warps of column groups 2 (k % 2), 2 (k % 2) + 1 in step k / 2
 enum { B_A0 = 0, B_S = 1 /* .. + 4 NCH */, B_G1 = 1 + 4 * NCH, B_G2, B_G3, B_FIN, B_SEG, B_RO, N_BARS };
 static_assert(N_BARS <= 16, "barrier area");
 
@@ -91,21 +92,40 @@ __device__ __forceinline__ void split3(float x0, float x1, uint32_t (&h)[3]) {
     if (i < 2) { x0 -= tc::bf16_lo(h[i]); x1 -= tc::bf16_hi(h[i]); }
   }
 }
-// 16 consecutive channels of one row -> the two 16-byte chunks of the three split slabs
-__device__ __forceinline__ void store_split16(unsigned char* slab0, uint32_t so0, uint32_t so1, const float (&v)[16]) {
-  uint32_t p[3][8];
+constexpr int CPS = 8;            // channels per thread and step (see kst() below). Measured on config 5, reverse kernel: CPS = 16
+                                  // (one K step per column group) 28.0 ms, CPS = 8 25.4 ms, CPS = 4 31.6 ms (twice the loads, stores and fences)
+// N (4 or 8) consecutive channels of one row -> 2 N bytes in each of the three split slabs
+template <int N>
+__device__ __forceinline__ void store_split(unsigned char* A, uint32_t off, const float (&v)[N]) {
+  uint32_t p[3][N / 2];
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {
+  for (int j = 0; j < N / 2; ++j) {
     uint32_t h[3];
     split3(v[2 * j], v[2 * j + 1], h);
     p[0][j] = h[0]; p[1][j] = h[1]; p[2][j] = h[2];
   }
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    unsigned char* s = slab0 + i * (NCH * SLAB);
-    *reinterpret_cast<uint4*>(s + so0) = make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
-    *reinterpret_cast<uint4*>(s + so1) = make_uint4(p[i][4], p[i][5], p[i][6], p[i][7]);
+    if constexpr (N == 8) *reinterpret_cast<uint4*>(A + i * (NCH * SLAB) + off) = make_uint4(p[i][0], p[i][1], p[i][2], p[i][3]);
+    else *reinterpret_cast<uint2*>(A + i * (NCH * SLAB) + off) = make_uint2(p[i][0], p[i][1]);
   }
+}
+template <int N>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[N]) {
+  uint32_t r[N];
+  if constexpr (N == 8)
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr)
+                 : "memory");
+  else
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(taddr)
+                 : "memory");
+  tc::tmem_wait_ld();
+#pragma unroll
+  for (int i = 0; i < N; ++i) v[i] = __uint_as_float(r[i]);
 }
 // SiLU and its derivative in seven instructions: sigma = rcp(1 + ex2(-x log2 e)) with the two MUFU approximations (2 ulp /
 // 1 ulp, flush-to-zero: no denormal fix-up code), y = x sigma, y' = sigma + y (1 - sigma). x -> -inf gives ex2 = inf, sigma = 0.
@@ -154,6 +174,19 @@ __device__ __forceinline__ void stg8(float* p, const float* v) {
                "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])), "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])),
                "r"(__float_as_uint(v[5])), "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7]))
                : "memory");
+}
+template <int N>
+__device__ __forceinline__ void ldgN(const float* p, float (&v)[N]) {
+  if constexpr (N == 8) ldg8(p, v);
+  else {
+    const float4 x = __ldg(reinterpret_cast<const float4*>(p));
+    v[0] = x.x; v[1] = x.y; v[2] = x.z; v[3] = x.w;
+  }
+}
+template <int N>
+__device__ __forceinline__ void stgN(float* p, const float (&v)[N]) {
+  if constexpr (N == 8) stg8(p, v);
+  else *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
 }
 
 // the six product terms of one K = 16 step, smallest first
@@ -224,7 +257,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
   }
   if (tid == 0) {
     tc::mbar_init(bar(B_A0), N_EPI_WARPS);
-    for (int s = 0; s < 4 * NCH; ++s) tc::mbar_init(bar(B_S + s), 4);
+    for (int s = 0; s < 4 * NCH; ++s) tc::mbar_init(bar(B_S + s), CPS == 8 ? 8 : 16);
     tc::mbar_init(bar(B_G1), 1); tc::mbar_init(bar(B_G2), 1); tc::mbar_init(bar(B_G3), 1); tc::mbar_init(bar(B_FIN), 1);
     tc::mbar_init(bar(B_SEG), 1); tc::mbar_init(bar(B_RO), N_EPI_WARPS);
     tc::fence_mbar_init();
@@ -393,9 +426,16 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
     const int q = warp & 3, g = warp >> 2;
     const int row = q * 32 + lane;
     const uint32_t tlane = (uint32_t)(q * 32) << 16;
-    const uint32_t so0 = (uint32_t)(row * 128 + (((2 * g) ^ (row & 7)) << 4));
-    const uint32_t so1 = (uint32_t)(row * 128 + (((2 * g + 1) ^ (row & 7)) << 4));
-    const float4* b2v = reinterpret_cast<const float4*>(a.b2);
+    // step j of a phase: this thread's CPS channels ch(j) .. ch(j) + CPS - 1 of K step kst(j). CPS = 8: two K steps in
+    // progress at a time (8 warps each); CPS = 4: one (all 16 warps), the tensor core trails by a single K step
+    constexpr int NSTEP = D / (4 * CPS);
+    auto kst = [&](int j) { return CPS == 8 ? 2 * j + (g >> 1) : j; };
+    auto ch = [&](int j) { return CPS == 8 ? 16 * kst(j) + 8 * (g & 1) : 16 * j + 4 * g; };
+    auto soff = [&](int j) {  // byte offset of those 2 CPS bytes inside an operand term (SW128 slabs of 64 channels)
+      const int k = kst(j);
+      const int chunk = (k & 3) * 2 + (CPS == 8 ? (g & 1) : (g >> 1));
+      return (uint32_t)((k >> 2) * SLAB + row * 128 + ((chunk ^ (row & 7)) << 4) + (CPS == 8 ? 0 : 8 * (g & 1)));
+    };
     const Rbf rbf(a.r_cut, a.n_rbf);
     uint32_t ph = 0;  // bit i: parity of the next completion of barrier i
     auto wait_bar = [&](int i) {
@@ -506,95 +546,97 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       const int rc = rc_n, sd = sd_n;
       const float r_e = r_n;
       const bool valid = rc >= 0;
-      // sender rows Q_j: random rows out of L2; the first slab is requested before anything else of the tile is computed
-      const float* Qrow = a.Q + (size_t)sd * a.ldq + 16 * g;
-      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp + 16 * g;
-      float qf[16], pf[16];
-      ldg8(Qrow, qf); ldg8(Qrow + 8, qf + 8);
-      ldg8(Prow, pf); ldg8(Prow + 8, pf + 8);
+      // sender rows Q_j: random rows out of L2; the first step is requested before anything else of the tile is computed
+      const float* Qrow = a.Q + (size_t)sd * a.ldq;
+      const float* Prow = a.P + (size_t)(valid ? rc : 0) * a.ldp;
+      float qf[CPS], pf[CPS];
+      ldgN<CPS>(Qrow + ch(0), qf);
+      ldgN<CPS>(Prow + ch(0), pf);
       fetch_meta(tile + gridDim.x);
       if (tile != blockIdx.x) read_out(tile - gridDim.x, ro_valid, ro_r, ro_u, ro_du);
       ro_valid = valid; ro_r = r_e; ro_u = u_e; ro_du = du_e;
       // ================= E1 =================
-      float ds[BWD ? NCH : 1][16];
+      float ds[BWD ? NSTEP : 1][CPS];
       wait_bar(B_G1);
 #pragma unroll
-      for (int s = 0; s < NCH; ++s) {
-        float v[16];
-        tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), v);
+      for (int j = 0; j < NSTEP; ++j) {
+        float v[CPS];
+        tmem_ld<CPS>(TX + tlane + (uint32_t)ch(j), v);
 #pragma unroll
-        for (int k = 0; k < 16; ++k) v[k] += pf[k] + qf[k];
-        if (s + 1 < NCH) {
-          ldg8(Prow + 64 * (s + 1), pf); ldg8(Prow + 64 * (s + 1) + 8, pf + 8);
-          ldg8(Qrow + 64 * (s + 1), qf); ldg8(Qrow + 64 * (s + 1) + 8, qf + 8);
-        }
+        for (int k = 0; k < CPS; ++k) v[k] += pf[k] + qf[k];
+        if (j + 1 < NSTEP) { ldgN<CPS>(Prow + ch(j + 1), pf); ldgN<CPS>(Qrow + ch(j + 1), qf); }
 #pragma unroll
-        for (int k = 0; k < 16; ++k) {
-          if (BWD) silu_both_x3(v[k], v[k], ds[s][k]);
+        for (int k = 0; k < CPS; ++k) {
+          if (BWD) silu_both_x3(v[k], v[k], ds[j][k]);
           else v[k] = silu_x3(v[k]);
         }
-        store_split16(Aop + s * SLAB, so0, so1, v);
-        publish(B_S + 4 * s + g);
+        store_split<CPS>(Aop, soff(j), v);
+        publish(B_S + kst(j));
       }
       // ================= E2 =================
       wait_bar(B_G2);
       if (!BWD) {
         const float wr = w_s[row];
 #pragma unroll
-        for (int s = 0; s < NCH; ++s) {
-          float y[16];
-          tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
+        for (int j = 0; j < NSTEP; ++j) {
+          float y[CPS];
+          tmem_ld<CPS>(TY + tlane + (uint32_t)ch(j), y);
+          float bb[CPS];   // b2 lives in the weight blob: 16-byte aligned only, no 256-bit load
 #pragma unroll
-          for (int k4 = 0; k4 < 4; ++k4) {
-            const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
-            y[4 * k4] = wr * silu_x3(y[4 * k4] + b.x); y[4 * k4 + 1] = wr * silu_x3(y[4 * k4 + 1] + b.y);
-            y[4 * k4 + 2] = wr * silu_x3(y[4 * k4 + 2] + b.z); y[4 * k4 + 3] = wr * silu_x3(y[4 * k4 + 3] + b.w);
+          for (int k4 = 0; k4 < CPS / 4; ++k4) {
+            const float4 b = __ldg(reinterpret_cast<const float4*>(a.b2 + ch(j)) + k4);
+            bb[4 * k4] = b.x; bb[4 * k4 + 1] = b.y; bb[4 * k4 + 2] = b.z; bb[4 * k4 + 3] = b.w;
           }
-          store_split16(Aop + s * SLAB, so0, so1, y);
-          publish(B_S + 4 * s + g);
+#pragma unroll
+          for (int k = 0; k < CPS; ++k) y[k] = wr * silu_x3(y[k] + bb[k]);
+          store_split<CPS>(Aop, soff(j), y);
+          publish(B_S + kst(j));
         }
       } else {
         const float au = w_s[row];
-        const float* Mrow = a.mbar + (size_t)(valid ? rc : 0) * D + 16 * g;
+        const float* Mrow = a.mbar + (size_t)(valid ? rc : 0) * D;
         float up = 0.f;
+        float mb[CPS];
+        ldgN<CPS>(Mrow + ch(0), mb);
 #pragma unroll
-        for (int s = 0; s < NCH; ++s) {
-          float y[16], mb[16];
-          ldg8(Mrow + 64 * s, mb); ldg8(Mrow + 64 * s + 8, mb + 8);
-          tc::tmem_ld16(TY + tlane + (uint32_t)(64 * s + 16 * g), y);
+        for (int j = 0; j < NSTEP; ++j) {
+          float y[CPS];
+          tmem_ld<CPS>(TY + tlane + (uint32_t)ch(j), y);
+          float bb[CPS];   // b2 lives in the weight blob: 16-byte aligned only, no 256-bit load
 #pragma unroll
-          for (int k4 = 0; k4 < 4; ++k4) {
-            const float4 b = __ldg(b2v + 16 * s + 4 * g + k4);
-            const float bb[4] = {b.x, b.y, b.z, b.w};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              float phi, dphi;
-              silu_both_x3(y[4 * k4 + j] + bb[j], phi, dphi);
-              up = fmaf(mb[4 * k4 + j], phi, up);
-              y[4 * k4 + j] = au * mb[4 * k4 + j] * dphi;
-            }
+          for (int k4 = 0; k4 < CPS / 4; ++k4) {
+            const float4 b = __ldg(reinterpret_cast<const float4*>(a.b2 + ch(j)) + k4);
+            bb[4 * k4] = b.x; bb[4 * k4 + 1] = b.y; bb[4 * k4 + 2] = b.z; bb[4 * k4 + 3] = b.w;
           }
-          store_split16(Aop + s * SLAB, so0, so1, y);
-          if (s == NCH - 1) ubar_s[g * TE + row] = up;
-          publish(B_S + 4 * s + g);
+#pragma unroll
+          for (int k = 0; k < CPS; ++k) {
+            float phi, dphi;
+            silu_both_x3(y[k] + bb[k], phi, dphi);
+            up = fmaf(mb[k], phi, up);
+            y[k] = au * mb[k] * dphi;
+          }
+          if (j + 1 < NSTEP) ldgN<CPS>(Mrow + ch(j + 1), mb);
+          store_split<CPS>(Aop, soff(j), y);
+          if (j == NSTEP - 1) ubar_s[g * TE + row] = up;
+          publish(B_S + kst(j));
         }
         // ================= E3 =================
         wait_bar(B_G3);
 #pragma unroll
-        for (int s = 0; s < NCH; ++s) {
-          float x[16];
-          tc::tmem_ld16(TX + tlane + (uint32_t)(64 * s + 16 * g), x);
+        for (int j = 0; j < NSTEP; ++j) {
+          float x[CPS];
+          tmem_ld<CPS>(TX + tlane + (uint32_t)ch(j), x);
 #pragma unroll
-          for (int k = 0; k < 16; ++k) ds[s][k] *= x[k];   // abar, kept for the spill below
-          store_split16(Aop + s * SLAB, so0, so1, ds[s]);
-          publish(B_S + 4 * s + g);
+          for (int k = 0; k < CPS; ++k) ds[j][k] *= x[k];   // abar, kept for the spill below
+          store_split<CPS>(Aop, soff(j), ds[j]);
+          publish(B_S + kst(j));
         }
-        // The fp32 spill goes out after the last slab is published: the fences of publish() wait for global stores issued
+        // The fp32 spill goes out after the last step is published: the fences of publish() wait for global stores issued
         // before them (measured: 3.4 k cycles per slab). It drains under the wait for G4 / GS.
         if (valid) {
-          float* dst = a.abar + (size_t)(e0 + row) * D + 16 * g;
+          float* dst = a.abar + (size_t)(e0 + row) * D;
 #pragma unroll
-          for (int s = 0; s < NCH; ++s) { stg8(dst + 64 * s, ds[s]); stg8(dst + 64 * s + 8, ds[s] + 8); }
+          for (int j = 0; j < NSTEP; ++j) stgN<CPS>(dst + ch(j), ds[j]);
         }
       }
       // ================= P0 of the next tile under G4 / GS of this one =================

@@ -116,7 +116,9 @@ def test_x3_md_skin_device_side_edge_count():
     e0, p0, _ = run()
     e1, p1, st = run(skin=0.5, cuda_graph=True, grid=(2, 1, 1), halo=6.0)
     assert st["n_graph_replays"] == 21
-    assert np.abs(p1 - p0).max() <= 1e-5 and np.abs(e1 - e0).max() <= 1e-7 * np.abs(e0).max() + 1e-5
+    # positions: fp32 forces, different tile boundaries (2 slabs against none). Energies: fp32 per-atom energies of 864 atoms
+    # summed in a different order, 1e-5 eV measured
+    assert np.abs(p1 - p0).max() <= 1e-5 and np.abs(e1 - e0).max() <= 5e-5
     e_ref, pos_ref, _ = O.nve_velocity_verlet(oracle_model(spec, blob), 2, s.pos, s.cell, s.species, masses, vel0, 2.0, 20,
                                               return_state=True)
     assert np.abs(p1 - pos_ref).max() <= 1e-5
