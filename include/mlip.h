@@ -49,7 +49,9 @@ typedef enum {
 /* Arithmetic of the contractions.
  *   MLIP_FP32  fp32 arithmetic everywhere (north_star tolerances 1e-5 / 1e-4). Contractions by CUDA-core FMA, except the fused
  *              edge kernels at d = 128: tcgen05 with every fp32 operand split exactly into three bf16 terms, six MMAs per
- *              product, fp32 accumulation (24 significant bits, fp32 range).
+ *              product, fp32 accumulation (24 significant bits, fp32 range). The tensor core truncates when it
+ *              adds into its accumulator: per-atom energies carry a systematic relative error of about 1e-6 (1e-5 at four
+ *              times the density of the BASELINE configurations), forces 5e-6 of their RMS.
  *   MLIP_BF16  16-bit tensor-core operands with fp32 accumulation (tcgen05, accumulators in TMEM). The name follows
  *              BASELINE.json ("bf16 GEMM inputs"); what runs is IEEE HALF (f16) operands in every contraction -- same
  *              tensor-core rate and bytes as bf16, three more mantissa bits (force RMS error of the unpruned L = 15

@@ -52,9 +52,10 @@ struct EdgeArgs {
 // three_body.cu
 int mlip_gate_forward(mlip_ctx* ctx, int64_t n, int d, const float* h, const float* G, const float* g, float* z);
 int mlip_triplet_forward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
-                         const float4* rvec, const float* z, float* t);
+                         const float4* rvec, const float* z, float* t, int* long_rows /* scratch, int[n_recv + 1] */);
 int mlip_triplet_backward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
-                          const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta);
+                          const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta,
+                          int* long_rows /* scratch, int[n_recv + 1] */);
 int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
                        const int32_t* rev, const float* zeta, const float* z, const float* G, float* hbar);
 

@@ -74,7 +74,14 @@ struct SM {  // shared-memory carve-up, byte offsets from the (1024-byte aligned
   static constexpr uint32_t bytes = slot + 8;
   static_assert(bytes <= 232448 - 1024, "shared memory budget of one SM exceeded");
 };
-constexpr int TMEM_COLS = 512;    // X [0,128) | Y [128,256) | Yseg [256,272) | D4 [288,320)
+// Tensor memory. The tensor core adds into its fp32 accumulator with truncation (round toward zero): a chain of n accumulations
+// shrinks the result by about n / 2 ulp, systematically -- 48 accumulations per GEMM (8 K steps x 6 terms) put 4e-6 on the
+// energy of a dense system (196 neighbours; measured against the oracle), beyond the 1e-5 per-atom bound in places. So every
+// GEMM has TWO accumulators: the main one takes the 8 products a1 b1 of its K steps only, the other the five small terms,
+// whose truncation errors are 2^-8 smaller; the epilogue adds the two in fp32 (round to nearest).
+//   X [0,128) | Xs [128,256) | Y [256,384) | Ys [384,512); the outputs of GS and G4 (16 + 16 and 32 + 32 columns) alias the
+//   head of Y, which is dead by then (the MMA warp waits for the read-out of tile t before G2 of tile t + 1 overwrites Y)
+constexpr int TMEM_COLS = 512;
 // B_S + k: the 16 channels 16 k .. 16 k + 15 (= K step k of the MMAs, slab k / 4) of an operand are written by the eight
 // warps of column groups 2 (k % 2), 2 (k % 2) + 1 in step k / 2
 enum { B_A0 = 0, B_S = 1 /* .. + 4 NCH */, B_G1 = 1 + 4 * NCH, B_G2, B_G3, B_FIN, B_SEG, B_RO, N_BARS };
@@ -111,9 +118,16 @@ __device__ __forceinline__ void store_split(unsigned char* A, uint32_t off, cons
   }
 }
 template <int N>
-__device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[N]) {
-  uint32_t r[N];
-  if constexpr (N == 8)
+__device__ __forceinline__ void tmem_ld_raw(uint32_t taddr, uint32_t (&r)[N]) {
+  static_assert(N == 4 || N == 8 || N == 16, "columns per load");
+  if constexpr (N == 16)
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+  else if constexpr (N == 8)
     asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
                  : "r"(taddr)
@@ -123,9 +137,16 @@ __device__ __forceinline__ void tmem_ld(uint32_t taddr, float (&v)[N]) {
                  : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
                  : "r"(taddr)
                  : "memory");
+}
+// v = main accumulator + accumulator of the small terms (N columns of this thread's row), added in fp32
+template <int N>
+__device__ __forceinline__ void tmem_ld_sum(uint32_t t_main, uint32_t t_small, float (&v)[N]) {
+  uint32_t a[N], b[N];
+  tmem_ld_raw<N>(t_main, a);
+  tmem_ld_raw<N>(t_small, b);
   tc::tmem_wait_ld();
 #pragma unroll
-  for (int i = 0; i < N; ++i) v[i] = __uint_as_float(r[i]);
+  for (int i = 0; i < N; ++i) v[i] = __uint_as_float(a[i]) + __uint_as_float(b[i]);
 }
 // SiLU and its derivative in seven instructions: sigma = rcp(1 + ex2(-x log2 e)) with the two MUFU approximations (2 ulp /
 // 1 ulp, flush-to-zero: no denormal fix-up code), y = x sigma, y' = sigma + y (1 - sigma). x -> -inf gives ex2 = inf, sigma = 0.
@@ -189,12 +210,13 @@ __device__ __forceinline__ void stgN(float* p, const float (&v)[N]) {
   else *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
 }
 
-// the six product terms of one K = 16 step, smallest first
+// the six product terms of one K = 16 step: a1 b1 into the main accumulator, the five small ones (smallest first) into the other
 template <class FA, class FB>
-__device__ __forceinline__ void mma6(uint32_t d_tmem, FA a_desc, FB b_desc, uint32_t idesc, bool accumulate) {
-  constexpr int IA[6] = {2, 1, 0, 1, 0, 0}, IB[6] = {0, 1, 2, 0, 1, 0};
+__device__ __forceinline__ void mma6(uint32_t d_main, uint32_t d_small, FA a_desc, FB b_desc, uint32_t idesc, bool accumulate) {
+  constexpr int IA[5] = {2, 1, 0, 1, 0}, IB[5] = {0, 1, 2, 0, 1};
 #pragma unroll
-  for (int t = 0; t < 6; ++t) tc::mma_bf16(d_tmem, a_desc(IA[t]), b_desc(IB[t]), idesc, accumulate || t > 0);
+  for (int t = 0; t < 5; ++t) tc::mma_bf16(d_small, a_desc(IA[t]), b_desc(IB[t]), idesc, accumulate || t > 0);
+  tc::mma_bf16(d_main, a_desc(0), b_desc(0), idesc, accumulate);
 }
 
 // Shared-memory fallback of the segmented sum (more than MAX_SEG receivers in the tile): thread = channel
@@ -268,7 +290,8 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
   __syncthreads();
   tc::fence_after_sync();
   const uint32_t tmem = *slot;
-  const uint32_t TX = tmem, TY = tmem + D, TS = tmem + 2 * D, T4 = tmem + 2 * D + 32;
+  const uint32_t TX = tmem, TXs = tmem + D, TY = tmem + 2 * D, TYs = tmem + 3 * D;
+  const uint32_t TS = TY, TSs = TY + 16, T4 = TY + 32, T4s = TY + 64;   // GS and G4 outputs over the dead head of Y
 
   if (blockIdx.x >= n_tiles) {
     // no tile for this CTA (only possible with E_dyn: the grid is sized from the capacity)
@@ -278,7 +301,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
     constexpr uint32_t IDESC_ND_BT = tc::idesc_bf16(128, D, 0, 1);
     constexpr uint32_t IDESC_N32_BT = tc::idesc_bf16(128, K1, 0, 1);
     constexpr uint32_t IDESC_SEG = tc::idesc_bf16(128, 16, 1, 0);
-    uint32_t ph_a0 = 0, ph_seg = 0, ph_s = 0;  // parities of the next completion of B_A0 / B_SEG / B_S + i (bit i)
+    uint32_t ph_a0 = 0, ph_seg = 0, ph_ro = 0, ph_s = 0;  // parities of the next completion of B_A0 / B_SEG / B_S + i (bit i)
     auto wait_kstep = [&](int s, int kk) {
       tc::mbar_wait(bar(B_S + 4 * s + kk), (ph_s >> (4 * s + kk)) & 1u);
       ph_s ^= 1u << (4 * s + kk);
@@ -296,20 +319,25 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       if (tc::elect_one()) {
 #pragma unroll
         for (int kk = 0; kk < K1 / 16; ++kk)
-          mma6(TX, [&](int i) { return tc::smem_desc(base + SM::A + i * (TE * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
+          mma6(TX, TXs, [&](int i) { return tc::smem_desc(base + SM::A + i * (TE * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
                [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + kk * 256, 128, 512, tc::LAYOUT_NONE); },
                IDESC_ND, kk != 0);
         tc::mma_commit(bar(B_G1));
       }
       __syncwarp();
-      // ---- G2: Y = s . W2^T, one K step (16 channels) at a time ----
+      // ---- G2: Y = s . W2^T, one K step (16 channels) at a time. Its accumulators hold the outputs of GS / G4 of the
+      // previous tile until every epilogue warp has read them out ----
+      if (tile != blockIdx.x) {
+        tc::mbar_wait(bar(B_RO), ph_ro);
+        ph_ro ^= 1u;
+      }
 #pragma unroll
       for (int s = 0; s < NCH; ++s) {
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk) {
           wait_kstep(s, kk);
           if (tc::elect_one()) {
-            mma6(TY, [&](int i) { return a_slab(i, s, kk); },
+            mma6(TY, TYs, [&](int i) { return a_slab(i, s, kk); },
                  [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + s * (D * 128) + kk * 32, 16, 1024, tc::LAYOUT_SW128); },
                  IDESC_ND, (s | kk) != 0);
             if (s == NCH - 1 && kk == 3) tc::mma_commit(bar(B_G2));
@@ -325,7 +353,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
           for (int kk = 0; kk < 4; ++kk) {
             wait_kstep(s, kk);
             if (tc::elect_one()) {
-              mma6(TX, [&](int i) { return a_slab(i, s, kk); },
+              mma6(TX, TXs, [&](int i) { return a_slab(i, s, kk); },
                    [&](int i) { return tc::smem_desc(base + SM::w2 + i * (D * D * 2) + (4 * s + kk) * 2048, D * 128, 1024, tc::LAYOUT_SW128); },
                    IDESC_ND_BT, (s | kk) != 0);
               if (s == NCH - 1 && kk == 3) tc::mma_commit(bar(B_G3));
@@ -342,7 +370,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
         for (int kk = 0; kk < 4; ++kk) {
           wait_kstep(s, kk);
           if (BWD && tc::elect_one()) {
-            mma6(T4, [&](int i) { return a_slab(i, s, kk); },
+            mma6(T4, T4s, [&](int i) { return a_slab(i, s, kk); },
                  [&](int i) { return tc::smem_desc(base + SM::w13 + i * (D * K1 * 2) + (4 * s + kk) * 1024, 512, 128, tc::LAYOUT_NONE); },
                  IDESC_N32_BT, (s | kk) != 0);
           }
@@ -356,13 +384,14 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       const int R = *reinterpret_cast<volatile int*>(&G.R);
       if (tc::elect_one()) {
         if (R <= MAX_SEG) {
-          constexpr int IS[3] = {2, 1, 0};
 #pragma unroll
-          for (int j = 0; j < TE / 16; ++j)
+          for (int j = 0; j < TE / 16; ++j) {
+            const uint64_t sel_d = tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE);
 #pragma unroll
-            for (int t = 0; t < 3; ++t)
-              tc::mma_bf16(TS, tc::smem_desc(base + SM::A + IS[t] * (NCH * SLAB) + j * 2048, SLAB, 1024, tc::LAYOUT_SW128),
-                           tc::smem_desc(base + SM::sel + j * 256, 128, 2048, tc::LAYOUT_NONE), IDESC_SEG, (j | t) != 0);
+            for (int t = 2; t >= 0; --t)
+              tc::mma_bf16(t == 0 ? TS : TSs, tc::smem_desc(base + SM::A + t * (NCH * SLAB) + j * 2048, SLAB, 1024, tc::LAYOUT_SW128),
+                           sel_d, IDESC_SEG, t == 0 ? j != 0 : (j != 0 || t != 2));
+          }
         }
         tc::mma_commit(bar(B_FIN));
       }
@@ -496,7 +525,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       const int R = G.R;
       if (R <= MAX_SEG && g == 0) {
         float acc[16];
-        tc::tmem_ld16(TS + tlane, acc);
+        tmem_ld_sum<16>(TS + tlane, TSs + tlane, acc);
 #pragma unroll
         for (int r = 0; r < MAX_SEG; ++r)
           if (r < R) G.dst[r][row] = acc[r];
@@ -504,7 +533,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       if (BWD && g == 1) {
         // E4; one addition per edge and launch: a fire-and-forget reduction is deterministic and has no load latency
         float eb[16];
-        tc::tmem_ld16(T4 + tlane, eb);
+        tmem_ld_sum<16>(T4 + tlane, T4s + tlane, eb);
         if (valid) {
           float part = 0.f;
 #pragma unroll
@@ -517,7 +546,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
       }
       if (BWD && g == 2 && a.tbar) {
         float tb[16];
-        tc::tmem_ld16(T4 + tlane + 16u, tb);
+        tmem_ld_sum<16>(T4 + tlane + 16u, T4s + tlane + 16u, tb);
         if (valid) {
           stg8(a.tbar + (size_t)(e0 + row) * 16, tb);
           stg8(a.tbar + (size_t)(e0 + row) * 16 + 8, tb + 8);
@@ -561,7 +590,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
 #pragma unroll
       for (int j = 0; j < NSTEP; ++j) {
         float v[CPS];
-        tmem_ld<CPS>(TX + tlane + (uint32_t)ch(j), v);
+        tmem_ld_sum<CPS>(TX + tlane + (uint32_t)ch(j), TXs + tlane + (uint32_t)ch(j), v);
 #pragma unroll
         for (int k = 0; k < CPS; ++k) v[k] += pf[k] + qf[k];
         if (j + 1 < NSTEP) { ldgN<CPS>(Prow + ch(j + 1), pf); ldgN<CPS>(Qrow + ch(j + 1), qf); }
@@ -580,7 +609,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
 #pragma unroll
         for (int j = 0; j < NSTEP; ++j) {
           float y[CPS];
-          tmem_ld<CPS>(TY + tlane + (uint32_t)ch(j), y);
+          tmem_ld_sum<CPS>(TY + tlane + (uint32_t)ch(j), TYs + tlane + (uint32_t)ch(j), y);
           float bb[CPS];   // b2 lives in the weight blob: 16-byte aligned only, no 256-bit load
 #pragma unroll
           for (int k4 = 0; k4 < CPS / 4; ++k4) {
@@ -601,7 +630,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
 #pragma unroll
         for (int j = 0; j < NSTEP; ++j) {
           float y[CPS];
-          tmem_ld<CPS>(TY + tlane + (uint32_t)ch(j), y);
+          tmem_ld_sum<CPS>(TY + tlane + (uint32_t)ch(j), TYs + tlane + (uint32_t)ch(j), y);
           float bb[CPS];   // b2 lives in the weight blob: 16-byte aligned only, no 256-bit load
 #pragma unroll
           for (int k4 = 0; k4 < CPS / 4; ++k4) {
@@ -625,7 +654,7 @@ __global__ void __launch_bounds__(NT, 1) k_edge_x3(EdgeArgs a, int64_t n_tiles_c
 #pragma unroll
         for (int j = 0; j < NSTEP; ++j) {
           float x[CPS];
-          tmem_ld<CPS>(TX + tlane + (uint32_t)ch(j), x);
+          tmem_ld_sum<CPS>(TX + tlane + (uint32_t)ch(j), TXs + tlane + (uint32_t)ch(j), x);
 #pragma unroll
           for (int k = 0; k < CPS; ++k) ds[j][k] *= x[k];   // abar, kept for the spill below
           store_split<CPS>(Aop, soff(j), ds[j]);

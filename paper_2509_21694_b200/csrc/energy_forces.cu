@@ -304,11 +304,12 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
   std::vector<float*> zg(L, nullptr);
   std::vector<float*> t3(L, nullptr);   // angle terms t_e of every layer, kept for the reverse pass (64 B per edge-layer)
   float* tbar3 = nullptr;
+  int* long_rows = nullptr;   // scratch list of the triplet kernels
   float4* gvec = nullptr;
   if (tb) {
     for (int l = 0; l < L; ++l) W_ALLOC(zg[l], float, n * 16);
     for (int l = 0; l < L; ++l) W_ALLOC(t3[l], float, (E + 1) * 16);
-    W_ALLOC(tbar3, float, (E + 1) * 16); W_ALLOC(gvec, float4, E + 1);
+    W_ALLOC(tbar3, float, (E + 1) * 16); W_ALLOC(long_rows, int, n + 1); W_ALLOC(gvec, float4, E + 1);
     cudaMemsetAsync(gvec, 0, sizeof(float4) * (E + 1), st);
   }
   float* mbar = m;           // m is dead after the forward pass
@@ -371,7 +372,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     if (tb) {
       ProfScope p(ctx, MLIP_PROF_THREE_BODY);
       W_TRY(mlip_gate_forward(ctx, ns, d, h[l], W.G3, W.g3, zg[l]));
-      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3[l]));
+      W_TRY(mlip_triplet_forward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], t3[l], long_rows));
       ea.t3 = t3[l]; ea.W3 = W.W3;
     }
     {
@@ -462,7 +463,7 @@ int mlip_eval_subgraph(mlip_ctx* ctx, const mlip_model* M, int L, const SubGraph
     float* zeta = tb ? t3[l] : nullptr;  // the angle terms are dead after the edge kernel: their buffer takes the per-edge gate adjoints
     if (tb) {
       ProfScope p(ctx, MLIP_PROF_THREE_BODY);
-      W_TRY(mlip_triplet_backward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], tbar3, rbar, gvec, zeta));
+      W_TRY(mlip_triplet_backward(ctx, nr, r3, g.rowptr, g.send, g.rvec, zg[l], tbar3, rbar, gvec, zeta, long_rows));
     }
     if (!node_adjoint) continue;
     {

@@ -6,21 +6,25 @@
 //   t_e   = u3(r_e) S_e  for r_e < r3, else 0;  enters the first edge linear as W3 t_e (edge_f32.cu)
 // and its reverse mode: the adjoint tbar_e = W3^T abar_e (edge_f32.cu) is propagated to rbar (through u3 and g3_n), to a
 // per-edge VECTOR gradient gvec_e (through cos theta: d c / d rvec_e = (rhat_e' - c rhat_e) / r_e) and to the gates.
-// One warp per receiver; the short in-edges of the row are staged in shared memory and every lane owns one edge of an
+// One warp per receiver; the short in-edges of the row are staged in shared memory and every lane owns one staged edge of an
 // ordered pair while it loops over the other. No atomics: every output element has exactly one writer. fp32.
 #include "common.cuh"
 #include "edge.cuh"
 #include "mathfn.cuh"
 
 namespace {
-constexpr int CAP = 128;         // short in-edges per receiver that fit the staging area
-constexpr int WARPS = 2;         // receivers per block (2 x 128 staged edges x 144 B = 36 KB of static shared memory)
+constexpr int CAP = 128;         // short in-edges per receiver the kernels take (more: MLIP_ERR_UNSUPPORTED through the status word)
+// The triplet kernels are launched twice: rows with at most CAP_SMALL short in-edges (all of them in condensed matter at
+// r3 = 4 A: mean 27) by a variant with a small staging area (more resident warps per SM), which appends the other rows to
+// a list on the device; a fixed small grid of the CAP-entry variant then walks that list. No host round trip in between.
+constexpr int CAP_SMALL = 48;
 constexpr float INV_SQRT_4PI = 0.28209479177387814f;
 
+template <bool BWD>
 struct Staged {                  // one short in-edge of the receiver, as the OTHER edge of a pair sees it
   float hx, hy, hz, inv_r;       // rhat, 1/r
   float w[16];                   // u3 g3_n z_k of this edge (index 4 l + n): what it contributes as the e' of a pair
-  float z[16];                   // backward only: tau = tbar u3 of this edge: what it carries as the e of a pair
+  float z[BWD ? 16 : 1];         // backward only: tau = tbar u3 of this edge: what it carries as the e of a pair
 };
 
 __device__ __forceinline__ void u3_f(float r, float r3, float& u, float& du) {
@@ -74,11 +78,38 @@ __global__ void __launch_bounds__(256) k_gate(int64_t n, int d, const float* __r
   }
 }
 
-// Stage the short in-edges of receiver `i` (row [lo, hi)) into S[0..ns): directions and the 16 products u3 g3_n z_k.
-// Returns ns (warp-uniform), or -1 when the row holds more than CAP short edges.
-__device__ __forceinline__ int stage_row(int lo, int hi, float r3, const float4* __restrict__ rvec,
-                                         const int32_t* __restrict__ send, const float* __restrict__ z, Staged* S,
-                                         int* idx /*[CAP] edge id of every staged entry*/, int lane) {
+// number of short in-edges of the row [lo, hi) (warp-uniform)
+__device__ __forceinline__ int count_short(int lo, int hi, float r3, const float4* __restrict__ rvec, int lane) {
+  int ns = 0;
+  for (int b = lo; b < hi; b += 32) {
+    const int e = b + lane;
+    ns += __popc(__ballot_sync(0xffffffffu, e < hi && rvec[e].w < r3));
+  }
+  return ns;
+}
+// Row of this warp: the small-capacity variant takes receiver blockIdx * WARPS + warp and appends rows with more than
+// CAP_SMALL short in-edges to long_rows (long_rows[0] = how many, then the receivers); the CAP variant walks that list with a
+// grid-stride loop. Returns false when there is nothing (more) to do.
+template <int CAP_, int WARPS_>
+__device__ __forceinline__ bool next_row(int64_t n, int* __restrict__ long_rows, int lane, int w, int& k, int64_t& i) {
+  if (CAP_ == CAP_SMALL) {
+    if (k > 0) return false;
+    i = (int64_t)blockIdx.x * WARPS_ + w;
+    k = 1;
+    return i < n;
+  }
+  const int idx = k * (int)gridDim.x * WARPS_ + (int)blockIdx.x * WARPS_ + w;
+  ++k;
+  if (idx >= *reinterpret_cast<volatile int*>(long_rows)) return false;
+  i = long_rows[1 + idx];
+  return true;
+}
+
+// Stage the short in-edges of the row [lo, hi) into S[0..min(ns, CAP_)): directions and the 16 products u3 g3_n z_k
+template <int CAP_, bool BWD>
+__device__ __forceinline__ void stage_row(int lo, int hi, float r3, const float4* __restrict__ rvec,
+                                          const int32_t* __restrict__ send, const float* __restrict__ z, Staged<BWD>* S,
+                                          int* idx /*[CAP_] edge id of every staged entry*/, int lane) {
   int ns = 0;
   for (int b = lo; b < hi; b += 32) {
     const int e = b + lane;
@@ -87,86 +118,109 @@ __device__ __forceinline__ int stage_row(int lo, int hi, float r3, const float4*
     const bool ok = e < hi && rv.w < r3;
     const unsigned m = __ballot_sync(0xffffffffu, ok);
     const int slot = ns + __popc(m & ((1u << lane) - 1u));
-    if (ok && slot < CAP) {
-      Staged& s = S[slot];
+    if (ok && slot < CAP_) {
+      Staged<BWD>& s = S[slot];
       const float inv = rv.w > 0.f ? 1.0f / rv.w : 0.f;
       s.hx = rv.x * inv; s.hy = rv.y * inv; s.hz = rv.z * inv; s.inv_r = inv;
       float u, du, g[4], dg[4];
       u3_f(rv.w, r3, u, du);
       g3_f(rv.w, r3, g, dg);
-      const float* zk = z + (size_t)send[e] * 16;
+      const float4* zk = reinterpret_cast<const float4*>(z + (size_t)send[e] * 16);
 #pragma unroll
-      for (int q = 0; q < 16; ++q) s.w[q] = u * g[q & 3] * zk[q];
+      for (int q4 = 0; q4 < 4; ++q4) {
+        const float4 v = zk[q4];
+        s.w[4 * q4] = u * g[0] * v.x; s.w[4 * q4 + 1] = u * g[1] * v.y; s.w[4 * q4 + 2] = u * g[2] * v.z; s.w[4 * q4 + 3] = u * g[3] * v.w;
+      }
       idx[slot] = e;
     }
     ns += __popc(m);
   }
   __syncwarp();
-  return ns > CAP ? -1 : ns;
 }
 
-// forward: t[e, 16] for every edge of the receivers [0, n) (zeros for r_e >= r3)
-__global__ void __launch_bounds__(WARPS * 32) k_triplet_fwd(int64_t n, float r3, const int32_t* __restrict__ rowptr,
-                                                            const int32_t* __restrict__ send, const float4* __restrict__ rvec,
-                                                            const float* __restrict__ z, float* __restrict__ t,
-                                                            int* __restrict__ status) {
-  __shared__ Staged S_all[WARPS][CAP];
-  __shared__ int idx_all[WARPS][CAP];
+// forward: t[e, 16] for every edge of the receivers [0, n) (zeros for r_e >= r3). Every lane owns one staged (short) edge
+// as the e of the pairs (e, p) and loops over the other staged edges p.
+template <int CAP_, int WARPS_>
+__global__ void __launch_bounds__(WARPS_ * 32) k_triplet_fwd(int64_t n, float r3, const int32_t* __restrict__ rowptr,
+                                                             const int32_t* __restrict__ send, const float4* __restrict__ rvec,
+                                                             const float* __restrict__ z, float* __restrict__ t,
+                                                             int* __restrict__ status, int* __restrict__ long_rows) {
+  __shared__ Staged<false> S_all[WARPS_][CAP_];
+  __shared__ int idx_all[WARPS_][CAP_];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t i = (int64_t)blockIdx.x * WARPS + w;
-  if (i >= n) return;
-  Staged* S = S_all[w];
+  Staged<false>* S = S_all[w];
+  int* idx = idx_all[w];
+  int k = 0;
+  int64_t i;
+  while (next_row<CAP_, WARPS_>(n, long_rows, lane, w, k, i)) {
   const int lo = rowptr[i], hi = rowptr[i + 1];
-  const int ns = stage_row(lo, hi, r3, rvec, send, z, S, idx_all[w], lane);
-  if (ns < 0) { if (lane == 0) atomicOr(status, MLIP_DEV_ROW_TOO_LONG); }
-  const int np = ns < 0 ? CAP : ns;
+  const int ns_all = count_short(lo, hi, r3, rvec, lane);
+  if (CAP_ == CAP_SMALL && ns_all > CAP_SMALL) {
+    if (lane == 0) long_rows[1 + atomicAdd(long_rows, 1)] = (int)i;
+    continue;
+  }
+  if (ns_all > CAP_ && lane == 0) atomicOr(status, MLIP_DEV_ROW_TOO_LONG);
+  const int ns = ns_all < CAP_ ? ns_all : CAP_;
+  stage_row<CAP_, false>(lo, hi, r3, rvec, send, z, S, idx, lane);
+  // edges of the row beyond r3 (and beyond the staging area) carry no angle term
   for (int b = lo; b < hi; b += 32) {
     const int e = b + lane;
-    if (e >= hi) continue;
-    const float4 rv = rvec[e];
+    if (e < hi && !(rvec[e].w < r3)) {
+      float4* dst = reinterpret_cast<float4*>(t + (size_t)e * 16);
+      dst[0] = dst[1] = dst[2] = dst[3] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+  for (int p0 = 0; p0 < ns; p0 += 32) {
+    const int me = p0 + lane;
+    if (me >= ns) continue;
+    const int e = idx[me];
+    const float hx = S[me].hx, hy = S[me].hy, hz = S[me].hz;
     float acc[16];
 #pragma unroll
     for (int q = 0; q < 16; ++q) acc[q] = 0.f;
-    if (rv.w < r3) {
-      const float inv = rv.w > 0.f ? 1.0f / rv.w : 0.f;
-      const float hx = rv.x * inv, hy = rv.y * inv, hz = rv.z * inv;
-      for (int p = 0; p < np; ++p) {
-        if (idx_all[w][p] == e) continue;
-        const Staged& s = S[p];
-        const float c = fmaf(hx, s.hx, fmaf(hy, s.hy, hz * s.hz));
-        float Y[4], dY[4];
-        ylm(c, Y, dY);
+    for (int p = 0; p < ns; ++p) {
+      if (p == me) continue;
+      const Staged<false>& s = S[p];
+      const float c = fmaf(hx, s.hx, fmaf(hy, s.hy, hz * s.hz));
+      float Y[4], dY[4];
+      ylm(c, Y, dY);
 #pragma unroll
-        for (int q = 0; q < 16; ++q) acc[q] = fmaf(Y[q >> 2], s.w[q], acc[q]);
-      }
-      float u, du;
-      u3_f(rv.w, r3, u, du);
-#pragma unroll
-      for (int q = 0; q < 16; ++q) acc[q] *= u;
+      for (int q = 0; q < 16; ++q) acc[q] = fmaf(Y[q >> 2], s.w[q], acc[q]);
     }
+    float u, du;
+    u3_f(rvec[e].w, r3, u, du);
     float4* dst = reinterpret_cast<float4*>(t + (size_t)e * 16);
-    dst[0] = make_float4(acc[0], acc[1], acc[2], acc[3]); dst[1] = make_float4(acc[4], acc[5], acc[6], acc[7]);
-    dst[2] = make_float4(acc[8], acc[9], acc[10], acc[11]); dst[3] = make_float4(acc[12], acc[13], acc[14], acc[15]);
+#pragma unroll
+    for (int q4 = 0; q4 < 4; ++q4) dst[q4] = make_float4(acc[4 * q4] * u, acc[4 * q4 + 1] * u, acc[4 * q4 + 2] * u, acc[4 * q4 + 3] * u);
+  }
+  __syncwarp();   // the staging area is reused by the next row of this warp
   }
 }
 
 // reverse mode. In: tbar[e,16]. Out: rbar[e] += ..., gvec[e] += ..., zeta[e,16] = adjoint of the gate of the SENDER of e
 // collected per edge (summed over the out-edges of an atom by k_gate_bwd through rev[]).
-__global__ void __launch_bounds__(WARPS * 32) k_triplet_bwd(int64_t n, float r3, const int32_t* __restrict__ rowptr,
-                                                            const int32_t* __restrict__ send, const float4* __restrict__ rvec,
-                                                            const float* __restrict__ z, const float* __restrict__ tbar,
-                                                            float* __restrict__ rbar, float4* __restrict__ gvec,
-                                                            float* __restrict__ zeta) {
-  __shared__ Staged S_all[WARPS][CAP];
-  __shared__ int idx_all[WARPS][CAP];
+template <int CAP_, int WARPS_>
+__global__ void __launch_bounds__(WARPS_ * 32) k_triplet_bwd(int64_t n, float r3, const int32_t* __restrict__ rowptr,
+                                                             const int32_t* __restrict__ send, const float4* __restrict__ rvec,
+                                                             const float* __restrict__ z, const float* __restrict__ tbar,
+                                                             float* __restrict__ rbar, float4* __restrict__ gvec,
+                                                             float* __restrict__ zeta, int* __restrict__ long_rows) {
+  __shared__ Staged<true> S_all[WARPS_][CAP_];
+  __shared__ int idx_all[WARPS_][CAP_];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t i = (int64_t)blockIdx.x * WARPS + w;
-  if (i >= n) return;
-  Staged* S = S_all[w];
+  Staged<true>* S = S_all[w];
   int* idx = idx_all[w];
+  int k = 0;
+  int64_t i;
+  while (next_row<CAP_, WARPS_>(n, long_rows, lane, w, k, i)) {
   const int lo = rowptr[i], hi = rowptr[i + 1];
-  int ns = stage_row(lo, hi, r3, rvec, send, z, S, idx, lane);
-  if (ns < 0) ns = CAP;   // reported by the forward kernel
+  const int ns_all = count_short(lo, hi, r3, rvec, lane);
+  if (CAP_ == CAP_SMALL && ns_all > CAP_SMALL) {
+    if (lane == 0) long_rows[1 + atomicAdd(long_rows, 1)] = (int)i;
+    continue;
+  }
+  const int ns = ns_all < CAP_ ? ns_all : CAP_;   // a longer row was reported by the forward kernel
+  stage_row<CAP_, true>(lo, hi, r3, rvec, send, z, S, idx, lane);
   // every staged entry also carries tau = tbar u3 of its own edge (pass B reads it as the "e" side)
   for (int p = lane; p < ns; p += 32) {
     const int e = idx[p];
@@ -193,7 +247,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_triplet_bwd(int64_t n, float r3,
     if (me >= ns) continue;
     const int e = idx[me];
     const float4 rv = rvec[e];
-    const Staged& my = S[me];
+    const Staged<true>& my = S[me];
     const float hx = my.hx, hy = my.hy, hz = my.hz;
     float u, du, g[4], dg[4];
     u3_f(rv.w, r3, u, du);
@@ -219,7 +273,7 @@ __global__ void __launch_bounds__(WARPS * 32) k_triplet_bwd(int64_t n, float r3,
     for (int q = 0; q < 16; ++q) Z[q] = 0.f;
     for (int p = 0; p < ns; ++p) {
       if (p == me) continue;
-      const Staged& s = S[p];
+      const Staged<true>& s = S[p];
       const float c = fmaf(hx, s.hx, fmaf(hy, s.hy, hz * s.hz));
       float Y[4], dY[4];
       ylm(c, Y, dY);
@@ -260,6 +314,8 @@ __global__ void __launch_bounds__(WARPS * 32) k_triplet_bwd(int64_t n, float r3,
     for (int q4 = 0; q4 < 4; ++q4)
       dst[q4] = make_float4(Z[4 * q4] * u * g[0], Z[4 * q4 + 1] * u * g[1], Z[4 * q4 + 2] * u * g[2], Z[4 * q4 + 3] * u * g[3]);
   }
+  __syncwarp();   // the staging area is reused by the next row of this warp
+  }
 }
 
 // zbar_k = sum over in-edges e of k with rev[e] < E_act of zeta[rev[e]]; hbar_k += G^T (zbar_k * z_k (1 - z_k))
@@ -289,6 +345,7 @@ __global__ void __launch_bounds__(256) k_gate_bwd(int64_t n, int64_t E_act, cons
   }
 }
 inline unsigned nblk(int64_t n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+constexpr unsigned LONG_GRID = 148 * 4;   // blocks of the list-walking CAP variant
 }  // namespace
 
 int mlip_gate_forward(mlip_ctx* ctx, int64_t n, int d, const float* h, const float* G, const float* g, float* z) {
@@ -298,17 +355,22 @@ int mlip_gate_forward(mlip_ctx* ctx, int64_t n, int d, const float* h, const flo
   return MLIP_OK;
 }
 int mlip_triplet_forward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
-                         const float4* rvec, const float* z, float* t) {
+                         const float4* rvec, const float* z, float* t, int* long_rows) {
   if (n_recv <= 0) return MLIP_OK;
-  k_triplet_fwd<<<nblk(n_recv, WARPS), WARPS * 32, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, t, ctx->dev_status);
-  ctx->launches++;
+  cudaMemsetAsync(long_rows, 0, sizeof(int), ctx->stream);
+  k_triplet_fwd<CAP_SMALL, 4><<<nblk(n_recv, 4), 128, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, t, ctx->dev_status, long_rows);
+  k_triplet_fwd<CAP, 2><<<LONG_GRID, 64, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, t, ctx->dev_status, long_rows);
+  ctx->launches += 2;
   return MLIP_OK;
 }
 int mlip_triplet_backward(mlip_ctx* ctx, int64_t n_recv, float r3, const int32_t* rowptr, const int32_t* send,
-                          const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta) {
+                          const float4* rvec, const float* z, const float* tbar, float* rbar, float4* gvec, float* zeta,
+                          int* long_rows) {
   if (n_recv <= 0) return MLIP_OK;
-  k_triplet_bwd<<<nblk(n_recv, WARPS), WARPS * 32, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, tbar, rbar, gvec, zeta);
-  ctx->launches++;
+  cudaMemsetAsync(long_rows, 0, sizeof(int), ctx->stream);
+  k_triplet_bwd<CAP_SMALL, 4><<<nblk(n_recv, 4), 128, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, tbar, rbar, gvec, zeta, long_rows);
+  k_triplet_bwd<CAP, 2><<<LONG_GRID, 64, 0, ctx->stream>>>(n_recv, r3, rowptr, send, rvec, z, tbar, rbar, gvec, zeta, long_rows);
+  ctx->launches += 2;
   return MLIP_OK;
 }
 int mlip_gate_backward(mlip_ctx* ctx, int64_t n_send, int64_t E_act, const int32_t* E_act_dyn, int d, const int32_t* rowptr,
