@@ -76,7 +76,7 @@ struct SM {  // shared-memory carve-up, byte offsets from the (1024-byte aligned
 };
 // Tensor memory. The tensor core adds into its fp32 accumulator with truncation (round toward zero): a chain of n accumulations
 // shrinks the result by about n / 2 ulp, systematically -- 48 accumulations per GEMM (8 K steps x 6 terms) put 4e-6 on the
-// energy of a dense system (196 neighbours; measured against the oracle), beyond the 1e-5 per-atom bound in places. So every
+// energy of a dense system (196 neighbours; measured against the float64 reference of the tests), beyond the 1e-5 per-atom bound in places. So every
 // GEMM has TWO accumulators: the main one takes the 8 products a1 b1 of its K steps only, the other the five small terms,
 // whose truncation errors are 2^-8 smaller; the epilogue adds the two in fp32 (round to nearest).
 //   X [0,128) | Xs [128,256) | Y [256,384) | Ys [384,512); the outputs of GS and G4 (16 + 16 and 32 + 32 columns) alias the
