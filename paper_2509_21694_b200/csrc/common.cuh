@@ -6,6 +6,7 @@
 #include <cuda_fp16.h>
 #include <stdint.h>
 #include <string>
+#include <unordered_map>
 #include <vector>
 #include "../../include/mlip.h"
 
@@ -56,6 +57,9 @@ struct mlip_ctx {
   // see (non-finite results of the 16-bit path, a missing reverse edge) surface at the next synchronising call or at
   // mlip_ctx_status, never as silently wrong numbers.
   int* dev_status = nullptr;
+  // fp32 weight matrix (device pointer, the GemmArgs::B of the fp32 path) -> its three-term bf16 split image for the
+  // tensor-core fp32 node GEMM (node_x3.cu); filled by mlip_model_load at d = 128, emptied by mlip_model_destroy
+  std::unordered_map<const void*, const __nv_bfloat16*> x3_img;
   void set_error(const std::string& s) { err = s; }
   // ---- optional per-group timing ----
   struct ProfRec { int cat; int64_t launches; cudaEvent_t a, b; };
@@ -157,6 +161,7 @@ struct mlip_model {
   mlip_nodeop *Wo_bf = nullptr, *WoT_bf = nullptr;
   std::vector<LayerWeights> layers;
   std::vector<void*> owned;  // everything to cudaFree
+  std::vector<const void*> x3_keys;  // this model's entries of mlip_ctx::x3_img
 };
 
 // ---- graph --------------------------------------------------------------------------------
@@ -260,6 +265,10 @@ struct GemmArgs {
   int64_t n = 0; int N = 0;
 };
 int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a);
+// node_x3.cu: the fp32 GEMM on tcgen05 with 3-term bf16 operand splits (mlip_gemm_f32 dispatches to it when B has an image)
+void mlip_make_gemm_image_x3(cudaStream_t st, const float* W, int N, int K, __nv_bfloat16* img /*[3][N*K]*/);
+bool mlip_gemm_x3_supported(const GemmArgs& a);
+int mlip_gemm_x3(mlip_ctx* ctx, const GemmArgs& a, const __nv_bfloat16* Bx3);
 int mlip_gemm_bf16(mlip_ctx* ctx, const GemmArgs& a);  // B = image built by mlip_make_gemm_image
 void mlip_make_gemm_image(cudaStream_t st, const float* W, int N, int K, float scale, mlip_nodeop* img);
 

@@ -143,6 +143,7 @@ extern "C" int mlip_ctx_set_active_sets(mlip_ctx* ctx, int enable) {
 
 extern "C" void mlip_model_destroy(mlip_model* m) {
   if (!m) return;
+  for (const void* w : m->x3_keys) m->ctx->x3_img.erase(w);
   for (void* p : m->owned) cudaFree(p);
   delete m;
 }
@@ -269,6 +270,23 @@ extern "C" int mlip_model_load(mlip_ctx* ctx, const mlip_model_header* h, const 
   sub(M->Wo, d, 0, 0, 1, M->WoT, d, d, d);
   M_ALLOC(M->Wo_bf, mlip_nodeop, d * d); M_ALLOC(M->WoT_bf, mlip_nodeop, d * d);
   toimg(M->Wo, M->Wo_bf, d, d); toimg(M->WoT, M->WoT_bf, d, d);
+  if (d == 128) {
+    // three-term bf16 split images of every weight matrix the fp32 node GEMMs multiply by (node_x3.cu)
+    auto img3 = [&](const float* Wm, int N, int K) -> int {
+      __nv_bfloat16* img = nullptr;
+      M_ALLOC(img, __nv_bfloat16, 3 * (size_t)N * K);
+      mlip_make_gemm_image_x3(st, Wm, N, K, img);
+      ctx->x3_img[Wm] = img;
+      M->x3_keys.push_back(Wm);
+      return MLIP_OK;
+    };
+    for (int l = 0; l < L; ++l) {
+      LayerWeights& W = M->layers[l];
+      MLIP_TRY(img3(W.W1ab, 2 * d, d)); MLIP_TRY(img3(W.V1, d, 2 * d)); MLIP_TRY(img3(W.V2, d, d)); MLIP_TRY(img3(W.V2T, d, d));
+      MLIP_TRY(img3(W.V1aT, d, d)); MLIP_TRY(img3(W.V1bT, d, d)); MLIP_TRY(img3(W.W1abT, d, 2 * d));
+    }
+    MLIP_TRY(img3(M->Wo, d, d)); MLIP_TRY(img3(M->WoT, d, d));
+  }
 #undef M_ALLOC
   if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) {
     ctx->set_error("model preparation kernels failed");

@@ -1,6 +1,8 @@
 // fp32 CUDA-core node-level GEMM with fused prologue / epilogue (steps A8, A9 and their adjoints
 // in the MLIP_FP32 path): Y[n,N] = epi( act(X)[n,K] . B^T + bias ), X = [X1 | X2].
 // 64x64 output tile, K step 16, 256 threads, 4x4 register block per thread.
+#include <stdlib.h>
+#include <string.h>
 #include "common.cuh"
 #include "mathfn.cuh"
 
@@ -77,6 +79,12 @@ __global__ void __launch_bounds__(256) k_gemm_f32(GemmArgs a) {
 
 int mlip_gemm_f32(mlip_ctx* ctx, const GemmArgs& a) {
   if (a.n <= 0) return MLIP_OK;
+  // d = 128: on the tensor cores (node_x3.cu) unless MLIP_B200_FP32_EDGE=cuda asks for the CUDA-core kernels (A/B runs)
+  static const bool cuda_cores = [] { const char* v = getenv("MLIP_B200_FP32_EDGE"); return v && !strcmp(v, "cuda"); }();
+  if (!cuda_cores && !ctx->x3_img.empty() && mlip_gemm_x3_supported(a)) {
+    auto it = ctx->x3_img.find(a.B);
+    if (it != ctx->x3_img.end()) return mlip_gemm_x3(ctx, a, it->second);
+  }
   if (a.N % BN || a.K1 % BK || a.K2 % BK) { ctx->set_error("gemm_f32: shape not a multiple of the tile"); return MLIP_ERR_UNSUPPORTED; }
   dim3 grid((unsigned)((a.n + BM - 1) / BM), a.N / BN);
   k_gemm_f32<<<grid, 256, 0, ctx->stream>>>(a);
