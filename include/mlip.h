@@ -47,8 +47,8 @@ typedef enum {
 } mlip_status;
 
 /* Arithmetic of the contractions.
- *   MLIP_FP32  fp32 arithmetic everywhere (north_star tolerances 1e-5 / 1e-4). Contractions by CUDA-core FMA, except the fused
- *              edge kernels at d = 128: tcgen05 with every fp32 operand split exactly into three bf16 terms, six MMAs per
+ *   MLIP_FP32  fp32 arithmetic everywhere (north_star tolerances 1e-5 / 1e-4). Contractions by CUDA-core FMA, except at
+ *              d = 128 (fused edge kernels and node GEMMs): tcgen05 with every fp32 operand split exactly into three bf16 terms, six MMAs per
  *              product, fp32 accumulation (24 significant bits, fp32 range). The tensor core truncates when it
  *              adds into its accumulator: per-atom energies carry a systematic relative error of about 1e-6 (1e-5 at four
  *              times the density of the BASELINE configurations), forces 5e-6 of their RMS.
