@@ -289,7 +289,8 @@ def run_ours(args):
 
     def step(collect=False):
         g = mlip.Graph(ctx, pos, s.cell, species, m.r_cut)
-        part = mlip.Partition(ctx, g, cfg.halo, grid=cfg.grid) if partitioned else None
+        # N > 1: every rank builds its own sub-domains only (mlip_partition_grid_shard)
+        part = mlip.Partition(ctx, g, cfg.halo, grid=cfg.grid, shard=rank, n_shards=world) if partitioned else None
         if world > 1:
             E, F, _ = mlip.energy_forces_shard(ctx, model, cfg.L, g, part, rank, world, prec, out=out)
             all_reduce_results(E, F)

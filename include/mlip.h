@@ -152,6 +152,13 @@ void mlip_graph_destroy(mlip_graph* g);
 int mlip_partition(mlip_ctx* ctx, const mlip_graph* g, int n_sub, double halo, mlip_part** out);
 int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* g, const int grid[3], double halo,
                         mlip_part** out);
+/* mlip_partition_grid for ONE shard of a multi-GPU run: only the sub-domains k with k mod n_shards == shard
+ * (k = (bx * gy + by) * gz + bz, the dealing rule of mlip_energy_forces_shard) are built; the others keep their index
+ * and stay empty (mlip_part_info reports zeros), so that a rank spends partition time and memory on its own
+ * sub-domains only. The handle must be evaluated by mlip_energy_forces_shard / _stress with the same (shard,
+ * n_shards); anything else is refused with MLIP_ERR_INVALID_ARG. */
+int mlip_partition_grid_shard(mlip_ctx* ctx, const mlip_graph* g, const int grid[3], double halo, int shard,
+                              int n_shards, mlip_part** out);
 int mlip_part_count(const mlip_part* p, int* n_sub);
 /* Sizes of sub-domain s: root (owned) atoms, extended atoms, induced directed edges. The halo
  * growth factor of PAPER.md:289 is (n_ext - n_owned) / n_owned. */

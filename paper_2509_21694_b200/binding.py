@@ -76,6 +76,7 @@ def load_library():
     lib.mlip_graph_destroy.argtypes = [vp]; lib.mlip_graph_destroy.restype = None
     lib.mlip_partition.argtypes = [vp, vp, i32, dbl, P(vp)]
     lib.mlip_partition_grid.argtypes = [vp, vp, P(i32), dbl, P(vp)]
+    lib.mlip_partition_grid_shard.argtypes = [vp, vp, P(i32), dbl, i32, i32, P(vp)]
     lib.mlip_part_count.argtypes = [vp, P(i32)]
     lib.mlip_part_info.argtypes = [vp, i32, P(i64), P(i64), P(i64)]
     lib.mlip_part_layer_info.argtypes = [vp, i32, i32, i32, P(i64), P(i64), P(i64)]
@@ -227,13 +228,18 @@ class Graph:
 
 
 class Partition:
-    """mlip_partition (n_sub slabs) or mlip_partition_grid (grid=(gx,gy,gz))."""
+    """mlip_partition (n_sub slabs), mlip_partition_grid (grid=(gx,gy,gz)) or, with n_shards > 1, mlip_partition_grid_shard
+    (only the sub-domains k with k mod n_shards == shard are built)."""
 
-    def __init__(self, ctx: Context, graph: Graph, halo: float, n_sub: int | None = None, grid=None):
+    def __init__(self, ctx: Context, graph: Graph, halo: float, n_sub: int | None = None, grid=None, shard: int = 0,
+                 n_shards: int = 1):
         self.ctx = ctx
         self.graph = graph
         h = C.c_void_p()
-        if grid is not None:
+        if grid is not None and n_shards > 1:
+            g = (C.c_int * 3)(*[int(x) for x in grid])
+            ctx.check(ctx.lib.mlip_partition_grid_shard(ctx.h, graph.h, g, float(halo), int(shard), int(n_shards), C.byref(h)))
+        elif grid is not None:
             g = (C.c_int * 3)(*[int(x) for x in grid])
             ctx.check(ctx.lib.mlip_partition_grid(ctx.h, graph.h, g, float(halo), C.byref(h)))
         else:

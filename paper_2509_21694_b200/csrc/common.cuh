@@ -235,11 +235,12 @@ struct mlip_part {
   double halo = 0;
   bool khop = false;  // classes are hop counts (K-hop search) rather than geometric shells
   int64_t N = 0;
+  int shard = 0, n_shards = 1;  // mlip_partition_grid_shard: only sub-domains k with k mod n_shards == shard were built
   std::vector<PartSub> subs;
 };
 
 int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo_box, double halo,
-                           double r_class, bool force_khop, bool keep_geid, mlip_part** out);
+                           double r_class, bool force_khop, bool keep_geid, mlip_part** out, int shard = 0, int n_shards = 1);
 
 // ---- launchers (each bumps ctx->launches by the number of kernels it enqueues) ---------------
 // scan.cu

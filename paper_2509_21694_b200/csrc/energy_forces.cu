@@ -531,6 +531,11 @@ static int energy_forces_impl(mlip_ctx* ctx, const mlip_model* M, int L, const m
   if (!ctx) return MLIP_ERR_INVALID_ARG;
   if (n_shards < 1 || shard < 0 || shard >= n_shards) { ctx->set_error("shard outside [0, n_shards)"); return MLIP_ERR_INVALID_ARG; }
   if (n_shards > 1 && !part) { ctx->set_error("sharded evaluation needs a partition"); return MLIP_ERR_INVALID_ARG; }
+  if (part && part->n_shards > 1 && (part->n_shards != n_shards || part->shard != shard)) {
+    ctx->set_error("this partition was built for shard " + std::to_string(part->shard) + " of " + std::to_string(part->n_shards) +
+                   " (mlip_partition_grid_shard): evaluate it with the same shard and n_shards");
+    return MLIP_ERR_INVALID_ARG;
+  }
   if (!M || !G || !energy_dev || (G->N > 0 && !forces_dev)) { ctx->set_error("mlip_energy_forces: null argument"); return MLIP_ERR_INVALID_ARG; }
   if (L < 0 || L > M->h.L_max) { ctx->set_error("L outside [0, L_max]"); return MLIP_ERR_UNSUPPORTED; }
   if (precision != MLIP_FP32 && precision != MLIP_BF16) { ctx->set_error("unknown precision"); return MLIP_ERR_INVALID_ARG; }

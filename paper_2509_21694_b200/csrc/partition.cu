@@ -164,8 +164,9 @@ extern "C" int mlip_partition_grid(mlip_ctx* ctx, const mlip_graph* G, const int
 // rule (hop counts over the candidate graph are lower bounds of the hop counts over any later exact graph) and keeps the
 // global edge id of every sub-domain edge.
 int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo_box, double halo,
-                           double r_class, bool force_khop, bool keep_geid, mlip_part** out) {
+                           double r_class, bool force_khop, bool keep_geid, mlip_part** out, int shard, int n_shards) {
   if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (n_shards < 1 || shard < 0 || shard >= n_shards) { ctx->set_error("mlip_partition_grid_shard: shard outside [0, n_shards)"); return MLIP_ERR_INVALID_ARG; }
   if (!G || !grid || !out || grid[0] < 1 || grid[1] < 1 || grid[2] < 1 || !(halo >= 0.0) || !(halo_box >= halo) || !(r_class > 0.0)) {
     ctx->set_error("mlip_partition_grid: invalid argument");
     return MLIP_ERR_INVALID_ARG;
@@ -175,7 +176,7 @@ int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3]
   cudaStream_t st = ctx->stream;
   const int64_t N = G->N;
   mlip_part* P = new mlip_part();
-  P->ctx = ctx; P->halo = halo; P->N = N;
+  P->ctx = ctx; P->halo = halo; P->N = N; P->shard = shard; P->n_shards = n_shards;
   for (int k = 0; k < 3; ++k) P->grid[k] = grid[k];
   auto fail = [&](int code) { mlip_part_destroy(P); return code; };
   ProfScope prof(ctx, MLIP_PROF_PARTITION);
@@ -206,6 +207,8 @@ int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3]
         }
         P->subs.emplace_back();
         PartSub& S = P->subs.back();
+        // sub-domains of other shards stay empty handles: their place in the numbering k = (bx, by, bz) is kept
+        if ((int)((P->subs.size() - 1) % (size_t)n_shards) != shard) continue;
         int64_t n_ext = 0, E = 0;
         int32_t cls_start[MLIP_MAX_CLS + 1] = {0}, E_at[MLIP_MAX_CLS] = {0};
         cudaMemsetAsync(ext, 0, sizeof(int32_t) * (CN + 1), st);
@@ -271,6 +274,13 @@ int mlip_partition_grid_ex(mlip_ctx* ctx, const mlip_graph* G, const int grid[3]
 #undef P_TRY
   *out = P;
   return MLIP_OK;
+}
+
+extern "C" int mlip_partition_grid_shard(mlip_ctx* ctx, const mlip_graph* G, const int grid[3], double halo, int shard,
+                                         int n_shards, mlip_part** out) {
+  if (!ctx) return MLIP_ERR_INVALID_ARG;
+  if (!G) { ctx->set_error("mlip_partition_grid_shard: invalid argument"); return MLIP_ERR_INVALID_ARG; }
+  return mlip_partition_grid_ex(ctx, G, grid, halo, halo, G->r_cut, false, false, out, shard, n_shards);
 }
 
 extern "C" int mlip_partition(mlip_ctx* ctx, const mlip_graph* G, int n_sub, double halo, mlip_part** out) {

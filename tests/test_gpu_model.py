@@ -410,3 +410,40 @@ def test_degenerate_systems(precision, d):
     assert abs(E - ref[0]) <= tolE * np.abs(ref[1]).sum()
     # the net force is what is left of much larger image contributions that cancel: the bf16 path is held to an absolute bound
     assert np.abs(F - ref[2]).max() <= tolF * max(rms(ref[2]), 1e-6) + (1e-6 if precision == 0 else 1e-4)
+
+
+def test_sharded_partition_builds_only_its_sub_domains_and_sums_to_the_full_result():
+    """mlip_partition_grid_shard (one rank, its sub-domains only): the sub-domains of other shards are empty
+    handles, the partial results of all shards sum to the result of the full partition, and a handle is refused by an
+    evaluation with another (shard, n_shards)."""
+    import torch
+    import paper_2509_21694_b200 as mlip
+    spec = ModelSpec(4, 64, 8, 2, 3.0, 1.0 / np.sqrt(12.0))
+    blob = make_weights(spec, 91)
+    s = small_system(8, 0.08, seed=17)
+    m, ctx, model = gpu_setup(spec, blob)
+    g = gpu_graph(m, ctx, s, spec.r_cut)
+    grid, halo, n_shards = (2, 2, 1), 6.0, 3
+    full = mlip.Partition(ctx, g, halo, grid=grid)
+    E0, F0, Ei0 = gpu_energy_forces(m, ctx, model, 2, g, full, 0)
+    info0 = full.info()
+    E, F, Ei = 0.0, 0.0, 0.0
+    for k in range(n_shards):
+        part = mlip.Partition(ctx, g, halo, grid=grid, shard=k, n_shards=n_shards)
+        info = part.info()
+        assert len(info) == 4
+        for j in range(4):
+            assert info[j] == (info0[j] if j % n_shards == k else dict(n_owned=0, n_ext=0, n_edges=0))
+        e, f, ei = mlip.energy_forces_shard(ctx, model, 2, g, part, k, n_shards, 0, want_atom_energy=True)
+        ctx.status()
+        E += float(e.item()); F = F + f.double().cpu().numpy(); Ei = Ei + ei.double().cpu().numpy()
+        with pytest.raises(mlip.MlipError) as err:
+            mlip.energy_forces_shard(ctx, model, 2, g, part, (k + 1) % n_shards, n_shards, 0)
+        assert err.value.code == -1
+        with pytest.raises(mlip.MlipError) as err:
+            mlip.energy_forces(ctx, model, 2, g, part, 0)
+        assert err.value.code == -1
+    assert abs(E - E0) <= 1e-6 * np.abs(Ei0).sum() and np.abs(F - F0).max() <= 1e-6 * rms(F0) and np.array_equal(Ei, Ei0)
+    with pytest.raises(mlip.MlipError):
+        mlip.Partition(ctx, g, halo, grid=grid, shard=3, n_shards=3)
+
