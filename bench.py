@@ -425,8 +425,9 @@ def run_ours(args):
                "extrapolated_to_workload": el_rate * N / max(edge_layers, 1),
                "extrapolated_note": "sample edge-layers/s x N / edge-layers evaluated per step of this workload"}
 
-    n_own = [x["n_owned"] for x in info["subs"]]
-    n_ext = [x["n_ext"] for x in info["subs"]]
+    own_subs = info["subs"][rank::world] if world > 1 else info["subs"]   # N > 1: a rank builds its own sub-domains only
+    n_own = [x["n_owned"] for x in own_subs]
+    n_ext = [x["n_ext"] for x in own_subs]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
